@@ -1,0 +1,193 @@
+// aux_kernels.cuh -- S0 (sample mask -> lineage queue) and S6 (resolve, radix sort, unique, labels).
+// PAPER.md L2162 (population generation), L958-967 (a-posteriori coalescence: duplicates of an event are
+// adjacent after sorting), L276 / L890-900 (species = distinct speciation events).
+#pragma once
+#include "../../include/necsim.h"
+#include "sim_types.cuh"
+
+namespace necsim {
+
+#define NS_CHUNK 4096u   // mask bytes per block in the compaction kernels (256 threads x 16 bytes)
+
+// cell of an indexed location: last cell with prefix[cell] <= loc (that cell has deme > 0)
+__device__ __forceinline__ u32 cell_of_loc(const ScenarioDev &sc, u32 loc) {
+    if (sc.kind == 0 || sc.kind == 1) return 0;      // non-spatial; implicit: only the local community is sampled
+    if (sc.uniform_deme) return loc / sc.uniform_deme;
+    u32 lo = 0, hi = sc.ncells;                      // invariant: prefix[lo] <= loc < prefix[hi]
+    while (hi - lo > 1) { u32 mid = lo + ((hi - lo) >> 1); if (sc.prefix[mid] <= loc) lo = mid; else hi = mid; }
+    return lo;
+}
+
+// S0, pass 1: number of sampled individuals per chunk
+__global__ void __launch_bounds__(256) mask_count_kernel(const uint8_t *__restrict__ mask, u64 n, u32 *__restrict__ chunk_count) {
+    __shared__ u32 wsum[8];
+    u64 base = (u64)blockIdx.x * NS_CHUNK + (u64)threadIdx.x * 16u;
+    u32 c = 0;
+    for (u32 t = 0; t < 16; ++t) { u64 i = base + t; if (i < n && mask[i]) ++c; }
+    for (int o = 16; o; o >>= 1) c += __shfl_down_sync(NS_FULL, c, o);
+    if ((threadIdx.x & 31) == 0) wsum[threadIdx.x >> 5] = c;
+    __syncthreads();
+    if (threadIdx.x == 0) { u32 s = 0; for (int w = 0; w < 8; ++w) s += wsum[w]; chunk_count[blockIdx.x] = s; }
+}
+
+// exclusive scan of a u32 array by one block (n up to a few 10^5); total -> *total_out (may be NULL)
+__global__ void __launch_bounds__(1024) scan_exclusive_kernel(u32 *__restrict__ a, u32 n, u32 *__restrict__ total_out) {
+    __shared__ u32 wsum[32];
+    __shared__ u32 carry;
+    if (threadIdx.x == 0) carry = 0;
+    __syncthreads();
+    const u32 lane = threadIdx.x & 31u, w = threadIdx.x >> 5;
+    for (u32 start = 0; start < n; start += 1024u) {
+        u32 i = start + threadIdx.x;
+        u32 v = i < n ? a[i] : 0u, x = v;
+        for (int o = 1; o < 32; o <<= 1) { u32 y = __shfl_up_sync(NS_FULL, x, o); if ((int)lane >= o) x += y; }
+        if (lane == 31) wsum[w] = x;
+        __syncthreads();
+        if (w == 0) {
+            u32 s = wsum[lane], t = s;
+            for (int o = 1; o < 32; o <<= 1) { u32 y = __shfl_up_sync(NS_FULL, t, o); if ((int)lane >= o) t += y; }
+            wsum[lane] = t - s;   // exclusive warp offsets
+        }
+        __syncthreads();
+        u32 excl = carry + wsum[w] + (x - v);
+        if (i < n) a[i] = excl;
+        __syncthreads();
+        if (threadIdx.x == 1023) carry = excl + v;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0 && total_out) *total_out = carry;
+}
+
+// S0, pass 2: ordered compaction -> queue entries {id, loc, cell, steps = 0}; id = rank in ascending loc
+__global__ void __launch_bounds__(256) mask_scatter_kernel(const ScenarioDev sc, const uint8_t *__restrict__ mask, u64 n,
+                                                           const u32 *__restrict__ chunk_offset, uint4 *__restrict__ queue, u32 capacity) {
+    __shared__ u32 wsum[8];
+    u64 base = (u64)blockIdx.x * NS_CHUNK + (u64)threadIdx.x * 16u;
+    u32 bits = 0;
+    for (u32 t = 0; t < 16; ++t) { u64 i = base + t; if (i < n && mask[i]) bits |= 1u << t; }
+    u32 c = __popc(bits), x = c;
+    const u32 lane = threadIdx.x & 31u, w = threadIdx.x >> 5;
+    for (int o = 1; o < 32; o <<= 1) { u32 y = __shfl_up_sync(NS_FULL, x, o); if ((int)lane >= o) x += y; }
+    if (lane == 31) wsum[w] = x;
+    __syncthreads();
+    u32 off = chunk_offset[blockIdx.x] + (x - c);
+    for (u32 ww = 0; ww < w; ++ww) off += wsum[ww];
+    while (bits) {
+        u32 t = __ffs(bits) - 1; bits &= bits - 1;
+        u32 loc = (u32)(base + t);
+        if (off < capacity) queue[off] = make_uint4(off, loc, cell_of_loc(sc, loc), 0u);
+        ++off;
+    }
+}
+
+// S0 without a mask: everyone is sampled
+__global__ void __launch_bounds__(256) all_sampled_kernel(const ScenarioDev sc, u32 n, uint4 *__restrict__ queue) {
+    u32 i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) queue[i] = make_uint4(i, i, cell_of_loc(sc, i), 0u);
+}
+
+// ---- S6 ------------------------------------------------------------------------------------------
+// 144-bit sort key (k, f, loc, j) as 18 little-endian bytes: j[0..3], loc[4..7], f[8..13], k[14..17]
+__device__ __forceinline__ u32 key_byte(const SimBuffers &bf, u32 id, u32 b) {
+    if (b < 4) return (bf.term_j[id] >> (8 * b)) & 255u;
+    if (b < 8) return (bf.term_loc[id] >> (8 * (b - 4))) & 255u;
+    if (b < 14) return (u32)(bf.term_f[id] >> (8 * (b - 8))) & 255u;
+    return (bf.term_k[id] >> (8 * (b - 14))) & 255u;
+}
+
+#define NS_SORT_TILE 2048u
+// one LSD pass, step 1: per-block digit histogram, bin-major: hist[d * nblocks + block]
+__global__ void __launch_bounds__(256) radix_hist_kernel(const SimBuffers bf, const u32 *__restrict__ perm, u32 n, u32 byte,
+                                                         u32 *__restrict__ hist, u32 nblocks) {
+    __shared__ u32 h[256];
+    h[threadIdx.x] = 0;
+    __syncthreads();
+    u32 start = blockIdx.x * NS_SORT_TILE;
+    for (u32 r = 0; r < NS_SORT_TILE; r += 256u) {
+        u32 i = start + r + threadIdx.x;
+        if (i < n) atomicAdd(&h[key_byte(bf, perm[i], byte)], 1u);
+    }
+    __syncthreads();
+    hist[threadIdx.x * nblocks + blockIdx.x] = h[threadIdx.x];
+}
+// step 3 (after an exclusive scan of hist): stable scatter
+__global__ void __launch_bounds__(256) radix_scatter_kernel(const SimBuffers bf, const u32 *__restrict__ perm_in, u32 *__restrict__ perm_out,
+                                                            u32 n, u32 byte, const u32 *__restrict__ hist, u32 nblocks) {
+    __shared__ u32 base[256];
+    __shared__ u32 wcount[8][256];
+    base[threadIdx.x] = hist[threadIdx.x * nblocks + blockIdx.x];
+    const u32 lane = threadIdx.x & 31u, w = threadIdx.x >> 5;
+    u32 start = blockIdx.x * NS_SORT_TILE;
+    for (u32 r = 0; r < NS_SORT_TILE; r += 256u) {
+        for (u32 ww = 0; ww < 8; ++ww) wcount[ww][threadIdx.x] = 0;
+        __syncthreads();
+        u32 i = start + r + threadIdx.x;
+        bool valid = i < n;
+        u32 item = valid ? perm_in[i] : 0u;
+        u32 d = valid ? key_byte(bf, item, byte) : 256u + lane;   // invalid lanes never match anyone
+        u32 peers = __match_any_sync(NS_FULL, d);
+        u32 rank = __popc(peers & lanemask_lt());
+        if (valid && rank == 0) wcount[w][d] = __popc(peers);
+        __syncthreads();
+        if (valid) {
+            u32 off = base[d] + rank;
+            for (u32 ww = 0; ww < w; ++ww) off += wcount[ww][d];
+            perm_out[off] = item;
+        }
+        __syncthreads();
+        u32 add = 0;
+        for (u32 ww = 0; ww < 8; ++ww) add += wcount[ww][threadIdx.x];
+        base[threadIdx.x] += add;
+        __syncthreads();
+    }
+}
+
+__device__ __forceinline__ bool same_event(const SimBuffers &bf, u32 a, u32 b) {
+    return bf.term_k[a] == bf.term_k[b] && bf.term_f[a] == bf.term_f[b] && bf.term_loc[a] == bf.term_loc[b] &&
+           bf.term_j[a] == bf.term_j[b];
+}
+// unique, step 1: head flags over the sorted records
+__global__ void __launch_bounds__(256) unique_flag_kernel(const SimBuffers bf, const u32 *__restrict__ perm, u32 n, u32 *__restrict__ flag) {
+    u32 i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) flag[i] = (i == 0 || !same_event(bf, perm[i], perm[i - 1])) ? 1u : 0u;
+}
+// unique, step 2 (flag scanned exclusively -> uidx): write the species table; species_of[lineage] = rank
+__global__ void __launch_bounds__(256) unique_write_kernel(const SimBuffers bf, const u32 *__restrict__ perm, u32 n, const u32 *__restrict__ uidx,
+                                                           necsim_event *__restrict__ events, u32 *__restrict__ species_of, double delta_t) {
+    u32 i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    u32 id = perm[i];
+    bool head = (i == 0) || !same_event(bf, id, perm[i - 1]);
+    u32 e = head ? uidx[i] : uidx[i] - 1u;     // exclusive scan of head flags: a non-head belongs to the previous head
+    species_of[id] = e;
+    if (head) {
+        necsim_event ev;
+        ev.loc = bf.term_loc[id]; ev.k = bf.term_k[id]; ev.j = bf.term_j[id]; ev.abundance = 0;
+        ev.f = bf.term_f[id]; ev.time = event_time(ev.k, ev.f, delta_t);
+        events[e] = ev;
+    }
+}
+// resolve + label: follow the "culled at an event another lineage executed" links to a lineage that
+// ended by itself (links point to earlier arrivals at one event and time increases along a lineage: a forest)
+__global__ void __launch_bounds__(256) label_kernel(const SimBuffers bf, u32 n, const u32 *__restrict__ species_of, necsim_event *__restrict__ events,
+                                                    u32 *__restrict__ labels) {
+    u32 i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    u32 r = i;
+    while (bf.state[r] == 2) r = bf.parent[r];
+    if (bf.state[r] == 1) {
+        u32 e = species_of[r];
+        labels[i] = e;
+        atomicAdd(&events[e].abundance, 1u);
+    } else {
+        labels[i] = 0xFFFFFFFFu;
+        atomicAdd(&bf.ctr->n_unfinished, 1u);
+    }
+}
+
+__global__ void copy_u32_kernel(u32 *a, const u32 *src, u32 n) {
+    u32 i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) a[i] = src[i];
+}
+
+}  // namespace necsim

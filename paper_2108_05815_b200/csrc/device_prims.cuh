@@ -1,0 +1,149 @@
+// device_prims.cuh -- device primitives of the Independent algorithm.
+//   2.2 primeable hash RNG       (PAPER.md 5.2.1 L693-707: prime() on (seed, location, time))
+//   2.3 fixed-point -ln          (PAPER.md Eq. C.3: Exp(lambda) = -ln(U)/lambda)
+//   2.4 scale by 1/(lambda*dt)
+// Integer-only: every decision on the hot path is made in u32/u64 arithmetic (no libdevice, no FMA).
+#pragma once
+#include <stdint.h>
+
+namespace necsim {
+
+typedef uint32_t u32;
+typedef uint64_t u64;
+typedef int64_t i64;
+
+// first twelve primes: MULT = frac(sqrt p) | 1, KEYC = frac(cbrt p), 32 bits each
+#define NS_M0 0x6a09e667u
+#define NS_M1 0xbb67ae85u
+#define NS_M2 0x3c6ef373u
+#define NS_M3 0xa54ff53bu
+#define NS_M4 0x510e527fu
+#define NS_M5 0x9b05688du
+#define NS_M6 0x1f83d9abu
+#define NS_M7 0x5be0cd19u
+#define NS_M8 0xcbbb9d5du
+#define NS_M9 0x629a292bu
+#define NS_M10 0x9159015bu
+#define NS_M11 0x152fecd9u
+#define NS_C6 0x923f82a4u
+#define NS_C7 0xab1c5ed5u
+#define NS_C8 0xd807aa98u
+#define NS_C9 0x12835b01u
+#define NS_C10 0x243185beu
+#define NS_C11 0x550c7dc3u
+#define NS_GAMMA 0x6a09e667f3bcc909ull
+#define NS_L_SPEC 0xbb67ae8584caa73bull
+#define NS_L_DISP 0x3c6ef372fe94f82bull
+#define NS_L_INDEX 0xa54ff53a5f1d36f1ull
+#define NS_L_MIGR 0x510e527fade682d1ull
+#define NS_TWO48 (1ull << 48)
+
+// one Feistel round: p = a*M; (a, b) <- (hi32(p) ^ b ^ K, lo32(p))   [1 IMAD.WIDE.U32 + 1 LOP3]
+__host__ __device__ __forceinline__ void feistel(u32 &a, u32 &b, u32 M, u32 K) {
+    u64 p = (u64)a * (u64)M;
+    u32 na = (u32)(p >> 32) ^ b ^ K;
+    b = (u32)p;
+    a = na;
+}
+
+// F: fixed-key 64-bit bijection, rounds 6..11
+__host__ __device__ __forceinline__ u64 hashF(u64 x) {
+    u32 a = (u32)x, b = (u32)(x >> 32);
+    feistel(a, b, NS_M6, NS_C6);
+    feistel(a, b, NS_M7, NS_C7);
+    feistel(a, b, NS_M8, NS_C8);
+    feistel(a, b, NS_M9, NS_C9);
+    feistel(a, b, NS_M10, NS_C10);
+    feistel(a, b, NS_M11, NS_C11);
+    return ((u64)a << 32) | (u64)b;
+}
+
+struct SeedKey {
+    u32 K[6];
+};
+
+// host side key schedule: h = F(seed); K[r] = hi32(F(h + (r+1)*GAMMA))
+static inline SeedKey key_schedule(u64 seed) {
+    SeedKey sk;
+    u64 h = hashF(seed);
+    for (int r = 0; r < 6; ++r) sk.K[r] = (u32)(hashF(h + (u64)(r + 1) * NS_GAMMA) >> 32);
+    return sk;
+}
+
+// prime(loc, k): keyed rounds 0..5 on (a, b) = (loc, k)
+__device__ __forceinline__ u64 prime(const SeedKey &sk, u32 loc, u32 k) {
+    u32 a = loc, b = k;
+    feistel(a, b, NS_M0, sk.K[0]);
+    feistel(a, b, NS_M1, sk.K[1]);
+    feistel(a, b, NS_M2, sk.K[2]);
+    feistel(a, b, NS_M3, sk.K[3]);
+    feistel(a, b, NS_M4, sk.K[4]);
+    feistel(a, b, NS_M5, sk.K[5]);
+    return ((u64)a << 32) | (u64)b;
+}
+
+// draws for the event candidate at stream position X = s + j*GAMMA
+__device__ __forceinline__ u64 draw_time(u64 X) { return hashF(X); }
+__device__ __forceinline__ u64 draw_spec(u64 X) { return hashF(X ^ NS_L_SPEC); }
+__device__ __forceinline__ u64 draw_disp(u64 X, u32 r) { return hashF((X ^ NS_L_DISP) + (u64)r * NS_GAMMA); }
+__device__ __forceinline__ u64 draw_index(u64 X) { return hashF(X ^ NS_L_INDEX); }
+__device__ __forceinline__ u64 draw_migr(u64 X) { return hashF(X ^ NS_L_MIGR); }
+
+__device__ __forceinline__ u64 mulhi64(u64 x, u64 n) { return __umul64hi(x, n); }
+// (x * d) >> 64 for a 32-bit d: two 32x32 products instead of a full 64x64
+__device__ __forceinline__ u32 mulhi64_u32(u64 x, u32 d) {
+    u64 lo = (u64)(u32)x * (u64)d;
+    u64 hi = (u64)(u32)(x >> 32) * (u64)d + (lo >> 32);
+    return (u32)(hi >> 32);
+}
+__device__ __forceinline__ bool bern(u64 x, u64 thr) { return (x >> 11) < thr; }
+
+// fixed-point -ln: Q8.56 of -ln(U), U = M * 2^-(z+50). tQ/tA: 512-entry tables (shared memory)
+#define NS_LN2_56 49946518145322873ull
+__device__ __forceinline__ u64 neglog(u64 x, const unsigned short *__restrict__ tQ, const u64 *__restrict__ tA) {
+    u32 z = (u32)__clzll((long long)x);         // 64 for x = 0
+    u64 y = (z >= 64) ? 0ull : (x << z);
+    u64 M = (y >> 14) | 1ull;
+    u32 i = (u32)(y >> 54) & 511u;
+    u64 P = M * (u64)tQ[i];
+    u64 r = P & ((1ull << 61) - 1);
+    u32 t = (u32)(r >> 21);
+    u32 h1 = 0x55555555u - (t >> 10);
+    u32 h2 = 0x80000000u - (__umulhi(t, h1) >> 8);
+    u64 u = (u64)__umulhi(t, h2);
+    u64 c = ((u64)t * u) >> 24;
+    u64 G = tA[i] + ((r >> 5) - c);
+    u64 Lz = (u64)(z + 1) * NS_LN2_56;
+    return Lz > G ? Lz - G : 0ull;
+}
+
+// E / mu in Q16.48: bits of the exact 96-bit product E * Cm
+__device__ __forceinline__ u64 scale_exp(u64 E, u32 Cm, u32 sh) {
+    u64 Eh = E >> 32, El = E & 0xFFFFFFFFull;
+    return ((Eh * (u64)Cm) + ((El * (u64)Cm) >> 32)) >> sh;
+}
+
+// real time of (k, f): ((double)k + (double)f * 2^-48) * delta_t, no contraction
+__device__ __forceinline__ double event_time(u32 k, u64 f, double delta_t) {
+    double a = __dmul_rn((double)f, 0x1p-48);
+    double b = __dadd_rn((double)k, a);
+    return __dmul_rn(b, delta_t);
+}
+
+// 128-bit atomic exchange in global memory (PTX ISA 8.3+, sm_90+): returns the previous 16 bytes
+__device__ __forceinline__ uint4 atomic_exch_128(uint4 *addr, uint4 v) {
+    u64 lo = ((u64)v.y << 32) | v.x, hi = ((u64)v.w << 32) | v.z, olo, ohi;
+    asm volatile(
+        "{\n\t"
+        ".reg .b128 vin, vout;\n\t"
+        "mov.b128 vin, {%2, %3};\n\t"
+        "atom.global.relaxed.gpu.exch.b128 vout, [%4], vin;\n\t"
+        "mov.b128 {%0, %1}, vout;\n\t"
+        "}"
+        : "=l"(olo), "=l"(ohi)
+        : "l"(lo), "l"(hi), "l"(addr)
+        : "memory");
+    return make_uint4((u32)olo, (u32)(olo >> 32), (u32)ohi, (u32)(ohi >> 32));
+}
+
+}  // namespace necsim

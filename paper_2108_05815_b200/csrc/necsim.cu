@@ -1,0 +1,766 @@
+// necsim.cu -- host side of libnecsim_b200.so: the C-ABI of include/necsim.h.
+// Scenario builder (validation, canonical indexing, alias / rounded-normal / turnover-scale tables,
+// DESIGN.md 2.4-2.5), the epoch loop around the persistent simulate kernel (Water-Level horizons,
+// PAPER.md App. G.1), and the S6 reduction to species. No torch types, no CPU fallback.
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+#include <string>
+#include <vector>
+#include <algorithm>
+
+#include "../../include/necsim.h"
+#include "device_prims.cuh"
+#include "sim_types.cuh"
+#include "sim_kernel.cuh"
+#include "aux_kernels.cuh"
+#include "neglog_tables.inc"
+
+using namespace necsim;
+
+static thread_local std::string g_err;
+static int fail(int code, const std::string &msg) { g_err = msg; return code; }
+#define CU(call)                                                                                         \
+    do {                                                                                                 \
+        cudaError_t e_ = (call);                                                                         \
+        if (e_ != cudaSuccess)                                                                           \
+            return fail(NECSIM_ERR_CUDA, std::string(#call) + ": " + cudaGetErrorString(e_));           \
+    } while (0)
+
+extern "C" const char *necsim_last_error(void) { return g_err.c_str(); }
+
+static inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+// ---------------------------------------------------------------------------------------------------
+// host-side table construction
+// ---------------------------------------------------------------------------------------------------
+// scale of 1/mu from binary64 inv = 1/(lambda*delta_t): Cm = floor(inv * 2^(31-e)), sh = 7 - e, e = floor(log2 inv)
+static bool turnover_scale(double lambda, double delta_t, u32 &Cm, u32 &sh) {
+    if (!(lambda > 0.0) || !(delta_t > 0.0) || !std::isfinite(lambda) || !std::isfinite(delta_t)) return false;
+    double inv = 1.0 / (lambda * delta_t);
+    if (!(inv >= 0x1p-6) || !(inv < 0x1p8)) return false;
+    int e = ilogb(inv);
+    double scaled = scalbn(inv, 31 - e);   // exact, in [2^31, 2^32)
+    Cm = (u32)(u64)scaled;                 // truncation = floor for positive values
+    sh = (u32)(7 - e);
+    return true;
+}
+
+static inline u32 to_thresh32(double p) {
+    double v = floor(p * 4294967296.0);
+    return (v >= 4294967295.0) ? 0xFFFFFFFFu : (u32)v;
+}
+
+// Walker alias table of one row, construction order of DESIGN.md 2.5 step 3. 0 ok, -1 bad weights, -3 dead column
+static int alias_row(const double *w, u32 n, uint2 *out, std::vector<double> &p, std::vector<u32> &small, std::vector<u32> &large) {
+    double S = 0.0;
+    for (u32 c = 0; c < n; ++c) {
+        if (!(w[c] >= 0.0) || !std::isfinite(w[c])) return -1;
+        S = S + w[c];
+    }
+    if (!(S > 0.0)) return -1;
+    small.clear(); large.clear();
+    for (u32 c = 0; c < n; ++c) {
+        volatile double num = w[c] * (double)n;
+        p[c] = num / S;
+        if (p[c] < 1.0) small.push_back(c); else large.push_back(c);
+    }
+    while (!small.empty() && !large.empty()) {
+        u32 s = small.back(); small.pop_back();
+        u32 l = large.back(); large.pop_back();
+        out[s].x = to_thresh32(p[s]); out[s].y = l;
+        volatile double sum = p[l] + p[s];
+        p[l] = sum - 1.0;
+        if (p[l] < 1.0) small.push_back(l); else large.push_back(l);
+    }
+    int rc = 0;
+    for (u32 l : large) { out[l].x = 0xFFFFFFFFu; out[l].y = l; if (w[l] == 0.0) rc = -3; }
+    for (u32 s : small) { out[s].x = 0xFFFFFFFFu; out[s].y = s; if (w[s] == 0.0) rc = -3; }
+    return rc;
+}
+
+// rounded-normal thresholds TG[i] = min(floor(Phi((i - R + 0.5)/sigma) * 2^32), 2^32 - 1), i in [0, 2R)
+static void gauss_table(double sigma, int R, std::vector<u32> &tg) {
+    tg.resize(2 * (size_t)R);
+    for (int i = 0; i < 2 * R; ++i) {
+        double z = ((double)(i - R) + 0.5) / sigma;
+        double phi = 0.5 * erfc(-z * 0.7071067811865476);
+        tg[i] = to_thresh32(phi);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// scenario handle
+// ---------------------------------------------------------------------------------------------------
+struct necsim_scenario {
+    ScenarioDev dev;
+    double migration;
+    double mu_max;            // max lambda*delta_t over habitat cells (epoch-horizon policy)
+    u64 n_individuals;
+    size_t ws_bytes;
+    int sm_count;
+    SimCounters *h_ctr;       // pinned read-back buffer
+    cudaEvent_t ev[4];
+    bool tables_uploaded;
+};
+
+struct ScenarioLayout {
+    size_t off_hab8, off_deme32, off_prefix, off_scale, off_alias, off_gauss, total;
+    u32 ncells, gauss_len;
+    int R;
+    bool uniform_deme, need_deme32, per_cell_turnover;
+};
+
+static int scenario_layout(const necsim_scenario_desc *d, ScenarioLayout &L) {
+    if (!d) return fail(NECSIM_ERR_INVALID_ARG, "desc is NULL");
+    memset(&L, 0, sizeof(L));
+    if (d->kind < 0 || d->kind > 3) return fail(NECSIM_ERR_INVALID_ARG, "unknown scenario kind");
+    if (!(d->delta_t > 0.0) || !std::isfinite(d->delta_t)) return fail(NECSIM_ERR_INVALID_ARG, "delta_t must be > 0 and finite");
+    if (d->kind == NECSIM_SPATIALLY_IMPLICIT) {
+        if (d->local_size == 0 || d->meta_size == 0 || d->local_size + d->meta_size >= (1ull << 32) || !(d->migration >= 0.0 && d->migration <= 1.0))
+            return fail(NECSIM_ERR_INVALID_ARG, "implicit: bad sizes or migration");
+        L.ncells = 2; L.uniform_deme = false; L.total = 256;
+        return NECSIM_OK;
+    }
+    if (d->width == 0 || d->height == 0 || (u64)d->width * d->height >= (1ull << 32)) return fail(NECSIM_ERR_INVALID_ARG, "bad width/height");
+    if (d->kind == NECSIM_NONSPATIAL && !(d->width == 1 && d->height == 1)) return fail(NECSIM_ERR_INVALID_ARG, "nonspatial needs 1x1");
+    L.ncells = d->width * d->height;
+    L.uniform_deme = (d->deme == NULL) || d->kind == NECSIM_NONSPATIAL;
+    L.per_cell_turnover = (d->turnover != NULL) && d->kind != NECSIM_NONSPATIAL;
+    if (!L.uniform_deme) {
+        for (u32 c = 0; c < L.ncells; ++c) if (d->deme[c] >= 255u) { L.need_deme32 = true; break; }
+    }
+    size_t off = 0;
+    if (d->kind >= NECSIM_EXPLICIT_MATRIX && !L.uniform_deme) {
+        L.off_hab8 = off; off = align256(off + L.ncells);
+        if (L.need_deme32) { L.off_deme32 = off; off = align256(off + 4 * (size_t)L.ncells); }
+        L.off_prefix = off; off = align256(off + 4 * ((size_t)L.ncells + 1));
+    } else if (!L.uniform_deme) {
+        return fail(NECSIM_ERR_INVALID_ARG, "internal: deme array with a non-explicit kind");
+    }
+    if (L.per_cell_turnover) { L.off_scale = off; off = align256(off + 8 * (size_t)L.ncells); }
+    if (d->kind == NECSIM_EXPLICIT_MATRIX) {
+        if (!d->dispersal_matrix) return fail(NECSIM_ERR_INVALID_ARG, "matrix missing");
+        L.off_alias = off; off = align256(off + 8 * (size_t)L.ncells * L.ncells);
+    }
+    if (d->kind == NECSIM_EXPLICIT_GAUSSIAN) {
+        if (!(d->sigma > 0.0) || !std::isfinite(d->sigma)) return fail(NECSIM_ERR_INVALID_ARG, "bad sigma");
+        L.R = (int)ceil(10.0 * d->sigma);
+        if ((u32)L.R >= d->width || (u32)L.R >= d->height) return fail(NECSIM_ERR_INVALID_ARG, "10*sigma must be < min(width,height)");
+        u32 len = 2; while (len < 2u * (u32)L.R) len <<= 1;
+        if (len > 1024u) return fail(NECSIM_ERR_UNSUPPORTED, "sigma too large: the threshold table must fit 1024 entries");
+        L.gauss_len = len;
+        L.off_gauss = off; off = align256(off + 4 * (size_t)len);
+    }
+    L.total = off ? off : 256;
+    return NECSIM_OK;
+}
+
+extern "C" int necsim_scenario_workspace_size(const necsim_scenario_desc *desc, size_t *device_bytes) {
+    if (!device_bytes) return fail(NECSIM_ERR_INVALID_ARG, "device_bytes is NULL");
+    ScenarioLayout L;
+    int rc = scenario_layout(desc, L);
+    if (rc) return rc;
+    *device_bytes = L.total;
+    return NECSIM_OK;
+}
+
+static int upload_neglog_tables(cudaStream_t st) {
+    CU(cudaMemcpyToSymbolAsync(NEGLOG_Q_DEV, NEGLOG_Q_HOST, sizeof(NEGLOG_Q_HOST), 0, cudaMemcpyHostToDevice, st));
+    CU(cudaMemcpyToSymbolAsync(NEGLOG_A_DEV, NEGLOG_A_HOST, sizeof(NEGLOG_A_HOST), 0, cudaMemcpyHostToDevice, st));
+    return NECSIM_OK;
+}
+
+extern "C" int necsim_create_scenario(const necsim_scenario_desc *d, void *d_workspace, size_t bytes, void *cuda_stream, necsim_scenario **out) {
+    if (!out) return fail(NECSIM_ERR_INVALID_ARG, "out is NULL");
+    *out = NULL;
+    ScenarioLayout L;
+    int rc = scenario_layout(d, L);
+    if (rc) return rc;
+    if (!d_workspace || bytes < L.total) return fail(NECSIM_ERR_WORKSPACE_TOO_SMALL, "scenario workspace too small");
+    if (((uintptr_t)d_workspace & 255u) != 0) return fail(NECSIM_ERR_INVALID_ARG, "workspace must be 256-byte aligned");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int dev_id = 0, sm_count = 0;
+    CU(cudaGetDevice(&dev_id));
+    CU(cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev_id));
+
+    ScenarioDev sd;
+    memset(&sd, 0, sizeof(sd));
+    sd.kind = d->kind; sd.delta_t = d->delta_t; sd.width_shift = 0xFFFFFFFFu;
+    uint8_t *base = (uint8_t *)d_workspace;
+    double mu_max = 0.0;
+    const u32 n = L.ncells;
+
+    if (d->kind == NECSIM_SPATIALLY_IMPLICIT) {
+        sd.width = 2; sd.height = 1; sd.ncells = 2;
+        sd.J_local = (u32)d->local_size; sd.J_meta = (u32)d->meta_size;
+        sd.n_locations = d->local_size + d->meta_size; sd.n_sampleable = d->local_size;
+        if (!turnover_scale(d->uniform_turnover, d->delta_t, sd.Cm_u, sd.sh_u)) return fail(NECSIM_ERR_INVALID_ARG, "turnover*delta_t out of range");
+        mu_max = d->uniform_turnover * d->delta_t;
+    } else {
+        sd.width = d->width; sd.height = d->height; sd.ncells = n;
+        if ((d->width & (d->width - 1)) == 0) { u32 s = 0; while ((1u << s) < d->width) ++s; sd.width_shift = s; }
+        // deme, prefix
+        u64 tot = 0;
+        std::vector<uint8_t> hab8; std::vector<u32> prefix;
+        if (L.uniform_deme) {
+            u32 ud = d->kind == NECSIM_NONSPATIAL ? (d->deme ? d->deme[0] : d->uniform_deme) : d->uniform_deme;
+            sd.uniform_deme = ud; tot = (u64)ud * n;
+        } else {
+            hab8.resize(n); prefix.resize((size_t)n + 1);
+            for (u32 c = 0; c < n; ++c) { prefix[c] = (u32)tot; tot += d->deme[c]; hab8[c] = (uint8_t)std::min(d->deme[c], 255u); }
+            prefix[n] = (u32)tot;
+        }
+        if (tot == 0 || tot >= (1ull << 32)) return fail(NECSIM_ERR_INVALID_ARG, "number of indexed locations must be in [1, 2^32)");
+        sd.n_locations = tot; sd.n_sampleable = tot;
+        // turnover scales
+        std::vector<uint2> scale;
+        if (L.per_cell_turnover) {
+            scale.resize(n);
+            for (u32 c = 0; c < n; ++c) {
+                u32 dm = L.uniform_deme ? sd.uniform_deme : d->deme[c];
+                if (dm > 0) {
+                    if (!turnover_scale(d->turnover[c], d->delta_t, scale[c].x, scale[c].y)) return fail(NECSIM_ERR_INVALID_ARG, "turnover*delta_t out of range");
+                    mu_max = std::max(mu_max, d->turnover[c] * d->delta_t);
+                } else scale[c] = make_uint2(0, 0);
+            }
+            sd.per_cell_turnover = 1;
+        } else {
+            if (!turnover_scale(d->uniform_turnover, d->delta_t, sd.Cm_u, sd.sh_u)) return fail(NECSIM_ERR_INVALID_ARG, "turnover*delta_t out of range");
+            mu_max = d->uniform_turnover * d->delta_t;
+        }
+        if (!L.uniform_deme) {
+            CU(cudaMemcpyAsync(base + L.off_hab8, hab8.data(), n, cudaMemcpyHostToDevice, st));
+            sd.hab8 = base + L.off_hab8;
+            if (L.need_deme32) {
+                CU(cudaMemcpyAsync(base + L.off_deme32, d->deme, 4 * (size_t)n, cudaMemcpyHostToDevice, st));
+                sd.deme32 = (const u32 *)(base + L.off_deme32);
+            }
+            CU(cudaMemcpyAsync(base + L.off_prefix, prefix.data(), 4 * ((size_t)n + 1), cudaMemcpyHostToDevice, st));
+            sd.prefix = (const u32 *)(base + L.off_prefix);
+        }
+        if (L.per_cell_turnover) {
+            CU(cudaMemcpyAsync(base + L.off_scale, scale.data(), 8 * (size_t)n, cudaMemcpyHostToDevice, st));
+            sd.scale = (const uint2 *)(base + L.off_scale);
+        }
+        if (d->kind == NECSIM_EXPLICIT_MATRIX) {
+            std::vector<uint2> tab((size_t)n * n);
+            std::vector<double> p(n); std::vector<u32> small, large; small.reserve(n); large.reserve(n);
+            for (u32 row = 0; row < n; ++row) {
+                u32 dm = L.uniform_deme ? sd.uniform_deme : d->deme[row];
+                uint2 *o = tab.data() + (size_t)row * n;
+                if (dm == 0) { for (u32 c = 0; c < n; ++c) o[c] = make_uint2(0xFFFFFFFFu, c); continue; }
+                const double *w = d->dispersal_matrix + (size_t)row * n;
+                if (!L.uniform_deme) for (u32 c = 0; c < n; ++c) if (d->deme[c] == 0 && w[c] != 0.0) return fail(NECSIM_ERR_INVALID_ARG, "dispersal into non-habitat");
+                if (L.uniform_deme && sd.uniform_deme == 0) return fail(NECSIM_ERR_INVALID_ARG, "no habitat");
+                if (alias_row(w, n, o, p, small, large) != 0) return fail(NECSIM_ERR_INVALID_ARG, "bad dispersal matrix row");
+            }
+            CU(cudaMemcpyAsync(base + L.off_alias, tab.data(), 8 * (size_t)n * n, cudaMemcpyHostToDevice, st));
+            CU(cudaStreamSynchronize(st));   // tab goes out of scope
+            sd.alias = (const uint2 *)(base + L.off_alias);
+        }
+        if (d->kind == NECSIM_EXPLICIT_GAUSSIAN) {
+            std::vector<u32> tg;
+            gauss_table(d->sigma, L.R, tg);
+            tg.resize(L.gauss_len, 0xFFFFFFFFu);
+            CU(cudaMemcpyAsync(base + L.off_gauss, tg.data(), 4 * (size_t)L.gauss_len, cudaMemcpyHostToDevice, st));
+            CU(cudaStreamSynchronize(st));
+            sd.gauss = (const u32 *)(base + L.off_gauss); sd.R = L.R; sd.gauss_len = L.gauss_len;
+        }
+    }
+    rc = upload_neglog_tables(st);
+    if (rc) return rc;
+    CU(cudaStreamSynchronize(st));
+
+    necsim_scenario *h = new necsim_scenario();
+    h->dev = sd; h->mu_max = mu_max; h->migration = (d->kind == NECSIM_SPATIALLY_IMPLICIT) ? d->migration : 0.0; h->n_individuals = sd.n_sampleable; h->ws_bytes = L.total; h->sm_count = sm_count;
+    h->h_ctr = NULL; h->tables_uploaded = true;
+    if (cudaHostAlloc((void **)&h->h_ctr, sizeof(SimCounters), cudaHostAllocDefault) != cudaSuccess) { delete h; return fail(NECSIM_ERR_CUDA, "cudaHostAlloc failed"); }
+    for (int i = 0; i < 4; ++i) if (cudaEventCreate(&h->ev[i]) != cudaSuccess) { delete h; return fail(NECSIM_ERR_CUDA, "cudaEventCreate failed"); }
+    *out = h;
+    return NECSIM_OK;
+}
+
+extern "C" int necsim_scenario_num_individuals(const necsim_scenario *scn, uint64_t *n_individuals) {
+    if (!scn || !n_individuals) return fail(NECSIM_ERR_INVALID_ARG, "NULL argument");
+    *n_individuals = scn->n_individuals;
+    return NECSIM_OK;
+}
+
+extern "C" int necsim_destroy(necsim_scenario *scn) {
+    if (!scn) return NECSIM_OK;
+    if (scn->h_ctr) cudaFreeHost(scn->h_ctr);
+    for (int i = 0; i < 4; ++i) cudaEventDestroy(scn->ev[i]);
+    delete scn;
+    return NECSIM_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// simulate
+// ---------------------------------------------------------------------------------------------------
+struct ResolvedParams {
+    u32 block_threads, grid_blocks, dedup_log2_slots, tail_threshold;
+    bool dedup;
+    u64 epoch_events, max_steps;
+};
+
+static int resolve_params(const necsim_scenario *scn, const necsim_sim_params *p, ResolvedParams &r) {
+    necsim_sim_params z;
+    memset(&z, 0, sizeof(z));
+    if (!p) p = &z;
+    r.block_threads = p->block_threads ? p->block_threads : 256u;
+    if (r.block_threads % 32u || r.block_threads > 256u) return fail(NECSIM_ERR_INVALID_ARG, "block_threads must be a multiple of 32 and <= 256");
+    r.grid_blocks = p->grid_blocks;
+    if (p->dedup > 2) return fail(NECSIM_ERR_INVALID_ARG, "dedup must be 0, 1 or 2");
+    r.dedup = p->dedup != 2;
+    r.dedup_log2_slots = p->dedup_log2_slots ? p->dedup_log2_slots : 22u;
+    if (r.dedup_log2_slots < 4 || r.dedup_log2_slots > 28) return fail(NECSIM_ERR_INVALID_ARG, "dedup_log2_slots must be in [4, 28]");
+    r.epoch_events = p->epoch_events ? p->epoch_events : (r.dedup ? (1ull << r.dedup_log2_slots) / 2 : 0);
+    r.max_steps = p->max_steps;
+    if (r.max_steps > 0xFFFFFFFFull) return fail(NECSIM_ERR_INVALID_ARG, "max_steps must fit 32 bits");
+    r.tail_threshold = p->tail_threshold;
+    (void)scn;
+    return NECSIM_OK;
+}
+
+struct SimLayout {
+    size_t off_ctr, off_qa, off_qb, off_cache, off_term_loc, off_term_k, off_term_j, off_steps, off_parent, off_ring, off_term_f,
+        off_state, off_events, off_labels, off_species, off_perm_a, off_perm_b, off_flag, off_hist, off_chunk, off_mask, total;
+    u32 n_chunks, sort_blocks;
+};
+
+static void sim_layout(u64 n_individuals, u64 cap, const ResolvedParams &rp, SimLayout &L) {
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off = align256(off + bytes); return o; };
+    L.n_chunks = (u32)((n_individuals + NS_CHUNK - 1) / NS_CHUNK);
+    L.sort_blocks = (u32)((cap + NS_SORT_TILE - 1) / NS_SORT_TILE);
+    if (L.sort_blocks == 0) L.sort_blocks = 1;
+    L.off_ctr = take(sizeof(SimCounters));
+    L.off_qa = take(16 * cap); L.off_qb = take(16 * cap);
+    L.off_cache = take(rp.dedup ? (16ull << rp.dedup_log2_slots) : 16);
+    L.off_term_loc = take(4 * cap); L.off_term_k = take(4 * cap); L.off_term_j = take(4 * cap); L.off_steps = take(4 * cap);
+    L.off_parent = take(4 * cap); L.off_ring = take(4 * cap); L.off_term_f = take(8 * cap); L.off_state = take(cap);
+    L.off_events = take(sizeof(necsim_event) * cap); L.off_labels = take(4 * cap); L.off_species = take(4 * cap);
+    L.off_perm_a = take(4 * cap); L.off_perm_b = take(4 * cap); L.off_flag = take(4 * cap);
+    L.off_hist = take(4 * 256 * (size_t)L.sort_blocks); L.off_chunk = take(4 * ((size_t)L.n_chunks + 1));
+    L.off_mask = take(n_individuals);
+    L.total = off;
+}
+
+extern "C" int necsim_simulate_workspace_size(const necsim_scenario *scn, uint64_t n_sampled, const necsim_sim_params *params, size_t *device_bytes) {
+    if (!scn || !device_bytes) return fail(NECSIM_ERR_INVALID_ARG, "NULL argument");
+    if (n_sampled == 0 || n_sampled > scn->n_individuals) return fail(NECSIM_ERR_INVALID_ARG, "n_sampled must be in [1, n_individuals]");
+    ResolvedParams rp;
+    int rc = resolve_params(scn, params, rp);
+    if (rc) return rc;
+    SimLayout L;
+    sim_layout(scn->n_individuals, n_sampled, rp, L);
+    *device_bytes = L.total;
+    return NECSIM_OK;
+}
+
+template <int KIND>
+static cudaError_t launch_epoch(bool dedup, u32 grid, u32 block, cudaStream_t st, const ScenarioDev &sd, const SimBuffers &bf, const EpochArgs &ep) {
+    if (dedup) simulate_kernel<KIND, true><<<grid, block, 0, st>>>(sd, bf, ep);
+    else simulate_kernel<KIND, false><<<grid, block, 0, st>>>(sd, bf, ep);
+    return cudaGetLastError();
+}
+template <int KIND>
+static int occupancy_blocks(bool dedup, u32 block) {
+    int nb = 0;
+    if (dedup) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, simulate_kernel<KIND, true>, (int)block, 0);
+    else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, simulate_kernel<KIND, false>, (int)block, 0);
+    return nb;
+}
+
+static u64 thr53(double p) { return (u64)floor(ldexp(p, 53)); }
+
+static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const uint8_t *d_mask, uint64_t cap, const necsim_sim_params *params,
+                         void *d_workspace, size_t bytes, cudaStream_t st, necsim_result *out, const SimLayout &L, const ResolvedParams &rp) {
+    const ScenarioDev &sd = scn->dev;
+    uint8_t *base = (uint8_t *)d_workspace;
+    memset(out, 0, sizeof(*out));
+    SimBuffers bf;
+    memset(&bf, 0, sizeof(bf));
+    bf.ctr = (SimCounters *)(base + L.off_ctr);
+    uint4 *qa = (uint4 *)(base + L.off_qa), *qb = (uint4 *)(base + L.off_qb);
+    bf.cache = (uint4 *)(base + L.off_cache); bf.cache_mask = rp.dedup ? ((1u << rp.dedup_log2_slots) - 1u) : 0u;
+    bf.term_loc = (u32 *)(base + L.off_term_loc); bf.term_k = (u32 *)(base + L.off_term_k); bf.term_j = (u32 *)(base + L.off_term_j);
+    bf.steps = (u32 *)(base + L.off_steps); bf.parent = (u32 *)(base + L.off_parent); bf.spec_ring = (u32 *)(base + L.off_ring);
+    bf.term_f = (u64 *)(base + L.off_term_f); bf.state = base + L.off_state;
+    necsim_event *events = (necsim_event *)(base + L.off_events);
+    u32 *labels = (u32 *)(base + L.off_labels), *species_of = (u32 *)(base + L.off_species);
+    u32 *perm_a = (u32 *)(base + L.off_perm_a), *perm_b = (u32 *)(base + L.off_perm_b), *flag = (u32 *)(base + L.off_flag);
+    u32 *hist = (u32 *)(base + L.off_hist), *chunk = (u32 *)(base + L.off_chunk);
+    SimCounters *hc = scn->h_ctr;
+
+    CU(cudaEventRecord(scn->ev[0], st));
+    CU(cudaMemsetAsync(bf.ctr, 0, sizeof(SimCounters), st));
+    CU(cudaMemsetAsync(bf.state, 0, cap, st));
+    if (rp.dedup) CU(cudaMemsetAsync(bf.cache, 0xFF, 16ull << rp.dedup_log2_slots, st));
+
+    // ---- S0: sample mask -> lineage queue ------------------------------------------------------------
+    u64 n_ind = scn->n_individuals;
+    u32 n_sampled = 0;
+    if (d_mask) {
+        mask_count_kernel<<<L.n_chunks, 256, 0, st>>>(d_mask, n_ind, chunk);
+        scan_exclusive_kernel<<<1, 1024, 0, st>>>(chunk, L.n_chunks, &bf.ctr->n_sampled);
+        mask_scatter_kernel<<<L.n_chunks, 256, 0, st>>>(sd, d_mask, n_ind, chunk, qa, (u32)cap);
+        CU(cudaGetLastError());
+        CU(cudaMemcpyAsync(hc, bf.ctr, sizeof(SimCounters), cudaMemcpyDeviceToHost, st));
+        CU(cudaStreamSynchronize(st));
+        n_sampled = hc->n_sampled;
+        if (n_sampled == 0) return fail(NECSIM_ERR_INVALID_ARG, "the sample mask selects nobody");
+        if (n_sampled > cap) return fail(NECSIM_ERR_WORKSPACE_TOO_SMALL, "more sampled individuals than n_sampled_capacity");
+    } else {
+        if (n_ind > cap) return fail(NECSIM_ERR_WORKSPACE_TOO_SMALL, "n_sampled_capacity < n_individuals with a NULL mask");
+        n_sampled = (u32)n_ind;
+        all_sampled_kernel<<<(n_sampled + 255) / 256, 256, 0, st>>>(sd, n_sampled, qa);
+        CU(cudaGetLastError());
+    }
+
+    // ---- S1-S5: epochs of the persistent simulate kernel ---------------------------------------------
+    EpochArgs ep;
+    ep.key = key_schedule(seed);
+    ep.thr_nu = thr53(nu);
+    ep.thr_m = thr53(scn->migration);
+    ep.max_steps = (u32)rp.max_steps;
+    int occ = 0;
+    switch (sd.kind) {
+    case 0: occ = occupancy_blocks<0>(rp.dedup, rp.block_threads); break;
+    case 1: occ = occupancy_blocks<1>(rp.dedup, rp.block_threads); break;
+    case 2: occ = occupancy_blocks<2>(rp.dedup, rp.block_threads); break;
+    default: occ = occupancy_blocks<3>(rp.dedup, rp.block_threads); break;
+    }
+    if (occ <= 0) return fail(NECSIM_ERR_CUDA, "simulate kernel cannot be resident (occupancy 0)");
+    const u32 full_grid = rp.grid_blocks ? rp.grid_blocks : (u32)(occ * scn->sm_count);
+    u32 active = n_sampled, k_start = 0;
+    uint4 *q_in = qa, *q_out = qb;
+    float ms_sim = 0.f;
+    u64 n_epochs = 0;
+    while (active > 0) {
+        u32 k_stop;
+        if (rp.epoch_events == 0) k_stop = 0xFFFFFFFFu;
+        else {
+            double span = (double)rp.epoch_events / ((double)active * scn->mu_max);
+            u64 sp = span < 1.0 ? 1ull : (span > 1e9 ? 1000000000ull : (u64)span);
+            u64 h = (u64)k_start + sp;
+            k_stop = h >= 0xFFFFFFFFull ? 0xFFFFFFFFu : (u32)h;
+        }
+        ep.k_start = k_start; ep.k_stop = k_stop;
+        const u64 total_warps = (u64)full_grid * (rp.block_threads / 32u);
+        u32 lanes = 32;
+        if ((u64)active < total_warps * 32ull) lanes = (u32)std::max<u64>(1, ((u64)active + total_warps - 1) / total_warps);
+        ep.lanes_per_warp = lanes;
+        u32 grid = full_grid;
+        if (lanes == 1) grid = (u32)std::min<u64>(full_grid, ((u64)active + rp.block_threads / 32u - 1) / (rp.block_threads / 32u));
+        bf.q_in = q_in; bf.q_out = q_out; bf.q_in_count = active;
+        CU(cudaMemsetAsync(bf.ctr, 0, 8, st));   // q_head, q_out
+        CU(cudaEventRecord(scn->ev[2], st));
+        cudaError_t ce;
+        switch (sd.kind) {
+        case 0: ce = launch_epoch<0>(rp.dedup, grid, rp.block_threads, st, sd, bf, ep); break;
+        case 1: ce = launch_epoch<1>(rp.dedup, grid, rp.block_threads, st, sd, bf, ep); break;
+        case 2: ce = launch_epoch<2>(rp.dedup, grid, rp.block_threads, st, sd, bf, ep); break;
+        default: ce = launch_epoch<3>(rp.dedup, grid, rp.block_threads, st, sd, bf, ep); break;
+        }
+        if (ce != cudaSuccess) return fail(NECSIM_ERR_CUDA, std::string("simulate kernel launch: ") + cudaGetErrorString(ce));
+        CU(cudaEventRecord(scn->ev[3], st));
+        CU(cudaMemcpyAsync(hc, bf.ctr, sizeof(SimCounters), cudaMemcpyDeviceToHost, st));
+        CU(cudaStreamSynchronize(st));
+        float ms = 0.f;
+        CU(cudaEventElapsedTime(&ms, scn->ev[2], scn->ev[3]));
+        ms_sim += ms;
+        ++n_epochs;
+        if (hc->error) return fail(NECSIM_ERR_CAPACITY, "interval index overflowed 2^32 or dispersal resampling exhausted");
+        active = hc->q_out;
+        std::swap(q_in, q_out);
+        k_start = k_stop;
+        if (active > 0 && k_stop == 0xFFFFFFFFu) return fail(NECSIM_ERR_CAPACITY, "lineages still active at interval 2^32-1");
+    }
+    (void)params; (void)bytes;
+
+    // ---- S6: speciation records -> species (sort / unique / rank), labels, abundances ----------------
+    const u32 n_spec = hc->n_spec;
+    const u32 j_max = hc->j_max;
+    u32 richness = 0;
+    if (n_spec > 0) {
+        const u32 nb = (n_spec + NS_SORT_TILE - 1) / NS_SORT_TILE;
+        const u32 g256 = (n_spec + 255) / 256;
+        u32 *src = bf.spec_ring, *dst = perm_a, *other = perm_b;
+        // byte b of (j, loc, f, k) is skipped when it is zero for every record
+        const u32 maxv[4] = {j_max, (u32)(sd.n_locations - 1), 0, k_start};
+        for (u32 b = 0; b < 18; ++b) {
+            bool needed;
+            if (b < 4) needed = (maxv[0] >> (8 * b)) != 0;
+            else if (b < 8) needed = (maxv[1] >> (8 * (b - 4))) != 0;
+            else if (b < 14) needed = true;
+            else needed = (maxv[3] >> (8 * (b - 14))) != 0;
+            if (!needed) continue;
+            radix_hist_kernel<<<nb, 256, 0, st>>>(bf, src, n_spec, b, hist, nb);
+            scan_exclusive_kernel<<<1, 1024, 0, st>>>(hist, 256 * nb, NULL);
+            radix_scatter_kernel<<<nb, 256, 0, st>>>(bf, src, dst, n_spec, b, hist, nb);
+            src = dst; std::swap(dst, other);
+        }
+        CU(cudaGetLastError());
+        unique_flag_kernel<<<g256, 256, 0, st>>>(bf, src, n_spec, flag);
+        scan_exclusive_kernel<<<1, 1024, 0, st>>>(flag, n_spec, &bf.ctr->q_head);   // q_head reused: richness
+        unique_write_kernel<<<g256, 256, 0, st>>>(bf, src, n_spec, flag, events, species_of, sd.delta_t);
+        CU(cudaGetLastError());
+    }
+    label_kernel<<<(n_sampled + 255) / 256, 256, 0, st>>>(bf, n_sampled, species_of, events, labels);
+    CU(cudaGetLastError());
+    CU(cudaEventRecord(scn->ev[1], st));
+    CU(cudaMemcpyAsync(hc, bf.ctr, sizeof(SimCounters), cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    richness = n_spec ? hc->q_head : 0;
+    float ms_total = 0.f;
+    CU(cudaEventElapsedTime(&ms_total, scn->ev[0], scn->ev[1]));
+
+    out->richness = richness; out->n_lineages = n_sampled; out->n_unfinished = hc->n_unfinished;
+    out->d_events = events; out->d_labels = labels;
+    out->d_term_loc = bf.term_loc; out->d_term_k = bf.term_k; out->d_term_j = bf.term_j; out->d_steps = bf.steps;
+    out->d_term_f = bf.term_f; out->d_state = bf.state;
+    out->n_events_raw = hc->n_events; out->n_culled = hc->n_culled; out->n_speciation_raw = n_spec; out->n_epochs = n_epochs;
+    out->resample_attempts = hc->resamples; out->ms_simulate = ms_sim; out->ms_total = ms_total;
+    return NECSIM_OK;
+}
+
+static int simulate_checked(necsim_scenario *scn, uint64_t seed, double nu, const uint8_t *mask, bool mask_on_host, uint64_t cap,
+                            const necsim_sim_params *params, void *d_workspace, size_t bytes, void *cuda_stream, necsim_result *out,
+                            necsim_event *h_events, uint32_t *h_labels) {
+    if (!scn || !out) return fail(NECSIM_ERR_INVALID_ARG, "NULL argument");
+    if (!(nu >= 0.0 && nu <= 1.0)) return fail(NECSIM_ERR_INVALID_ARG, "nu must be in [0,1]");
+    ResolvedParams rp;
+    int rc = resolve_params(scn, params, rp);
+    if (rc) return rc;
+    if (nu == 0.0 && rp.max_steps == 0) return fail(NECSIM_ERR_INVALID_ARG, "nu = 0 never terminates (set max_steps)");
+    if (cap == 0 || cap > scn->n_individuals) return fail(NECSIM_ERR_INVALID_ARG, "n_sampled_capacity must be in [1, n_individuals]");
+    SimLayout L;
+    sim_layout(scn->n_individuals, cap, rp, L);
+    if (!d_workspace || bytes < L.total) return fail(NECSIM_ERR_WORKSPACE_TOO_SMALL, "simulate workspace too small");
+    if (((uintptr_t)d_workspace & 255u) != 0) return fail(NECSIM_ERR_INVALID_ARG, "workspace must be 256-byte aligned");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const uint8_t *d_mask = mask;
+    if (mask && mask_on_host) {
+        uint8_t *stage = (uint8_t *)d_workspace + L.off_mask;
+        CU(cudaMemcpyAsync(stage, mask, scn->n_individuals, cudaMemcpyHostToDevice, st));
+        d_mask = stage;
+    }
+    rc = simulate_impl(scn, seed, nu, d_mask, cap, params, d_workspace, bytes, st, out, L, rp);
+    if (rc) { cudaStreamSynchronize(st); return rc; }
+    if (h_events && out->richness) CU(cudaMemcpyAsync(h_events, out->d_events, sizeof(necsim_event) * out->richness, cudaMemcpyDeviceToHost, st));
+    if (h_labels) CU(cudaMemcpyAsync(h_labels, out->d_labels, 4 * out->n_lineages, cudaMemcpyDeviceToHost, st));
+    if (h_events || h_labels) CU(cudaStreamSynchronize(st));
+    return NECSIM_OK;
+}
+
+extern "C" int necsim_simulate(necsim_scenario *scn, uint64_t seed, double nu, const uint8_t *d_sample_mask, uint64_t n_sampled_capacity,
+                               const necsim_sim_params *params, void *d_workspace, size_t bytes, void *cuda_stream, necsim_result *out) {
+    return simulate_checked(scn, seed, nu, d_sample_mask, false, n_sampled_capacity, params, d_workspace, bytes, cuda_stream, out, NULL, NULL);
+}
+
+extern "C" int necsim_simulate_host(necsim_scenario *scn, uint64_t seed, double nu, const uint8_t *h_sample_mask, uint64_t n_sampled_capacity,
+                                    const necsim_sim_params *params, void *d_workspace, size_t bytes, void *cuda_stream, necsim_result *out,
+                                    necsim_event *h_events, uint32_t *h_labels) {
+    return simulate_checked(scn, seed, nu, h_sample_mask, true, n_sampled_capacity, params, d_workspace, bytes, cuda_stream, out, h_events, h_labels);
+}
+
+// ---------------------------------------------------------------------------------------------------
+// test-only exports: device primitives over arrays
+// ---------------------------------------------------------------------------------------------------
+__global__ void debug_draw_kernel(SeedKey key, int lane_kind, const u32 *loc, const u32 *k, const u32 *j, const u32 *r, u64 *out, u64 n) {
+    u64 i = (u64)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    u64 s = prime(key, loc[i], k[i]);
+    u64 X = s + (u64)j[i] * NS_GAMMA;
+    u64 v;
+    switch (lane_kind) {
+    case 0: v = draw_time(X); break;
+    case 1: v = draw_spec(X); break;
+    case 2: v = draw_disp(X, r ? r[i] : 0u); break;
+    case 3: v = draw_index(X); break;
+    case 4: v = draw_migr(X); break;
+    default: v = s; break;
+    }
+    out[i] = v;
+}
+__global__ void debug_neglog_kernel(const u64 *x, u64 *out, u64 n) {
+    __shared__ unsigned short sQ[512];
+    __shared__ u64 sA[512];
+    for (u32 i = threadIdx.x; i < 512; i += blockDim.x) { sQ[i] = NEGLOG_Q_DEV[i]; sA[i] = NEGLOG_A_DEV[i]; }
+    __syncthreads();
+    u64 i = (u64)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) out[i] = neglog(x[i], sQ, sA);
+}
+__global__ void debug_next_event_kernel(SeedKey key, const u32 *loc, const u32 *k, const i64 *f_last, const u32 *Cm, const u32 *sh, u32 *k_out,
+                                        u32 *j_out, u64 *T_out, int *rc, u64 n) {
+    __shared__ unsigned short sQ[512];
+    __shared__ u64 sA[512];
+    for (u32 i = threadIdx.x; i < 512; i += blockDim.x) { sQ[i] = NEGLOG_Q_DEV[i]; sA[i] = NEGLOG_A_DEV[i]; }
+    __syncthreads();
+    u64 i = (u64)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    u32 kk = k[i];
+    i64 fl = f_last[i];
+    for (;;) {
+        u64 X = prime(key, loc[i], kk), T = 0;
+        u32 j = 0;
+        bool crossed = false;
+        for (;;) {
+            j += 1; X += NS_GAMMA;
+            T += scale_exp(neglog(draw_time(X), sQ, sA), Cm[i], sh[i]);
+            if (T >= NS_TWO48) { crossed = true; break; }
+            if ((i64)T > fl) { k_out[i] = kk; j_out[i] = j; T_out[i] = T; rc[i] = 0; return; }
+        }
+        if (crossed) {
+            if (kk == 0xFFFFFFFFu) { k_out[i] = kk; j_out[i] = 0; T_out[i] = 0; rc[i] = -3; return; }
+            kk += 1; fl = -1;
+        }
+    }
+}
+template <int KIND>
+__global__ void debug_disperse_kernel(const ScenarioDev sc, SeedKey key, u64 thr_m, const u32 *loc, const u32 *k, const u32 *j, u32 *loc_out, u64 n) {
+    __shared__ u32 sG[KIND == 3 ? 1024 : 1];
+    if (KIND == 3) for (u32 i = threadIdx.x; i < sc.gauss_len; i += blockDim.x) sG[i] = sc.gauss[i];
+    __syncthreads();
+    u64 i = (u64)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    u32 cell = (KIND == 1) ? (loc[i] >= sc.J_local ? 1u : 0u) : cell_of_loc(sc, loc[i]);
+    u64 X = prime(key, loc[i], k[i]) + (u64)j[i] * NS_GAMMA;
+    u32 l2 = 0xFFFFFFFFu, c2 = 0, rs = 0;
+    disperse<KIND>(sc, thr_m, X, cell, l2, c2, sG, rs);
+    loc_out[i] = l2;
+}
+
+static inline u32 grid_for(u64 n, u32 block) { return (u32)((n + block - 1) / block); }
+
+extern "C" int necsim_debug_draw(uint64_t seed, int lane, const uint32_t *d_loc, const uint32_t *d_k, const uint32_t *d_j, const uint32_t *d_r,
+                                 uint64_t *d_out, uint64_t n, void *cuda_stream) {
+    if (n == 0) return NECSIM_OK;
+    debug_draw_kernel<<<grid_for(n, 256), 256, 0, (cudaStream_t)cuda_stream>>>(key_schedule(seed), lane, d_loc, d_k, d_j, d_r, d_out, n);
+    CU(cudaGetLastError());
+    return NECSIM_OK;
+}
+extern "C" int necsim_debug_neglog(const uint64_t *d_x, uint64_t *d_out, uint64_t n, void *cuda_stream) {
+    if (n == 0) return NECSIM_OK;
+    int rc = upload_neglog_tables((cudaStream_t)cuda_stream);
+    if (rc) return rc;
+    debug_neglog_kernel<<<grid_for(n, 256), 256, 0, (cudaStream_t)cuda_stream>>>(d_x, d_out, n);
+    CU(cudaGetLastError());
+    return NECSIM_OK;
+}
+extern "C" int necsim_debug_next_event(uint64_t seed, const uint32_t *d_loc, const uint32_t *d_k, const int64_t *d_f_last, const uint32_t *d_Cm,
+                                       const uint32_t *d_sh, uint32_t *d_k_out, uint32_t *d_j_out, uint64_t *d_T_out, int32_t *d_rc, uint64_t n,
+                                       void *cuda_stream) {
+    if (n == 0) return NECSIM_OK;
+    int rc = upload_neglog_tables((cudaStream_t)cuda_stream);
+    if (rc) return rc;
+    debug_next_event_kernel<<<grid_for(n, 256), 256, 0, (cudaStream_t)cuda_stream>>>(key_schedule(seed), d_loc, d_k, (const i64 *)d_f_last, d_Cm, d_sh,
+                                                                                      d_k_out, d_j_out, d_T_out, d_rc, n);
+    CU(cudaGetLastError());
+    return NECSIM_OK;
+}
+extern "C" int necsim_debug_disperse(const necsim_scenario *scn, uint64_t seed, const uint32_t *d_loc, const uint32_t *d_k, const uint32_t *d_j,
+                                     uint32_t *d_loc_out, uint64_t n, void *cuda_stream) {
+    if (!scn) return fail(NECSIM_ERR_INVALID_ARG, "NULL scenario");
+    if (n == 0) return NECSIM_OK;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    SeedKey key = key_schedule(seed);
+    u64 thr_m = thr53(scn->migration);
+    u32 g = grid_for(n, 256);
+    switch (scn->dev.kind) {
+    case 0: debug_disperse_kernel<0><<<g, 256, 0, st>>>(scn->dev, key, thr_m, d_loc, d_k, d_j, d_loc_out, n); break;
+    case 1: debug_disperse_kernel<1><<<g, 256, 0, st>>>(scn->dev, key, thr_m, d_loc, d_k, d_j, d_loc_out, n); break;
+    case 2: debug_disperse_kernel<2><<<g, 256, 0, st>>>(scn->dev, key, thr_m, d_loc, d_k, d_j, d_loc_out, n); break;
+    default: debug_disperse_kernel<3><<<g, 256, 0, st>>>(scn->dev, key, thr_m, d_loc, d_k, d_j, d_loc_out, n); break;
+    }
+    CU(cudaGetLastError());
+    return NECSIM_OK;
+}
+extern "C" int necsim_debug_tables(const necsim_scenario *scn, uint32_t *h_thresh, uint32_t *h_alias, uint32_t *h_gauss, int32_t *R_out,
+                                   uint32_t *h_Cm, uint32_t *h_sh, void *cuda_stream) {
+    if (!scn) return fail(NECSIM_ERR_INVALID_ARG, "NULL scenario");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const ScenarioDev &sd = scn->dev;
+    size_t n = sd.ncells;
+    if ((h_thresh || h_alias) && sd.alias) {
+        std::vector<uint2> tab(n * n);
+        CU(cudaMemcpyAsync(tab.data(), sd.alias, 8 * n * n, cudaMemcpyDeviceToHost, st));
+        CU(cudaStreamSynchronize(st));
+        for (size_t i = 0; i < n * n; ++i) { if (h_thresh) h_thresh[i] = tab[i].x; if (h_alias) h_alias[i] = tab[i].y; }
+    }
+    if (R_out) *R_out = sd.R;
+    if (h_gauss && sd.gauss) {
+        CU(cudaMemcpyAsync(h_gauss, sd.gauss, 4 * 2 * (size_t)sd.R, cudaMemcpyDeviceToHost, st));
+        CU(cudaStreamSynchronize(st));
+    }
+    if (h_Cm || h_sh) {
+        if (sd.per_cell_turnover) {
+            std::vector<uint2> sc(n);
+            CU(cudaMemcpyAsync(sc.data(), sd.scale, 8 * n, cudaMemcpyDeviceToHost, st));
+            CU(cudaStreamSynchronize(st));
+            for (size_t i = 0; i < n; ++i) { if (h_Cm) h_Cm[i] = sc[i].x; if (h_sh) h_sh[i] = sc[i].y; }
+        } else {
+            for (size_t i = 0; i < n; ++i) { if (h_Cm) h_Cm[i] = sd.Cm_u; if (h_sh) h_sh[i] = sd.sh_u; }
+        }
+    }
+    return NECSIM_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// integer-pipe peak micro-benchmark: independent chains, full occupancy
+// ---------------------------------------------------------------------------------------------------
+template <int KIND>
+__global__ void __launch_bounds__(256) int_peak_kernel(u32 iters, u32 *sink) {
+    u32 a0 = threadIdx.x * 2654435761u + 1u, a1 = a0 ^ 0x9E3779B9u, a2 = a0 + 0x7F4A7C15u, a3 = a1 * 3u;
+    u32 b0 = blockIdx.x + 17u, b1 = b0 ^ 0x85EBCA6Bu, b2 = b0 + 0xC2B2AE35u, b3 = b1 * 5u;
+    for (u32 it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            if (KIND == 0) {   // the hash round: IMAD.WIDE + LOP3 on four independent chains
+                feistel(a0, b0, NS_M6, NS_C6); feistel(a1, b1, NS_M7, NS_C7);
+                feistel(a2, b2, NS_M8, NS_C8); feistel(a3, b3, NS_M9, NS_C9);
+            } else if (KIND == 1) {   // IMAD only
+                a0 = a0 * NS_M6 + b0; a1 = a1 * NS_M7 + b1; a2 = a2 * NS_M8 + b2; a3 = a3 * NS_M9 + b3;
+                b0 = b0 * NS_M10 + a0; b1 = b1 * NS_M11 + a1; b2 = b2 * NS_M0 + a2; b3 = b3 * NS_M1 + a3;
+            } else {   // ALU only: LOP3 / SHF / IADD3
+                a0 = (a0 ^ b0 ^ NS_C6) + __funnelshift_l(a0, b0, 7); a1 = (a1 ^ b1 ^ NS_C7) + __funnelshift_l(a1, b1, 9);
+                a2 = (a2 ^ b2 ^ NS_C8) + __funnelshift_l(a2, b2, 11); a3 = (a3 ^ b3 ^ NS_C9) + __funnelshift_l(a3, b3, 13);
+                b0 = (b0 ^ a0 ^ NS_C10) + __funnelshift_l(b0, a0, 5); b1 = (b1 ^ a1 ^ NS_C11) + __funnelshift_l(b1, a1, 3);
+                b2 = (b2 ^ a2 ^ NS_C6) + __funnelshift_l(b2, a2, 15); b3 = (b3 ^ a3 ^ NS_C7) + __funnelshift_l(b3, a3, 17);
+            }
+        }
+    }
+    u32 r = a0 ^ a1 ^ a2 ^ a3 ^ b0 ^ b1 ^ b2 ^ b3;
+    if (r == 0x12345678u) sink[0] = r;   // keeps the chains alive
+}
+
+extern "C" int necsim_debug_int_peak(int kind, uint32_t iters, void *cuda_stream, double *thread_instr_per_s, float *ms_out) {
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int dev_id = 0, sm = 0;
+    CU(cudaGetDevice(&dev_id));
+    CU(cudaDeviceGetAttribute(&sm, cudaDevAttrMultiProcessorCount, dev_id));
+    u32 *sink = NULL;
+    CU(cudaMalloc((void **)&sink, 4));   // test-only export: the one place the library allocates
+    cudaEvent_t e0, e1;
+    CU(cudaEventCreate(&e0)); CU(cudaEventCreate(&e1));
+    const u32 grid = (u32)sm * 8u, block = 256u;
+    // instructions per inner step: KIND 0: 4 x (IMAD.WIDE + LOP3) = 8; KIND 1: 8 IMAD; KIND 2: 8 x (LOP3 + SHF + IADD3) = 24
+    const double per_step = kind == 0 ? 8.0 : (kind == 1 ? 8.0 : 24.0);
+    for (int rep = 0; rep < 2; ++rep) {
+        if (rep == 1) CU(cudaEventRecord(e0, st));
+        if (kind == 0) int_peak_kernel<0><<<grid, block, 0, st>>>(iters, sink);
+        else if (kind == 1) int_peak_kernel<1><<<grid, block, 0, st>>>(iters, sink);
+        else int_peak_kernel<2><<<grid, block, 0, st>>>(iters, sink);
+    }
+    CU(cudaEventRecord(e1, st));
+    CU(cudaStreamSynchronize(st));
+    float ms = 0.f;
+    CU(cudaEventElapsedTime(&ms, e0, e1));
+    if (ms_out) *ms_out = ms;
+    if (thread_instr_per_s) *thread_instr_per_s = per_step * 8.0 * (double)iters * (double)grid * (double)block / ((double)ms * 1e-3);
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(sink);
+    return NECSIM_OK;
+}

@@ -1,0 +1,230 @@
+// sim_kernel.cuh -- the persistent lineage-scheduler kernel.
+//
+// One lineage per lane (PAPER.md 5.2 L675-747: "each lineage simulated alone"). A lane whose lineage
+// ended (speciated / culled as a duplicate / reached the epoch's time horizon / step cap) takes the
+// next lineage from the device work queue: one atomicAdd per warp per refill (ballot + popc).
+// The loop body is a state machine that performs exactly one event-time draw per iteration for every
+// live lane (sum Exp draws from the interval start until the first partial sum
+// after the lineage's last event), so lanes of a warp only diverge on the rarer event branch.
+#pragma once
+#include "sim_types.cuh"
+
+namespace necsim {
+
+#define NS_FULL 0xFFFFFFFFu
+#define NS_MAX_RESAMPLE (1u << 20)
+
+__device__ __forceinline__ u32 lanemask_lt() {
+    u32 m;
+    asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
+    return m;
+}
+
+// rounded-normal displacement: G(u) = -R + #{i : u >= TG[i]}  (R15). tg: padded table in smem.
+__device__ __forceinline__ int gauss_disp(const u32 *tg, u32 len, int R, u32 u) {
+    u32 pos = 0;
+    for (u32 s = len >> 1; s; s >>= 1)
+        if (tg[pos + s - 1] <= u) pos += s;
+    pos += (tg[pos] <= u) ? 1u : 0u;
+    int c = (int)min(pos, (u32)(2 * R));
+    return c - R;
+}
+
+__device__ __forceinline__ u32 cell_deme(const ScenarioDev &sc, u32 cell) {
+    if (sc.uniform_deme) return sc.uniform_deme;
+    u32 d = sc.hab8[cell];
+    if (d == 255u) d = sc.deme32[cell];
+    return d;
+}
+__device__ __forceinline__ u32 cell_prefix(const ScenarioDev &sc, u32 cell) {
+    return sc.uniform_deme ? cell * sc.uniform_deme : sc.prefix[cell];
+}
+
+// DESIGN.md 2.5 step 2: dispersal of the event at stream position X from (loc, cell). Returns false on
+// resampling exhaustion. `resamples` counts rejected targets.
+template <int KIND>
+__device__ __forceinline__ bool disperse(const ScenarioDev &sc, u64 thr_m, u64 X, u32 cell, u32 &loc2, u32 &cell2,
+                                         const u32 *tg, u32 &resamples) {
+    if (KIND == 0) {  // NONSPATIAL: uniform over all J positions, self allowed (R12)
+        loc2 = mulhi64_u32(draw_disp(X, 0), (u32)sc.n_locations);
+        cell2 = 0;
+        return true;
+    } else if (KIND == 1) {  // SPATIALLY_IMPLICIT (L294-298, L1830; R13)
+        u64 x = draw_disp(X, 0);
+        bool to_meta = (cell != 0) || bern(draw_migr(X), thr_m);
+        if (to_meta) { loc2 = sc.J_local + mulhi64_u32(x, sc.J_meta); cell2 = 1; }
+        else         { loc2 = mulhi64_u32(x, sc.J_local); cell2 = 0; }
+        return true;
+    } else if (KIND == 2) {  // EXPLICIT_MATRIX: alias-table gather (R18)
+        u64 x = draw_disp(X, 0);
+        u32 n = sc.ncells;
+        u32 col = __umulhi((u32)(x >> 32), n);
+        uint2 e = __ldg(&sc.alias[(size_t)cell * n + col]);
+        u32 c2 = ((u32)x < e.x) ? col : e.y;
+        u32 d = cell_deme(sc, c2);
+        u32 idx = (d == 1u) ? 0u : mulhi64_u32(draw_index(X), d);
+        cell2 = c2;
+        loc2 = cell_prefix(sc, c2) + idx;
+        return true;
+    } else {  // EXPLICIT_GAUSSIAN: rounded normal on a torus, resample until habitat (R15-R17)
+        u32 x0, y0;
+        if (sc.width_shift != 0xFFFFFFFFu) { x0 = cell & (sc.width - 1); y0 = cell >> sc.width_shift; }
+        else { y0 = cell / sc.width; x0 = cell - y0 * sc.width; }
+        for (u32 r = 0; r < NS_MAX_RESAMPLE; ++r) {
+            u64 x = draw_disp(X, r);
+            int dx = gauss_disp(tg, sc.gauss_len, sc.R, (u32)(x >> 32));
+            int dy = gauss_disp(tg, sc.gauss_len, sc.R, (u32)x);
+            int xx = (int)x0 + dx, yy = (int)y0 + dy;      // |d| <= R < min(width, height): one wrap suffices
+            if (xx < 0) xx += (int)sc.width; else if (xx >= (int)sc.width) xx -= (int)sc.width;
+            if (yy < 0) yy += (int)sc.height; else if (yy >= (int)sc.height) yy -= (int)sc.height;
+            u32 c2 = (u32)yy * sc.width + (u32)xx;
+            u32 d = cell_deme(sc, c2);
+            if (d > 0) {
+                u32 idx = (d == 1u) ? 0u : mulhi64_u32(draw_index(X), d);
+                cell2 = c2;
+                loc2 = cell_prefix(sc, c2) + idx;
+                return true;
+            }
+            ++resamples;
+        }
+        return false;
+    }
+}
+
+__device__ __forceinline__ u32 cache_slot(u32 loc, u32 k, u32 j, u32 mask) {
+    // slot hash only chooses a bucket; a hit always compares the full key
+    u32 h = loc * 0x9E3779B1u;
+    h ^= (k + j * 0x7FEB352Du) * 0x85EBCA6Bu;
+    h ^= h >> 15;
+    h *= 0x2C1B3C6Du;
+    h ^= h >> 13;
+    return h & mask;
+}
+
+// -ln tables in global memory (filled once per process from neglog_tables.inc), staged to smem per block
+__device__ unsigned short NEGLOG_Q_DEV[512];
+__device__ u64 NEGLOG_A_DEV[512];
+
+template <int KIND, bool DEDUP>
+__global__ void __launch_bounds__(256) simulate_kernel(const ScenarioDev sc, const SimBuffers bf, const EpochArgs ep) {
+    __shared__ unsigned short sQ[512];
+    __shared__ u64 sA[512];
+    __shared__ u32 sG[KIND == 3 ? 1024 : 1];
+    for (u32 i = threadIdx.x; i < 512; i += blockDim.x) { sQ[i] = NEGLOG_Q_DEV[i]; sA[i] = NEGLOG_A_DEV[i]; }
+    if (KIND == 3) for (u32 i = threadIdx.x; i < sc.gauss_len; i += blockDim.x) sG[i] = sc.gauss[i];
+    __syncthreads();
+
+    const u32 lane = threadIdx.x & 31u;
+    const bool lane_on = lane < ep.lanes_per_warp;
+
+    // lineage state (registers)
+    bool has = false, need_prime = false, exhausted = false;
+    u32 id = 0, loc = 0, cell = 0, k = 0, steps = 0, j = 0, Cm = sc.Cm_u, sh = sc.sh_u;
+    i64 f_last = -1;
+    u64 X = 0, T = 0;
+    u32 c_events = 0, c_culled = 0, c_resamples = 0;   // per-thread counters, reduced at the end
+
+    for (;;) {
+        // ---- S4: refill idle lanes from the device work queue (one atomic per warp) -----------------
+        u32 need = __ballot_sync(NS_FULL, lane_on && !has);
+        if (need != 0u && !exhausted) {
+            u32 cnt = __popc(need), base = 0;
+            if (lane == 0) base = atomicAdd(&bf.ctr->q_head, cnt);
+            base = __shfl_sync(NS_FULL, base, 0);
+            if (lane_on && !has) {
+                u32 idx = base + __popc(need & lanemask_lt());
+                if (idx < bf.q_in_count) {
+                    uint4 e = bf.q_in[idx];
+                    id = e.x; loc = e.y; cell = e.z; steps = e.w;
+                    k = ep.k_start; f_last = -1; need_prime = true; has = true;
+                }
+            }
+            exhausted = (base + cnt >= bf.q_in_count);
+        }
+        if (!__any_sync(NS_FULL, has)) break;
+
+        // ---- S1a: (re-)prime on (loc, k); pause at the epoch horizon -------------------------------
+        bool pause = false;
+        if (has && need_prime) {
+            if (k == ep.k_stop) {
+                pause = true;
+            } else {
+                X = prime(ep.key, loc, k);
+                T = 0; j = 0; need_prime = false;
+                if (sc.per_cell_turnover) { uint2 cs = __ldg(&sc.scale[cell]); Cm = cs.x; sh = cs.y; }
+            }
+        }
+        {   // survivors of this epoch go to the output queue (warp-aggregated append)
+            u32 pm = __ballot_sync(NS_FULL, pause);
+            if (pm) {
+                u32 base = 0;
+                if (lane == (u32)(__ffs(pm) - 1)) base = atomicAdd(&bf.ctr->q_out, __popc(pm));
+                base = __shfl_sync(NS_FULL, base, __ffs(pm) - 1);
+                if (pause) {
+                    bf.q_out[base + __popc(pm & lanemask_lt())] = make_uint4(id, loc, cell, steps);
+                    has = false;
+                }
+            }
+        }
+        if (!has) continue;
+
+        // ---- S1b: one exponential draw of the event-time search ------------------------------------
+        j += 1; X += NS_GAMMA;
+        T += scale_exp(neglog(draw_time(X), sQ, sA), Cm, sh);
+        if (T >= NS_TWO48) {                       // interval exhausted: cross and re-prime (L719, L727)
+            if (k == 0xFFFFFFFFu) { atomicMax(&bf.ctr->error, 3u); has = false; continue; }
+            k += 1; f_last = -1; need_prime = true;
+            continue;
+        }
+        if ((i64)T <= f_last) continue;            // not strictly later than the last event (L729)
+
+        // ---- event (loc, k, j) at offset T ----------------------------------------------------------
+        if (DEDUP) {   // S5: duplicate-culling cache keyed on the full event identity
+            uint4 mine = make_uint4(loc, k, j, id);
+            uint4 old = atomic_exch_128(&bf.cache[cache_slot(loc, k, j, bf.cache_mask)], mine);
+            if (old.x == loc && old.y == k && old.z == j && old.w != id) {
+                // another lineage executed this event: identical future (L687, L697) -> cull, link to it
+                bf.parent[id] = old.w; bf.state[id] = 2;
+                bf.term_loc[id] = loc; bf.term_k[id] = k; bf.term_j[id] = j; bf.term_f[id] = T; bf.steps[id] = steps;
+                c_culled++; has = false;
+                continue;
+            }
+        }
+        f_last = (i64)T; steps++; c_events++;
+        // S2: speciation test on the event's SPEC lane
+        bool can_speciate = !(KIND == 1 && cell == 0);     // local community of the implicit model: nu = 0 (L1830)
+        if (can_speciate && bern(draw_spec(X), ep.thr_nu)) {
+            bf.state[id] = 1;
+            bf.term_loc[id] = loc; bf.term_k[id] = k; bf.term_j[id] = j; bf.term_f[id] = T; bf.steps[id] = steps;
+            bf.spec_ring[atomicAdd(&bf.ctr->n_spec, 1u)] = id;
+            atomicMax(&bf.ctr->j_max, j);
+            has = false;
+            continue;
+        }
+        // S3: dispersal to the parent's location
+        u32 loc2, cell2;
+        if (!disperse<KIND>(sc, ep.thr_m, X, cell, loc2, cell2, sG, c_resamples)) {
+            atomicMax(&bf.ctr->error, 3u); has = false; continue;
+        }
+        loc = loc2; cell = cell2; need_prime = true;
+        if (ep.max_steps && steps >= ep.max_steps) {
+            bf.state[id] = 3;
+            bf.term_loc[id] = loc; bf.term_k[id] = k; bf.term_j[id] = j; bf.term_f[id] = T; bf.steps[id] = steps;
+            has = false;
+        }
+    }
+    // reduce the per-thread counters: warp shuffle, then one atomic per warp
+    unsigned long long r_events = c_events, r_culled = c_culled, r_resamples = c_resamples;
+    for (int o = 16; o; o >>= 1) {
+        r_events += __shfl_down_sync(NS_FULL, r_events, o);
+        r_culled += __shfl_down_sync(NS_FULL, r_culled, o);
+        r_resamples += __shfl_down_sync(NS_FULL, r_resamples, o);
+    }
+    if (lane == 0) {
+        if (r_events) atomicAdd((unsigned long long *)&bf.ctr->n_events, r_events);
+        if (r_culled) atomicAdd((unsigned long long *)&bf.ctr->n_culled, r_culled);
+        if (r_resamples) atomicAdd((unsigned long long *)&bf.ctr->resamples, r_resamples);
+    }
+}
+
+}  // namespace necsim

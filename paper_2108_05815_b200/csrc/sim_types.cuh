@@ -1,0 +1,67 @@
+// sim_types.cuh -- plain structs passed by value to the kernels (constants live in the kernel
+// parameter bank, the analogue of the paper's PTX-JIT constant folding).
+#pragma once
+#include "device_prims.cuh"
+
+namespace necsim {
+
+// Device view of a scenario (tables live in the caller's scenario workspace).
+struct ScenarioDev {
+    int kind;
+    u32 width, height, ncells;
+    u32 width_shift;           // log2(width) if width is a power of two, else 0xFFFFFFFF
+    u32 uniform_deme;          // != 0: every cell has this deme (no per-cell deme/prefix gathers needed)
+    u32 per_cell_turnover;     // 0: Cm_u/sh_u apply everywhere
+    u32 Cm_u, sh_u;
+    u64 n_locations;           // all indexed locations
+    u64 n_sampleable;          // domain of the sample mask
+    u32 J_local, J_meta;       // spatially implicit
+    const uint8_t *hab8;       // [ncells] min(deme, 255)
+    const u32 *deme32;         // [ncells] full deme (read only where hab8 == 255)
+    const u32 *prefix;         // [ncells+1] exclusive prefix sum of deme
+    const uint2 *scale;        // [ncells] (Cm, sh) when per_cell_turnover
+    const uint2 *alias;        // [ncells*ncells] (thresh, alias) for EXPLICIT_MATRIX
+    const u32 *gauss;          // [gauss_len] rounded-normal thresholds, padded with 0xFFFFFFFF to a power of two
+    int R;                     // displacement range: dx in [-R, R]
+    u32 gauss_len;             // power of two >= 2R
+    double delta_t;
+};
+
+// Device counters of one simulate call (zeroed at its start). 64-bit where they can exceed 2^32.
+struct SimCounters {
+    u32 q_head;                // next entry of the input queue to hand out
+    u32 q_out;                 // entries written to the output queue (survivors of this epoch)
+    u32 n_spec;                // speciation records in the ring
+    u32 error;                 // sticky NECSIM_ERR_* (positive value of the negative code)
+    u32 j_max;                 // largest event ordinal seen in a speciation record
+    u32 n_unfinished;
+    u32 n_sampled;             // written by the init kernels
+    u32 pad;
+    u64 n_events;              // events executed (raw)
+    u64 n_culled;
+    u64 resamples;
+};
+
+// Per-lineage SoA outputs + queues + dedup cache (all inside the simulate workspace).
+struct SimBuffers {
+    uint4 *q_in;               // {id, loc, cell, steps}
+    uint4 *q_out;
+    u32 q_in_count;
+    uint4 *cache;              // {loc, k, j, owner id}; 0xFF.. = empty
+    u32 cache_mask;
+    u32 *term_loc, *term_k, *term_j, *steps, *parent, *spec_ring;
+    u64 *term_f;
+    uint8_t *state;            // 0 active, 1 speciated, 2 culled, 3 stopped by max_steps
+    SimCounters *ctr;
+};
+
+struct EpochArgs {
+    SeedKey key;
+    u64 thr_nu, thr_m;
+    u32 k_start;               // every queued lineage is fresh at the start of interval k_start
+    u32 k_stop;                // horizon: a lineage pauses when its interval index reaches k_stop
+    u32 max_steps;             // 0 = unlimited
+    u32 lanes_per_warp;        // lanes of each warp that hold lineages (32 = saturated; fewer in the tail)
+};
+
+}  // namespace necsim
