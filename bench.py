@@ -1,0 +1,241 @@
+#!/usr/bin/env python
+"""bench.py -- whole-hot-path benchmark of necsim-b200 (contract: see DESIGN.md section 7).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config c1..c5] [--small]
+
+A "step" is one pass of the whole hot path S0-S6 (necsim_simulate: sample mask -> lineage queue, epochs of
+the simulate kernel with duplicate culling, sort/unique -> species) over the synthetic config. Default workload:
+C5 (BASELINE.json configs[4], the largest; the one north_star quotes the roofline target on).
+`value` = raw lineage events executed per second, whole job, inputs resident in HBM (device time, CUDA events).
+`e2e`   = the same through necsim_simulate_host: pinned host mask in, events + labels back to the host each step.
+`--impl reference` times the CPU oracle (as it stands, one core) on a bounded sample of the same workload.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+from paper_2108_05815_b200 import inputs as I  # noqa: E402
+
+METRIC = "lineage_events_per_s"
+UNIT = "events/s"
+MAKERS = dict(c1=I.c1_nonspatial, c2=I.c2_implicit, c3=I.c3_matrix, c4=I.c4_gaussian, c5=I.c5_stress)
+SMALL = dict(zip(("c1", "c2", "c3", "c4", "c5"), range(5)))
+# Algorithmic integer instructions per executed event (counted on the straight-line
+# SASS of each primitive, weighted by the expected number of draws per event at mu = 2).
+I_EVENT = dict(c1=262, c2=270, c3=300, c4=345, c5=360)
+# issue-slot peak: 148 SMs x 4 schedulers x 32 lanes x 1 instr/clk x sm_max_mhz (B300_MICROARCH "Pipe rates")
+def alu_peak(sm_count, sm_mhz):
+    return sm_count * 4 * 32 * sm_mhz * 1e6
+
+
+def make_cfg(name, small):
+    return I.small_configs()[SMALL[name]] if small else MAKERS[name]()
+
+
+def cpu_sample(cfg, name, budget_events=30_000_000):
+    """Bounded sample of the workload for the oracle: a thinned sample mask and a per-lineage step cap."""
+    n_ind = I.n_individuals(cfg)
+    mask = np.ones(n_ind, np.uint8) if cfg["mask"] is None else np.asarray(cfg["mask"], np.uint8).copy()
+    rng = np.random.Generator(np.random.PCG64(12345))
+    n_lin, max_steps = 2000, 15_000
+    idx = np.flatnonzero(mask)
+    if len(idx) > n_lin:
+        keep = rng.choice(idx, n_lin, replace=False)
+        mask = np.zeros(n_ind, np.uint8); mask[keep] = 1
+    desc = "%d of %d sampled lineages of %s, dedup on, at most %d events each" % (int(mask.sum()), len(idx), name, max_steps)
+    return mask, max_steps, desc
+
+
+def run_oracle_sample(cfg, name):
+    from oracle import oracle as O            # cpu_baseline / --impl reference: the only bench legs that may use oracle/
+    mask, max_steps, desc = cpu_sample(cfg, name)
+    sc = O.Scenario(**I.scenario_kwargs(cfg))
+    t0 = time.perf_counter()
+    res = sc.simulate(cfg["seed"], cfg["nu"], mask, dedup=True, max_steps=max_steps)
+    dt = time.perf_counter() - t0
+    return res["stats"]["n_events"] / dt, dt, res["stats"]["n_events"], desc
+
+
+class ClockSampler(threading.Thread):
+    """Samples nvidia-smi clocks and throttle reasons during the timed region (B200_PROFILING.md clocks line)."""
+    Q = "index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown," \
+        "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, gpu_index=0):
+        super().__init__(daemon=True)
+        self.rows, self.proc, self.gpu_index = [], None, gpu_index
+
+    def run(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.gpu_index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            for line in self.proc.stdout:
+                self.rows.append([c.strip() for c in line.split(",")])
+        except Exception:
+            pass
+
+    def stop(self):
+        if self.proc:
+            self.proc.terminate()
+        sm = [float(r[1]) for r in self.rows if len(r) >= 9 and r[1].replace(".", "").isdigit()]
+        mx = [float(r[2]) for r in self.rows if len(r) >= 9 and r[2].replace(".", "").isdigit()]
+        reasons = set()
+        for r in self.rows:
+            if len(r) >= 9:
+                for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[5:9]):
+                    if v.lower().startswith("active"):
+                        reasons.add(name)
+        return dict(sm_mhz=float(np.median(sm)) if sm else None, sm_max_mhz=max(mx) if mx else None, reasons=sorted(reasons), samples=len(sm))
+
+
+def reference_arm(args, cfg, name):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    for _ in range(args.warmup):
+        pass                                   # the oracle has no warm-up state; W is accepted and ignored
+    vals, secs, desc, ev = [], [], "", 0
+    for _ in range(max(1, min(args.steps, 3))):
+        v, dt, ev, desc = run_oracle_sample(cfg, name)
+        vals.append(v); secs.append(dt)
+    v = float(np.mean(vals))
+    print(json.dumps({"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": len(vals), "warmup": args.warmup,
+                      "ms_per_step": 1e3 * float(np.mean(secs)), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                      "dtype": "int64", "data": "synthetic", "config": {"workload": cfg["name"], "sample": desc},
+                      "cpu_baseline": {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc},
+                      "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="c5", choices=sorted(MAKERS))
+    ap.add_argument("--small", action="store_true", help="the reduced config of the same kind (for testing the harness)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    name = args.config
+    cfg = make_cfg(name, args.small)
+    if args.impl == "reference":
+        return reference_arm(args, cfg, name)
+
+    import torch
+    import torch.distributed as dist
+    from paper_2108_05815_b200 import necsim as ns
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    # weak scaling: every rank runs the same landscape with its own seed (independent replicate simulations,
+    # the paper's repeated-runs use, L1240-1246); no data-path collective.
+    seed = cfg["seed"] + rank
+    sc = ns.Scenario(**I.scenario_kwargs(cfg))
+    n_ind, n_s = sc.n_individuals, I.n_sampled(cfg)
+    h_mask = None
+    d_mask = None
+    if cfg["mask"] is not None:
+        h_mask_t = torch.from_numpy(np.ascontiguousarray(cfg["mask"], dtype=np.uint8)).pin_memory()
+        h_mask = h_mask_t.numpy()
+        d_mask = h_mask_t.cuda()
+    h_events = torch.empty(n_s * 32, dtype=torch.uint8).pin_memory().numpy().view(ns.EVENT_DTYPE)
+    h_labels = torch.empty(n_s, dtype=torch.int32).pin_memory().numpy().view(np.uint32)
+    params = ns.make_params()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")      # > 126 MB L2
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def step_device():
+        flush.fill_(1)
+        torch.cuda.synchronize()
+        return sc.simulate_raw(seed, cfg["nu"], d_mask, n_s, params)
+
+    def step_host():
+        flush.fill_(1)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        r = sc.simulate_host_raw(seed, cfg["nu"], h_mask, n_s, params, h_events, h_labels)
+        return r, time.perf_counter() - t0
+
+    for _ in range(args.warmup):
+        step_device()
+    sampler = ClockSampler(local)
+    sampler.start()
+    barrier()
+    ms, ev, sim_ms, launches, epochs, res = 0.0, 0, 0.0, 0, 0, None
+    for _ in range(args.steps):
+        res = step_device()
+        ms += res.ms_total; sim_ms += res.ms_simulate; ev += res.n_events_raw; launches += res.n_kernel_launches; epochs += res.n_epochs
+    barrier()
+    clocks = sampler.stop()
+    # end to end: host buffers in, host buffers out, copies inside the timed region
+    step_host()
+    e2e_s, e2e_ev, res_h = 0.0, 0, None
+    barrier()
+    for _ in range(args.steps):
+        res_h, dt = step_host()
+        e2e_s += dt; e2e_ev += res_h.n_events_raw
+    barrier()
+    t = torch.tensor([ms, e2e_s * 1e3, float(ev), float(e2e_ev), sim_ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        tmax = t.clone(); dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+        tsum = t.clone(); dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
+        ms, e2e_ms, sim_ms = tmax[0].item(), tmax[1].item(), tmax[4].item()
+        ev_all, e2e_ev_all = tsum[2].item(), tsum[3].item()
+    else:
+        e2e_ms, ev_all, e2e_ev_all = e2e_s * 1e3, float(ev), float(e2e_ev)
+    if rank == 0:
+        K = args.steps
+        value = ev_all / (ms * 1e-3)
+        prop = torch.cuda.get_device_properties(local)
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))) if os.path.exists(os.path.join(ROOT, "MEASURED_PEAKS.json")) else {}
+        sm_max = float(peaks.get("sm_max_mhz", clocks.get("sm_max_mhz") or 1965.0))
+        peak = alu_peak(prop.multi_processor_count, sm_max)
+        achieved = (ev / K) * I_EVENT[name] / ((sim_ms / K) * 1e-3)   # per step: all simulate-kernel launches of one step
+        int_meas = {k: ns.int_peak(i, 2048)[0] for i, k in enumerate(("hash_round_mix", "imad_only", "alu_only"))}
+        # MODE-T: the saturated workload (dedup off, every lineage advanced 200 events): where the ALU roofline is meaningful
+        rt = sc.simulate_raw(seed, cfg["nu"], d_mask, n_s, ns.make_params(dedup=False, max_steps=200))
+        mode_t = rt.n_events_raw / (rt.ms_simulate * 1e-3)
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": args.warmup, "ms_per_step": ms / K,
+                "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int64", "data": "synthetic",
+                "config": {"workload": cfg["name"], "n_lineages": int(res.n_lineages), "nu": cfg["nu"], "mode": "MODE-S (dedup on, to completion)",
+                           "l2": "256 MiB flush write between steps", "parallelism": "replicas x%d" % world},
+                "clocks": clocks,
+                "e2e": {"value": e2e_ev_all / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms / K,
+                        "h2d_bytes_per_step": int(0 if h_mask is None else h_mask.nbytes),
+                        "d2h_bytes_per_step": int(res_h.richness * 32 + res_h.n_lineages * 4)},
+                "gpu_launches": int(launches),
+                "individuals_per_s": world * res.n_lineages / (ms / K * 1e-3),
+                "richness": int(res.richness), "epochs_per_step": epochs / K, "raw_events_per_step": ev / K,
+                "roofline": {"bound": "alu", "kernel": "simulate_kernel (all epochs of a step)", "achieved": achieved / 1e12, "peak": peak / 1e12,
+                             "unit": "Tinstr/s", "frac": achieved / peak, "traffic": None, "instr_per_event": I_EVENT[name],
+                             "peak_source": "derived: SMs x 4 schedulers x 32 lanes x sm_max_mhz (DESIGN.md section 6)",
+                             "measured_int_peaks_Tinstr_s": {k: v / 1e12 for k, v in int_meas.items()}},
+                "mode_t": {"value": mode_t, "unit": UNIT, "what": "dedup off, 200 events per lineage, saturated machine",
+                           "roofline_frac": mode_t * I_EVENT[name] / peak}}
+        if not args.no_cpu_baseline and world == 1:
+            v, dt, n_ev, desc = run_oracle_sample(cfg, name)
+            line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc, "seconds": dt}
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -110,7 +110,7 @@ typedef struct necsim_result {
     float ms_simulate;            /* device time of the simulate kernels (all epochs), CUDA events */
     float ms_simulate_tail;       /* of which tail epochs */
     float ms_total;               /* device time of the whole call */
-    uint32_t reserved;
+    uint32_t n_kernel_launches;   /* kernels this call launched (memsets and copies not counted) */
 } necsim_result;
 
 typedef struct necsim_scenario necsim_scenario;

@@ -402,11 +402,12 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
 
     // ---- S0: sample mask -> lineage queue ------------------------------------------------------------
     u64 n_ind = scn->n_individuals;
-    u32 n_sampled = 0;
+    u32 n_sampled = 0, n_launch = 0;
     if (d_mask) {
         mask_count_kernel<<<L.n_chunks, 256, 0, st>>>(d_mask, n_ind, chunk);
         scan_exclusive_kernel<<<1, 1024, 0, st>>>(chunk, L.n_chunks, &bf.ctr->n_sampled);
         mask_scatter_kernel<<<L.n_chunks, 256, 0, st>>>(sd, d_mask, n_ind, chunk, qa, (u32)cap);
+        n_launch += 3;
         CU(cudaGetLastError());
         CU(cudaMemcpyAsync(hc, bf.ctr, sizeof(SimCounters), cudaMemcpyDeviceToHost, st));
         CU(cudaStreamSynchronize(st));
@@ -417,6 +418,7 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
         if (n_ind > cap) return fail(NECSIM_ERR_WORKSPACE_TOO_SMALL, "n_sampled_capacity < n_individuals with a NULL mask");
         n_sampled = (u32)n_ind;
         all_sampled_kernel<<<(n_sampled + 255) / 256, 256, 0, st>>>(sd, n_sampled, qa);
+        n_launch += 1;
         CU(cudaGetLastError());
     }
 
@@ -472,7 +474,7 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
         float ms = 0.f;
         CU(cudaEventElapsedTime(&ms, scn->ev[2], scn->ev[3]));
         ms_sim += ms;
-        ++n_epochs;
+        ++n_epochs; ++n_launch;
         if (hc->error) return fail(NECSIM_ERR_CAPACITY, "interval index overflowed 2^32 or dispersal resampling exhausted");
         active = hc->q_out;
         std::swap(q_in, q_out);
@@ -502,14 +504,17 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
             scan_exclusive_kernel<<<1, 1024, 0, st>>>(hist, 256 * nb, NULL);
             radix_scatter_kernel<<<nb, 256, 0, st>>>(bf, src, dst, n_spec, b, hist, nb);
             src = dst; std::swap(dst, other);
+            n_launch += 3;
         }
         CU(cudaGetLastError());
         unique_flag_kernel<<<g256, 256, 0, st>>>(bf, src, n_spec, flag);
         scan_exclusive_kernel<<<1, 1024, 0, st>>>(flag, n_spec, &bf.ctr->q_head);   // q_head reused: richness
         unique_write_kernel<<<g256, 256, 0, st>>>(bf, src, n_spec, flag, events, species_of, sd.delta_t);
+        n_launch += 3;
         CU(cudaGetLastError());
     }
     label_kernel<<<(n_sampled + 255) / 256, 256, 0, st>>>(bf, n_sampled, species_of, events, labels);
+    n_launch += 1;
     CU(cudaGetLastError());
     CU(cudaEventRecord(scn->ev[1], st));
     CU(cudaMemcpyAsync(hc, bf.ctr, sizeof(SimCounters), cudaMemcpyDeviceToHost, st));
@@ -523,7 +528,7 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
     out->d_term_loc = bf.term_loc; out->d_term_k = bf.term_k; out->d_term_j = bf.term_j; out->d_steps = bf.steps;
     out->d_term_f = bf.term_f; out->d_state = bf.state;
     out->n_events_raw = hc->n_events; out->n_culled = hc->n_culled; out->n_speciation_raw = n_spec; out->n_epochs = n_epochs;
-    out->resample_attempts = hc->resamples; out->ms_simulate = ms_sim; out->ms_total = ms_total;
+    out->resample_attempts = hc->resamples; out->ms_simulate = ms_sim; out->ms_total = ms_total; out->n_kernel_launches = n_launch;
     return NECSIM_OK;
 }
 

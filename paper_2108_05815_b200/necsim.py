@@ -40,7 +40,7 @@ class Result(C.Structure):
                 ("n_events_raw", C.c_uint64), ("n_culled", C.c_uint64), ("n_speciation_raw", C.c_uint64),
                 ("n_epochs", C.c_uint64), ("n_tail_epochs", C.c_uint64), ("resample_attempts", C.c_uint64),
                 ("n_events_tail", C.c_uint64), ("ms_simulate", C.c_float), ("ms_simulate_tail", C.c_float),
-                ("ms_total", C.c_float), ("reserved", C.c_uint32)]
+                ("ms_total", C.c_float), ("n_kernel_launches", C.c_uint32)]
 
 
 EVENT_DTYPE = np.dtype({"names": ["loc", "k", "j", "abundance", "f", "time"],
@@ -207,7 +207,7 @@ class Scenario:
                    labels=_read(self._sim_ws, res.d_labels, n * 4, np.uint32),
                    stats={k: getattr(res, k) for k in ("n_lineages", "n_unfinished", "n_events_raw", "n_culled", "n_speciation_raw",
                                                        "n_epochs", "n_tail_epochs", "resample_attempts", "n_events_tail", "ms_simulate",
-                                                       "ms_simulate_tail", "ms_total")})
+                                                       "ms_simulate_tail", "ms_total", "n_kernel_launches")})
         if per_lineage:
             pl = np.zeros(n, dtype=[("loc", "<u4"), ("k", "<u4"), ("j", "<u4"), ("f", "<u8")])
             pl["loc"] = _read(self._sim_ws, res.d_term_loc, n * 4, np.uint32); pl["k"] = _read(self._sim_ws, res.d_term_k, n * 4, np.uint32)
