@@ -10,7 +10,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OUT = os.path.join(CSRC, "libnecsim_b200.so")
 SOURCES = ["necsim.cu"]
-DEPS = ["necsim.cu", "device_prims.cuh", "sim_types.cuh", "sim_kernel.cuh", "aux_kernels.cuh", "neglog_tables.inc",
+DEPS = ["necsim.cu", "device_prims.cuh", "sim_types.cuh", "sim_kernel.cuh", "tail_kernel.cuh", "aux_kernels.cuh", "neglog_tables.inc",
         os.path.join("..", "..", "include", "necsim.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "--fmad=false",
               "-Xcompiler", "-fPIC", "-shared"]

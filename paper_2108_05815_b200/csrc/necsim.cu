@@ -14,6 +14,7 @@
 #include "device_prims.cuh"
 #include "sim_types.cuh"
 #include "sim_kernel.cuh"
+#include "tail_kernel.cuh"
 #include "aux_kernels.cuh"
 #include "neglog_tables.inc"
 
@@ -361,17 +362,36 @@ extern "C" int necsim_simulate_workspace_size(const necsim_scenario *scn, uint64
 }
 
 template <int KIND>
-static cudaError_t launch_epoch(bool dedup, u32 grid, u32 block, cudaStream_t st, const ScenarioDev &sd, const SimBuffers &bf, const EpochArgs &ep) {
-    if (dedup) simulate_kernel<KIND, true><<<grid, block, 0, st>>>(sd, bf, ep);
-    else simulate_kernel<KIND, false><<<grid, block, 0, st>>>(sd, bf, ep);
+static cudaError_t launch_epoch(bool dedup, bool tail, u32 grid, u32 block, cudaStream_t st, const ScenarioDev &sd, const SimBuffers &bf,
+                                const EpochArgs &ep) {
+    if (tail) {
+        if (dedup) tail_kernel<KIND, true><<<grid, block, 0, st>>>(sd, bf, ep);
+        else tail_kernel<KIND, false><<<grid, block, 0, st>>>(sd, bf, ep);
+    } else {
+        if (dedup) simulate_kernel<KIND, true><<<grid, block, 0, st>>>(sd, bf, ep);
+        else simulate_kernel<KIND, false><<<grid, block, 0, st>>>(sd, bf, ep);
+    }
     return cudaGetLastError();
 }
 template <int KIND>
-static int occupancy_blocks(bool dedup, u32 block) {
+static int occupancy_blocks(bool dedup, bool tail, u32 block) {
     int nb = 0;
-    if (dedup) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, simulate_kernel<KIND, true>, (int)block, 0);
-    else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, simulate_kernel<KIND, false>, (int)block, 0);
+    if (tail) {
+        if (dedup) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, tail_kernel<KIND, true>, (int)block, 0);
+        else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, tail_kernel<KIND, false>, (int)block, 0);
+    } else {
+        if (dedup) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, simulate_kernel<KIND, true>, (int)block, 0);
+        else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, simulate_kernel<KIND, false>, (int)block, 0);
+    }
     return nb;
+}
+static int occupancy_for(int kind, bool dedup, bool tail, u32 block) {
+    switch (kind) {
+    case 0: return occupancy_blocks<0>(dedup, tail, block);
+    case 1: return occupancy_blocks<1>(dedup, tail, block);
+    case 2: return occupancy_blocks<2>(dedup, tail, block);
+    default: return occupancy_blocks<3>(dedup, tail, block);
+    }
 }
 
 static u64 thr53(double p) { return (u64)floor(ldexp(p, 53)); }
@@ -428,19 +448,18 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
     ep.thr_nu = thr53(nu);
     ep.thr_m = thr53(scn->migration);
     ep.max_steps = (u32)rp.max_steps;
-    int occ = 0;
-    switch (sd.kind) {
-    case 0: occ = occupancy_blocks<0>(rp.dedup, rp.block_threads); break;
-    case 1: occ = occupancy_blocks<1>(rp.dedup, rp.block_threads); break;
-    case 2: occ = occupancy_blocks<2>(rp.dedup, rp.block_threads); break;
-    default: occ = occupancy_blocks<3>(rp.dedup, rp.block_threads); break;
-    }
-    if (occ <= 0) return fail(NECSIM_ERR_CUDA, "simulate kernel cannot be resident (occupancy 0)");
+    const int occ = occupancy_for(sd.kind, rp.dedup, false, rp.block_threads);
+    const int occ_tail = occupancy_for(sd.kind, rp.dedup, true, rp.block_threads);
+    if (occ <= 0 || occ_tail <= 0) return fail(NECSIM_ERR_CUDA, "simulate kernel cannot be resident (occupancy 0)");
     const u32 full_grid = rp.grid_blocks ? rp.grid_blocks : (u32)(occ * scn->sm_count);
+    const u32 tail_grid = rp.grid_blocks ? rp.grid_blocks : (u32)(occ_tail * scn->sm_count);
+    const u32 warps_per_block = rp.block_threads / 32u;
+    // one lineage per warp pays off once every active lineage can have a resident warp of its own
+    const u32 tail_threshold = rp.tail_threshold ? rp.tail_threshold : tail_grid * warps_per_block;
     u32 active = n_sampled, k_start = 0;
     uint4 *q_in = qa, *q_out = qb;
-    float ms_sim = 0.f;
-    u64 n_epochs = 0;
+    float ms_sim = 0.f, ms_tail = 0.f;
+    u64 n_epochs = 0, n_tail_epochs = 0, ev_before = 0, ev_tail = 0;
     while (active > 0) {
         u32 k_stop;
         if (rp.epoch_events == 0) k_stop = 0xFFFFFFFFu;
@@ -451,21 +470,28 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
             k_stop = h >= 0xFFFFFFFFull ? 0xFFFFFFFFu : (u32)h;
         }
         ep.k_start = k_start; ep.k_stop = k_stop;
-        const u64 total_warps = (u64)full_grid * (rp.block_threads / 32u);
-        u32 lanes = 32;
-        if ((u64)active < total_warps * 32ull) lanes = (u32)std::max<u64>(1, ((u64)active + total_warps - 1) / total_warps);
-        ep.lanes_per_warp = lanes;
-        u32 grid = full_grid;
-        if (lanes == 1) grid = (u32)std::min<u64>(full_grid, ((u64)active + rp.block_threads / 32u - 1) / (rp.block_threads / 32u));
+        const bool tail = active <= tail_threshold;
+        u32 grid;
+        if (tail) {
+            ep.lanes_per_warp = 32;
+            grid = (u32)std::min<u64>(tail_grid, ((u64)active + warps_per_block - 1) / warps_per_block);
+        } else {
+            const u64 total_warps = (u64)full_grid * warps_per_block;
+            u32 lanes = 32;
+            if ((u64)active < total_warps * 32ull) lanes = (u32)std::max<u64>(1, ((u64)active + total_warps - 1) / total_warps);
+            ep.lanes_per_warp = lanes;
+            grid = full_grid;
+            if (lanes == 1) grid = (u32)std::min<u64>(full_grid, ((u64)active + warps_per_block - 1) / warps_per_block);
+        }
         bf.q_in = q_in; bf.q_out = q_out; bf.q_in_count = active;
         CU(cudaMemsetAsync(bf.ctr, 0, 8, st));   // q_head, q_out
         CU(cudaEventRecord(scn->ev[2], st));
         cudaError_t ce;
         switch (sd.kind) {
-        case 0: ce = launch_epoch<0>(rp.dedup, grid, rp.block_threads, st, sd, bf, ep); break;
-        case 1: ce = launch_epoch<1>(rp.dedup, grid, rp.block_threads, st, sd, bf, ep); break;
-        case 2: ce = launch_epoch<2>(rp.dedup, grid, rp.block_threads, st, sd, bf, ep); break;
-        default: ce = launch_epoch<3>(rp.dedup, grid, rp.block_threads, st, sd, bf, ep); break;
+        case 0: ce = launch_epoch<0>(rp.dedup, tail, grid, rp.block_threads, st, sd, bf, ep); break;
+        case 1: ce = launch_epoch<1>(rp.dedup, tail, grid, rp.block_threads, st, sd, bf, ep); break;
+        case 2: ce = launch_epoch<2>(rp.dedup, tail, grid, rp.block_threads, st, sd, bf, ep); break;
+        default: ce = launch_epoch<3>(rp.dedup, tail, grid, rp.block_threads, st, sd, bf, ep); break;
         }
         if (ce != cudaSuccess) return fail(NECSIM_ERR_CUDA, std::string("simulate kernel launch: ") + cudaGetErrorString(ce));
         CU(cudaEventRecord(scn->ev[3], st));
@@ -475,6 +501,8 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
         CU(cudaEventElapsedTime(&ms, scn->ev[2], scn->ev[3]));
         ms_sim += ms;
         ++n_epochs; ++n_launch;
+        if (tail) { ms_tail += ms; ++n_tail_epochs; ev_tail += hc->n_events - ev_before; }
+        ev_before = hc->n_events;
         if (hc->error) return fail(NECSIM_ERR_CAPACITY, "interval index overflowed 2^32 or dispersal resampling exhausted");
         active = hc->q_out;
         std::swap(q_in, q_out);
@@ -528,7 +556,8 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
     out->d_term_loc = bf.term_loc; out->d_term_k = bf.term_k; out->d_term_j = bf.term_j; out->d_steps = bf.steps;
     out->d_term_f = bf.term_f; out->d_state = bf.state;
     out->n_events_raw = hc->n_events; out->n_culled = hc->n_culled; out->n_speciation_raw = n_spec; out->n_epochs = n_epochs;
-    out->resample_attempts = hc->resamples; out->ms_simulate = ms_sim; out->ms_total = ms_total; out->n_kernel_launches = n_launch;
+    out->resample_attempts = hc->resamples; out->ms_simulate = ms_sim; out->ms_simulate_tail = ms_tail; out->n_tail_epochs = n_tail_epochs; out->n_events_tail = ev_tail;
+    out->ms_total = ms_total; out->n_kernel_launches = n_launch;
     return NECSIM_OK;
 }
 
@@ -628,14 +657,16 @@ __global__ void debug_next_event_kernel(SeedKey key, const u32 *loc, const u32 *
 template <int KIND>
 __global__ void debug_disperse_kernel(const ScenarioDev sc, SeedKey key, u64 thr_m, const u32 *loc, const u32 *k, const u32 *j, u32 *loc_out, u64 n) {
     __shared__ u32 sG[KIND == 3 ? 1024 : 1];
-    if (KIND == 3) for (u32 i = threadIdx.x; i < sc.gauss_len; i += blockDim.x) sG[i] = sc.gauss[i];
+    __shared__ unsigned short sGuide[KIND == 3 ? 256 : 1];
+    if (KIND == 3) gauss_stage(sc, sG, sGuide);
     __syncthreads();
+    GaussLut gl; gl.tg = sG; gl.guide = sGuide; gl.R = sc.R;
     u64 i = (u64)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     u32 cell = (KIND == 1) ? (loc[i] >= sc.J_local ? 1u : 0u) : cell_of_loc(sc, loc[i]);
     u64 X = prime(key, loc[i], k[i]) + (u64)j[i] * NS_GAMMA;
     u32 l2 = 0xFFFFFFFFu, c2 = 0, rs = 0;
-    disperse<KIND>(sc, thr_m, X, cell, l2, c2, sG, rs);
+    disperse<KIND>(sc, thr_m, X, cell, l2, c2, gl, rs);
     loc_out[i] = l2;
 }
 

@@ -20,14 +20,28 @@ __device__ __forceinline__ u32 lanemask_lt() {
     return m;
 }
 
-// rounded-normal displacement: G(u) = -R + #{i : u >= TG[i]}  (R15). tg: padded table in smem.
-__device__ __forceinline__ int gauss_disp(const u32 *tg, u32 len, int R, u32 u) {
-    u32 pos = 0;
-    for (u32 s = len >> 1; s; s >>= 1)
-        if (tg[pos + s - 1] <= u) pos += s;
-    pos += (tg[pos] <= u) ? 1u : 0u;
-    int c = (int)min(pos, (u32)(2 * R));
-    return c - R;
+// rounded-normal displacement: G(u) = -R + #{i : u >= TG[i]}  (R15). tg: thresholds in smem (padded
+// with 0xFFFFFFFF); guide[b] = #{i : TG[i] < b<<24} gives the start of a short forward scan (TG is non-decreasing).
+struct GaussLut {
+    const u32 *tg;
+    const unsigned short *guide;
+    int R;
+};
+__device__ __forceinline__ int gauss_disp(const GaussLut &g, u32 u) {
+    u32 pos = g.guide[u >> 24];
+    const u32 n = 2u * (u32)g.R;
+    while (pos < n && g.tg[pos] <= u) ++pos;
+    return (int)pos - g.R;
+}
+// fills sG / sGuide from the scenario's table (call by all threads of the block, then __syncthreads)
+__device__ __forceinline__ void gauss_stage(const ScenarioDev &sc, u32 *sG, unsigned short *sGuide) {
+    for (u32 i = threadIdx.x; i < sc.gauss_len; i += blockDim.x) sG[i] = sc.gauss[i];
+    __syncthreads();
+    for (u32 b = threadIdx.x; b < 256u; b += blockDim.x) {
+        u32 lim = b << 24, c = 0, n = 2u * (u32)sc.R;
+        while (c < n && sG[c] < lim) ++c;
+        sGuide[b] = (unsigned short)c;
+    }
 }
 
 __device__ __forceinline__ u32 cell_deme(const ScenarioDev &sc, u32 cell) {
@@ -44,7 +58,7 @@ __device__ __forceinline__ u32 cell_prefix(const ScenarioDev &sc, u32 cell) {
 // resampling exhaustion. `resamples` counts rejected targets.
 template <int KIND>
 __device__ __forceinline__ bool disperse(const ScenarioDev &sc, u64 thr_m, u64 X, u32 cell, u32 &loc2, u32 &cell2,
-                                         const u32 *tg, u32 &resamples) {
+                                         const GaussLut &gl, u32 &resamples) {
     if (KIND == 0) {  // NONSPATIAL: uniform over all J positions, self allowed (R12)
         loc2 = mulhi64_u32(draw_disp(X, 0), (u32)sc.n_locations);
         cell2 = 0;
@@ -72,8 +86,8 @@ __device__ __forceinline__ bool disperse(const ScenarioDev &sc, u64 thr_m, u64 X
         else { y0 = cell / sc.width; x0 = cell - y0 * sc.width; }
         for (u32 r = 0; r < NS_MAX_RESAMPLE; ++r) {
             u64 x = draw_disp(X, r);
-            int dx = gauss_disp(tg, sc.gauss_len, sc.R, (u32)(x >> 32));
-            int dy = gauss_disp(tg, sc.gauss_len, sc.R, (u32)x);
+            int dx = gauss_disp(gl, (u32)(x >> 32));
+            int dy = gauss_disp(gl, (u32)x);
             int xx = (int)x0 + dx, yy = (int)y0 + dy;      // |d| <= R < min(width, height): one wrap suffices
             if (xx < 0) xx += (int)sc.width; else if (xx >= (int)sc.width) xx -= (int)sc.width;
             if (yy < 0) yy += (int)sc.height; else if (yy >= (int)sc.height) yy -= (int)sc.height;
@@ -110,9 +124,11 @@ __global__ void __launch_bounds__(256) simulate_kernel(const ScenarioDev sc, con
     __shared__ unsigned short sQ[512];
     __shared__ u64 sA[512];
     __shared__ u32 sG[KIND == 3 ? 1024 : 1];
+    __shared__ unsigned short sGuide[KIND == 3 ? 256 : 1];
     for (u32 i = threadIdx.x; i < 512; i += blockDim.x) { sQ[i] = NEGLOG_Q_DEV[i]; sA[i] = NEGLOG_A_DEV[i]; }
-    if (KIND == 3) for (u32 i = threadIdx.x; i < sc.gauss_len; i += blockDim.x) sG[i] = sc.gauss[i];
+    if (KIND == 3) gauss_stage(sc, sG, sGuide);
     __syncthreads();
+    GaussLut gl; gl.tg = sG; gl.guide = sGuide; gl.R = sc.R;
 
     const u32 lane = threadIdx.x & 31u;
     const bool lane_on = lane < ep.lanes_per_warp;
@@ -179,21 +195,26 @@ __global__ void __launch_bounds__(256) simulate_kernel(const ScenarioDev sc, con
         if ((i64)T <= f_last) continue;            // not strictly later than the last event (L729)
 
         // ---- event (loc, k, j) at offset T ----------------------------------------------------------
-        if (DEDUP) {   // S5: duplicate-culling cache keyed on the full event identity
-            uint4 mine = make_uint4(loc, k, j, id);
-            uint4 old = atomic_exch_128(&bf.cache[cache_slot(loc, k, j, bf.cache_mask)], mine);
-            if (old.x == loc && old.y == k && old.z == j && old.w != id) {
-                // another lineage executed this event: identical future (L687, L697) -> cull, link to it
-                bf.parent[id] = old.w; bf.state[id] = 2;
-                bf.term_loc[id] = loc; bf.term_k[id] = k; bf.term_j[id] = j; bf.term_f[id] = T; bf.steps[id] = steps;
-                c_culled++; has = false;
-                continue;
-            }
+        // S5: duplicate-culling cache keyed on the full event identity. The 128-bit exchange is issued first and
+        // its result consumed after the (side-effect free) speciation and dispersal draws, hiding the L2 round trip.
+        uint4 old = make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu);
+        if (DEDUP) old = atomic_exch_128(&bf.cache[cache_slot(loc, k, j, bf.cache_mask)], make_uint4(loc, k, j, id));
+        // S2: speciation test on the event's SPEC lane
+        const bool can_speciate = !(KIND == 1 && cell == 0);     // local community of the implicit model: nu = 0 (L1830)
+        const bool speciates = can_speciate && bern(draw_spec(X), ep.thr_nu);
+        // S3: dispersal to the parent's location
+        u32 loc2 = loc, cell2 = cell;
+        bool ok = true;
+        if (!speciates) ok = disperse<KIND>(sc, ep.thr_m, X, cell, loc2, cell2, gl, c_resamples);
+        if (DEDUP && old.x == loc && old.y == k && old.z == j && old.w != id) {
+            // another lineage executed this event: identical future (L687, L697) -> cull, link to it
+            bf.parent[id] = old.w; bf.state[id] = 2;
+            bf.term_loc[id] = loc; bf.term_k[id] = k; bf.term_j[id] = j; bf.term_f[id] = T; bf.steps[id] = steps;
+            c_culled++; has = false;
+            continue;
         }
         f_last = (i64)T; steps++; c_events++;
-        // S2: speciation test on the event's SPEC lane
-        bool can_speciate = !(KIND == 1 && cell == 0);     // local community of the implicit model: nu = 0 (L1830)
-        if (can_speciate && bern(draw_spec(X), ep.thr_nu)) {
+        if (speciates) {
             bf.state[id] = 1;
             bf.term_loc[id] = loc; bf.term_k[id] = k; bf.term_j[id] = j; bf.term_f[id] = T; bf.steps[id] = steps;
             bf.spec_ring[atomicAdd(&bf.ctr->n_spec, 1u)] = id;
@@ -201,11 +222,7 @@ __global__ void __launch_bounds__(256) simulate_kernel(const ScenarioDev sc, con
             has = false;
             continue;
         }
-        // S3: dispersal to the parent's location
-        u32 loc2, cell2;
-        if (!disperse<KIND>(sc, ep.thr_m, X, cell, loc2, cell2, sG, c_resamples)) {
-            atomicMax(&bf.ctr->error, 3u); has = false; continue;
-        }
+        if (!ok) { atomicMax(&bf.ctr->error, 3u); has = false; continue; }
         loc = loc2; cell = cell2; need_prime = true;
         if (ep.max_steps && steps >= ep.max_steps) {
             bf.state[id] = 3;

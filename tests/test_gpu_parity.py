@@ -35,14 +35,19 @@ def assert_same_result(got, ref, name=""):
     assert np.array_equal(got["labels"], ref["labels"]), name
 
 
+KERNELS = {"per_thread": 1, "tail": 0xFFFFFFFF}      # tail_threshold: which simulate kernel runs every epoch
+
+
+@pytest.mark.parametrize("kernel", sorted(KERNELS))
 @pytest.mark.parametrize("idx", range(5))
-def test_small_configs_dedup_on(ns, O, I, idx):
+def test_small_configs_dedup_on(ns, O, I, idx, kernel):
     cfg = I.small_configs()[idx]
     kw = I.scenario_kwargs(cfg)
     ref = O.Scenario(**kw).simulate(cfg["seed"], cfg["nu"], cfg["mask"], dedup=True)
     sc = ns.Scenario(**kw)
-    got = sc.simulate(cfg["seed"], cfg["nu"], cfg["mask"])
+    got = sc.simulate(cfg["seed"], cfg["nu"], cfg["mask"], tail_threshold=KERNELS[kernel])
     assert_same_result(got, ref, cfg["name"])
+    assert (got["stats"]["n_tail_epochs"] == got["stats"]["n_epochs"]) == (kernel == "tail")
     golden = json.load(open(os.path.join(HERE, "golden", "small_configs.json")))[idx]     # written by the oracle only
     assert golden["name"] == cfg["name"] and golden["richness"] == got["richness"]
     assert golden["labels_head"] == [int(v) for v in got["labels"][:16]]
@@ -51,14 +56,15 @@ def test_small_configs_dedup_on(ns, O, I, idx):
     sc.close()
 
 
+@pytest.mark.parametrize("kernel", sorted(KERNELS))
 @pytest.mark.parametrize("idx", range(5))
-def test_small_configs_dedup_off_per_lineage(ns, O, I, idx):
+def test_small_configs_dedup_off_per_lineage(ns, O, I, idx, kernel):
     cfg = I.small_configs()[idx]
     kw = I.scenario_kwargs(cfg)
     nu = max(cfg["nu"], 5e-3)                      # no dedup: n/nu events
     ref = O.Scenario(**kw).simulate(cfg["seed"], nu, cfg["mask"], dedup=False, per_lineage=True)
     sc = ns.Scenario(**kw)
-    got = sc.simulate(cfg["seed"], nu, cfg["mask"], per_lineage=True, dedup=False)
+    got = sc.simulate(cfg["seed"], nu, cfg["mask"], per_lineage=True, dedup=False, tail_threshold=KERNELS[kernel])
     assert_same_result(got, ref, cfg["name"])
     for f in ("loc", "k", "j", "f"):
         assert np.array_equal(got["per_lineage"][f], ref["per_lineage"][f]), (cfg["name"], f)
@@ -68,14 +74,15 @@ def test_small_configs_dedup_off_per_lineage(ns, O, I, idx):
     sc.close()
 
 
+@pytest.mark.parametrize("kernel", sorted(KERNELS))
 @pytest.mark.parametrize("idx", [0, 3])
-def test_step_cap_mode(ns, O, I, idx):
+def test_step_cap_mode(ns, O, I, idx, kernel):
     """MODE-T workload: dedup off, every lineage advanced at most max_steps events."""
     cfg = I.small_configs()[idx]
     kw = I.scenario_kwargs(cfg)
     ref = O.Scenario(**kw).simulate(cfg["seed"], 1e-3, cfg["mask"], dedup=False, max_steps=100, per_lineage=True)
     sc = ns.Scenario(**kw)
-    got = sc.simulate(cfg["seed"], 1e-3, cfg["mask"], per_lineage=True, dedup=False, max_steps=100)
+    got = sc.simulate(cfg["seed"], 1e-3, cfg["mask"], per_lineage=True, dedup=False, max_steps=100, tail_threshold=KERNELS[kernel])
     assert_same_result(got, ref, cfg["name"])
     assert got["stats"]["n_unfinished"] == ref["stats"]["n_unfinished"] > 0
     for f in ("loc", "k", "j", "f"):
