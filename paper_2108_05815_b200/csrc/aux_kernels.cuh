@@ -3,7 +3,7 @@
 // adjacent after sorting), L276 / L890-900 (species = distinct speciation events).
 #pragma once
 #include "../../include/necsim.h"
-#include "sim_types.cuh"
+#include "sim_kernel.cuh"
 
 namespace necsim {
 
@@ -16,6 +16,11 @@ __device__ __forceinline__ u32 cell_of_loc(const ScenarioDev &sc, u32 loc) {
     u32 lo = 0, hi = sc.ncells;                      // invariant: prefix[lo] <= loc < prefix[hi]
     while (hi - lo > 1) { u32 mid = lo + ((hi - lo) >> 1); if (sc.prefix[mid] <= loc) lo = mid; else hi = mid; }
     return lo;
+}
+// the `cell` word of a queue entry: the cell index, or packed (y << 16 | x) for EXPLICIT_GAUSSIAN
+__device__ __forceinline__ u32 queue_cell(const ScenarioDev &sc, u32 loc) {
+    const u32 c = cell_of_loc(sc, loc);
+    return sc.kind == 3 ? pack_xy(sc, c) : c;
 }
 
 // S0, pass 1: number of sampled individuals per chunk
@@ -75,7 +80,7 @@ __global__ void __launch_bounds__(256) mask_scatter_kernel(const ScenarioDev sc,
     while (bits) {
         u32 t = __ffs(bits) - 1; bits &= bits - 1;
         u32 loc = (u32)(base + t);
-        if (off < capacity) queue[off] = make_uint4(off, loc, cell_of_loc(sc, loc), 0u);
+        if (off < capacity) queue[off] = make_uint4(off, loc, queue_cell(sc, loc), 0u);
         ++off;
     }
 }
@@ -83,7 +88,7 @@ __global__ void __launch_bounds__(256) mask_scatter_kernel(const ScenarioDev sc,
 // S0 without a mask: everyone is sampled
 __global__ void __launch_bounds__(256) all_sampled_kernel(const ScenarioDev sc, u32 n, uint4 *__restrict__ queue) {
     u32 i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) queue[i] = make_uint4(i, i, cell_of_loc(sc, i), 0u);
+    if (i < n) queue[i] = make_uint4(i, i, queue_cell(sc, i), 0u);
 }
 
 // ---- S6 ------------------------------------------------------------------------------------------

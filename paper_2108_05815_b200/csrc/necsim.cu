@@ -131,14 +131,12 @@ static int scenario_layout(const necsim_scenario_desc *d, ScenarioLayout &L) {
     L.per_cell_turnover = (d->turnover != NULL) && d->kind != NECSIM_NONSPATIAL;
     if (!L.uniform_deme) {
         for (u32 c = 0; c < L.ncells; ++c) if (d->deme[c] >= 255u) { L.need_deme32 = true; break; }
-    }
+    } else if (d->kind >= NECSIM_EXPLICIT_MATRIX && d->uniform_deme >= 255u) L.need_deme32 = true;
     size_t off = 0;
-    if (d->kind >= NECSIM_EXPLICIT_MATRIX && !L.uniform_deme) {
+    if (d->kind >= NECSIM_EXPLICIT_MATRIX) {   // explicit kinds always carry the per-cell tables
         L.off_hab8 = off; off = align256(off + L.ncells);
         if (L.need_deme32) { L.off_deme32 = off; off = align256(off + 4 * (size_t)L.ncells); }
         L.off_prefix = off; off = align256(off + 4 * ((size_t)L.ncells + 1));
-    } else if (!L.uniform_deme) {
-        return fail(NECSIM_ERR_INVALID_ARG, "internal: deme array with a non-explicit kind");
     }
     if (L.per_cell_turnover) { L.off_scale = off; off = align256(off + 8 * (size_t)L.ncells); }
     if (d->kind == NECSIM_EXPLICIT_MATRIX) {
@@ -147,6 +145,7 @@ static int scenario_layout(const necsim_scenario_desc *d, ScenarioLayout &L) {
     }
     if (d->kind == NECSIM_EXPLICIT_GAUSSIAN) {
         if (!(d->sigma > 0.0) || !std::isfinite(d->sigma)) return fail(NECSIM_ERR_INVALID_ARG, "bad sigma");
+        if (d->width > 65536u || d->height > 65536u) return fail(NECSIM_ERR_UNSUPPORTED, "gaussian dispersal: width and height must be <= 65536");
         L.R = (int)ceil(10.0 * d->sigma);
         if ((u32)L.R >= d->width || (u32)L.R >= d->height) return fail(NECSIM_ERR_INVALID_ARG, "10*sigma must be < min(width,height)");
         u32 len = 2; while (len < 2u * (u32)L.R) len <<= 1;
@@ -204,14 +203,21 @@ extern "C" int necsim_create_scenario(const necsim_scenario_desc *d, void *d_wor
         if ((d->width & (d->width - 1)) == 0) { u32 s = 0; while ((1u << s) < d->width) ++s; sd.width_shift = s; }
         // deme, prefix
         u64 tot = 0;
-        std::vector<uint8_t> hab8; std::vector<u32> prefix;
+        std::vector<uint8_t> hab8; std::vector<u32> prefix, deme_full;
+        const bool tables = d->kind >= NECSIM_EXPLICIT_MATRIX;
         if (L.uniform_deme) {
             u32 ud = d->kind == NECSIM_NONSPATIAL ? (d->deme ? d->deme[0] : d->uniform_deme) : d->uniform_deme;
             sd.uniform_deme = ud; tot = (u64)ud * n;
+            if (tables) {
+                hab8.assign(n, (uint8_t)std::min(ud, 255u)); prefix.resize((size_t)n + 1);
+                for (u32 c = 0; c <= n; ++c) prefix[c] = (u32)std::min<u64>((u64)ud * c, 0xFFFFFFFFull);
+                if (L.need_deme32) deme_full.assign(n, ud);
+            }
         } else {
             hab8.resize(n); prefix.resize((size_t)n + 1);
             for (u32 c = 0; c < n; ++c) { prefix[c] = (u32)tot; tot += d->deme[c]; hab8[c] = (uint8_t)std::min(d->deme[c], 255u); }
             prefix[n] = (u32)tot;
+            if (L.need_deme32) deme_full.assign(d->deme, d->deme + n);
         }
         if (tot == 0 || tot >= (1ull << 32)) return fail(NECSIM_ERR_INVALID_ARG, "number of indexed locations must be in [1, 2^32)");
         sd.n_locations = tot; sd.n_sampleable = tot;
@@ -231,11 +237,11 @@ extern "C" int necsim_create_scenario(const necsim_scenario_desc *d, void *d_wor
             if (!turnover_scale(d->uniform_turnover, d->delta_t, sd.Cm_u, sd.sh_u)) return fail(NECSIM_ERR_INVALID_ARG, "turnover*delta_t out of range");
             mu_max = d->uniform_turnover * d->delta_t;
         }
-        if (!L.uniform_deme) {
+        if (tables) {
             CU(cudaMemcpyAsync(base + L.off_hab8, hab8.data(), n, cudaMemcpyHostToDevice, st));
             sd.hab8 = base + L.off_hab8;
             if (L.need_deme32) {
-                CU(cudaMemcpyAsync(base + L.off_deme32, d->deme, 4 * (size_t)n, cudaMemcpyHostToDevice, st));
+                CU(cudaMemcpyAsync(base + L.off_deme32, deme_full.data(), 4 * (size_t)n, cudaMemcpyHostToDevice, st));
                 sd.deme32 = (const u32 *)(base + L.off_deme32);
             }
             CU(cudaMemcpyAsync(base + L.off_prefix, prefix.data(), 4 * ((size_t)n + 1), cudaMemcpyHostToDevice, st));
@@ -301,7 +307,7 @@ extern "C" int necsim_destroy(necsim_scenario *scn) {
 // simulate
 // ---------------------------------------------------------------------------------------------------
 struct ResolvedParams {
-    u32 block_threads, grid_blocks, dedup_log2_slots, tail_threshold;
+    u32 block_threads, grid_blocks, dedup_log2_slots, tail_threshold, probe_mask;
     bool dedup;
     u64 epoch_events, max_steps;
 };
@@ -321,6 +327,8 @@ static int resolve_params(const necsim_scenario *scn, const necsim_sim_params *p
     r.max_steps = p->max_steps;
     if (r.max_steps > 0xFFFFFFFFull) return fail(NECSIM_ERR_INVALID_ARG, "max_steps must fit 32 bits");
     r.tail_threshold = p->tail_threshold;
+    if (p->dedup_probe > 4) return fail(NECSIM_ERR_INVALID_ARG, "dedup_probe must be in [0, 4]");
+    r.probe_mask = p->dedup_probe ? ((1u << (p->dedup_probe - 1u)) - 1u) : 3u;   // default: every 4th event probes
     (void)scn;
     return NECSIM_OK;
 }
@@ -361,37 +369,25 @@ extern "C" int necsim_simulate_workspace_size(const necsim_scenario *scn, uint64
     return NECSIM_OK;
 }
 
-template <int KIND>
-static cudaError_t launch_epoch(bool dedup, bool tail, u32 grid, u32 block, cudaStream_t st, const ScenarioDev &sd, const SimBuffers &bf,
-                                const EpochArgs &ep) {
-    if (tail) {
-        if (dedup) tail_kernel<KIND, true><<<grid, block, 0, st>>>(sd, bf, ep);
-        else tail_kernel<KIND, false><<<grid, block, 0, st>>>(sd, bf, ep);
-    } else {
-        if (dedup) simulate_kernel<KIND, true><<<grid, block, 0, st>>>(sd, bf, ep);
-        else simulate_kernel<KIND, false><<<grid, block, 0, st>>>(sd, bf, ep);
-    }
-    return cudaGetLastError();
+typedef void (*EpochKernel)(const ScenarioDev, const SimBuffers, const EpochArgs);
+template <int KIND, bool PERCELL>
+static EpochKernel pick_kernel2(bool dedup, bool tail) {
+    if (tail) return dedup ? (EpochKernel)tail_kernel<KIND, true, PERCELL> : (EpochKernel)tail_kernel<KIND, false, PERCELL>;
+    return dedup ? (EpochKernel)simulate_kernel<KIND, true, PERCELL> : (EpochKernel)simulate_kernel<KIND, false, PERCELL>;
 }
-template <int KIND>
-static int occupancy_blocks(bool dedup, bool tail, u32 block) {
-    int nb = 0;
-    if (tail) {
-        if (dedup) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, tail_kernel<KIND, true>, (int)block, 0);
-        else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, tail_kernel<KIND, false>, (int)block, 0);
-    } else {
-        if (dedup) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, simulate_kernel<KIND, true>, (int)block, 0);
-        else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, simulate_kernel<KIND, false>, (int)block, 0);
-    }
-    return nb;
-}
-static int occupancy_for(int kind, bool dedup, bool tail, u32 block) {
+// per-cell turnover exists for the explicit kinds only
+static EpochKernel pick_kernel(int kind, bool percell, bool dedup, bool tail) {
     switch (kind) {
-    case 0: return occupancy_blocks<0>(dedup, tail, block);
-    case 1: return occupancy_blocks<1>(dedup, tail, block);
-    case 2: return occupancy_blocks<2>(dedup, tail, block);
-    default: return occupancy_blocks<3>(dedup, tail, block);
+    case 0: return pick_kernel2<0, false>(dedup, tail);
+    case 1: return pick_kernel2<1, false>(dedup, tail);
+    case 2: return percell ? pick_kernel2<2, true>(dedup, tail) : pick_kernel2<2, false>(dedup, tail);
+    default: return percell ? pick_kernel2<3, true>(dedup, tail) : pick_kernel2<3, false>(dedup, tail);
     }
+}
+static int occupancy_for(EpochKernel fn, u32 block) {
+    int nb = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, fn, (int)block, 0) != cudaSuccess) return 0;
+    return nb;
 }
 
 static u64 thr53(double p) { return (u64)floor(ldexp(p, 53)); }
@@ -448,8 +444,11 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
     ep.thr_nu = thr53(nu);
     ep.thr_m = thr53(scn->migration);
     ep.max_steps = (u32)rp.max_steps;
-    const int occ = occupancy_for(sd.kind, rp.dedup, false, rp.block_threads);
-    const int occ_tail = occupancy_for(sd.kind, rp.dedup, true, rp.block_threads);
+    const EpochKernel fn_main = pick_kernel(sd.kind, sd.per_cell_turnover != 0, rp.dedup, false);
+    const EpochKernel fn_tail = pick_kernel(sd.kind, sd.per_cell_turnover != 0, rp.dedup, true);
+    const int occ = occupancy_for(fn_main, rp.block_threads);
+    const int occ_tail = occupancy_for(fn_tail, rp.block_threads);
+    ep.probe_mask = rp.probe_mask;
     if (occ <= 0 || occ_tail <= 0) return fail(NECSIM_ERR_CUDA, "simulate kernel cannot be resident (occupancy 0)");
     const u32 full_grid = rp.grid_blocks ? rp.grid_blocks : (u32)(occ * scn->sm_count);
     const u32 tail_grid = rp.grid_blocks ? rp.grid_blocks : (u32)(occ_tail * scn->sm_count);
@@ -486,13 +485,8 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
         bf.q_in = q_in; bf.q_out = q_out; bf.q_in_count = active;
         CU(cudaMemsetAsync(bf.ctr, 0, 8, st));   // q_head, q_out
         CU(cudaEventRecord(scn->ev[2], st));
-        cudaError_t ce;
-        switch (sd.kind) {
-        case 0: ce = launch_epoch<0>(rp.dedup, tail, grid, rp.block_threads, st, sd, bf, ep); break;
-        case 1: ce = launch_epoch<1>(rp.dedup, tail, grid, rp.block_threads, st, sd, bf, ep); break;
-        case 2: ce = launch_epoch<2>(rp.dedup, tail, grid, rp.block_threads, st, sd, bf, ep); break;
-        default: ce = launch_epoch<3>(rp.dedup, tail, grid, rp.block_threads, st, sd, bf, ep); break;
-        }
+        (tail ? fn_tail : fn_main)<<<grid, rp.block_threads, 0, st>>>(sd, bf, ep);
+        cudaError_t ce = cudaGetLastError();
         if (ce != cudaSuccess) return fail(NECSIM_ERR_CUDA, std::string("simulate kernel launch: ") + cudaGetErrorString(ce));
         CU(cudaEventRecord(scn->ev[3], st));
         CU(cudaMemcpyAsync(hc, bf.ctr, sizeof(SimCounters), cudaMemcpyDeviceToHost, st));
@@ -657,13 +651,14 @@ __global__ void debug_next_event_kernel(SeedKey key, const u32 *loc, const u32 *
 template <int KIND>
 __global__ void debug_disperse_kernel(const ScenarioDev sc, SeedKey key, u64 thr_m, const u32 *loc, const u32 *k, const u32 *j, u32 *loc_out, u64 n) {
     __shared__ u32 sG[KIND == 3 ? 1024 : 1];
-    __shared__ unsigned short sGuide[KIND == 3 ? 256 : 1];
-    if (KIND == 3) gauss_stage(sc, sG, sGuide);
+    __shared__ uint2 sG2[KIND == 3 ? NS_G2_LEN : 1];
+    if (KIND == 3) gauss_stage(sc, sG, sG2);
     __syncthreads();
-    GaussLut gl; gl.tg = sG; gl.guide = sGuide; gl.R = sc.R;
+    GaussLut gl; gl.tg = sG; gl.g2 = sG2; gl.R = sc.R;
     u64 i = (u64)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     u32 cell = (KIND == 1) ? (loc[i] >= sc.J_local ? 1u : 0u) : cell_of_loc(sc, loc[i]);
+    if (KIND == 3) cell = pack_xy(sc, cell);
     u64 X = prime(key, loc[i], k[i]) + (u64)j[i] * NS_GAMMA;
     u32 l2 = 0xFFFFFFFFu, c2 = 0, rs = 0;
     disperse<KIND>(sc, thr_m, X, cell, l2, c2, gl, rs);

@@ -20,42 +20,81 @@ __device__ __forceinline__ u32 lanemask_lt() {
     return m;
 }
 
-// rounded-normal displacement: G(u) = -R + #{i : u >= TG[i]}  (R15). tg: thresholds in smem (padded
-// with 0xFFFFFFFF); guide[b] = #{i : TG[i] < b<<24} gives the start of a short forward scan (TG is non-decreasing).
+// rounded-normal displacement: G(u) = -R + #{i : u >= TG[i]}  (R15). TG is non-decreasing.
+// tg: the 2R thresholds in smem. g2: 2048-entry guide indexed by the top 11 bits of u:
+//   g2[b].x = pos0 | multi << 16,  pos0 = #{i : TG[i] < b << 21},  g2[b].y = TG[pos0]
+//   multi = 1 when bucket b holds two or more thresholds or pos0 == 2R (then the exact forward scan runs).
+#define NS_G2_BITS 11
+#define NS_G2_LEN (1u << NS_G2_BITS)
 struct GaussLut {
     const u32 *tg;
-    const unsigned short *guide;
+    const uint2 *g2;
     int R;
 };
+// exact for every u; `fast` = false when the rare forward scan was needed
 __device__ __forceinline__ int gauss_disp(const GaussLut &g, u32 u) {
-    u32 pos = g.guide[u >> 24];
-    const u32 n = 2u * (u32)g.R;
-    while (pos < n && g.tg[pos] <= u) ++pos;
+    const uint2 e = g.g2[u >> (32 - NS_G2_BITS)];
+    u32 pos = e.x & 0xFFFFu;
+    if (e.x >> 16) {
+        const u32 n = 2u * (u32)g.R;
+        while (pos < n && g.tg[pos] <= u) ++pos;
+    } else {
+        pos += (e.y <= u) ? 1u : 0u;
+    }
     return (int)pos - g.R;
 }
-// fills sG / sGuide from the scenario's table (call by all threads of the block, then __syncthreads)
-__device__ __forceinline__ void gauss_stage(const ScenarioDev &sc, u32 *sG, unsigned short *sGuide) {
+// branch-free variant for speculative candidates: `exact` = false where the forward scan would be needed
+__device__ __forceinline__ int gauss_disp_fast(const GaussLut &g, u32 u, bool &exact) {
+    const uint2 e = g.g2[u >> (32 - NS_G2_BITS)];
+    exact = (e.x >> 16) == 0u;
+    return (int)((e.x & 0xFFFFu) + ((e.y <= u) ? 1u : 0u)) - g.R;
+}
+// fills sG / sG2 from the scenario's table (call by all threads of the block; ends with __syncthreads)
+__device__ __forceinline__ void gauss_stage(const ScenarioDev &sc, u32 *sG, uint2 *sG2) {
     for (u32 i = threadIdx.x; i < sc.gauss_len; i += blockDim.x) sG[i] = sc.gauss[i];
     __syncthreads();
-    for (u32 b = threadIdx.x; b < 256u; b += blockDim.x) {
-        u32 lim = b << 24, c = 0, n = 2u * (u32)sc.R;
-        while (c < n && sG[c] < lim) ++c;
-        sGuide[b] = (unsigned short)c;
+    const u32 n = 2u * (u32)sc.R;
+    for (u32 b = threadIdx.x; b < NS_G2_LEN; b += blockDim.x) {
+        // pos0(b) by binary search: first index with TG[i] >= b << 21
+        const u32 lim = b << (32 - NS_G2_BITS);
+        u32 lo = 0, hi = n;
+        while (lo < hi) { u32 mid = (lo + hi) >> 1; if (sG[mid] < lim) lo = mid + 1; else hi = mid; }
+        u32 nxt = n;
+        if (b + 1 < NS_G2_LEN) {
+            const u32 lim2 = (b + 1) << (32 - NS_G2_BITS);
+            u32 l2 = lo, h2 = n;
+            while (l2 < h2) { u32 mid = (l2 + h2) >> 1; if (sG[mid] < lim2) l2 = mid + 1; else h2 = mid; }
+            nxt = l2;
+        }
+        const u32 multi = (nxt - lo >= 2u || lo == n) ? 1u : 0u;
+        sG2[b] = make_uint2(lo | (multi << 16), lo < n ? sG[lo] : 0xFFFFFFFFu);
     }
+    __syncthreads();
 }
 
+// explicit kinds always have the per-cell tables (hab8 = min(deme, 255), deme32 where needed, prefix)
 __device__ __forceinline__ u32 cell_deme(const ScenarioDev &sc, u32 cell) {
-    if (sc.uniform_deme) return sc.uniform_deme;
-    u32 d = sc.hab8[cell];
-    if (d == 255u) d = sc.deme32[cell];
+    u32 d = __ldg(&sc.hab8[cell]);
+    if (d == 255u) d = __ldg(&sc.deme32[cell]);
     return d;
 }
-__device__ __forceinline__ u32 cell_prefix(const ScenarioDev &sc, u32 cell) {
-    return sc.uniform_deme ? cell * sc.uniform_deme : sc.prefix[cell];
+__device__ __forceinline__ u32 cell_prefix(const ScenarioDev &sc, u32 cell) { return __ldg(&sc.prefix[cell]); }
+
+// EXPLICIT_GAUSSIAN lineages carry their cell as packed coordinates (y << 16 | x): no division on the hot path.
+__device__ __forceinline__ u32 pack_xy(const ScenarioDev &sc, u32 cell) {
+    u32 y = cell / sc.width;
+    return (y << 16) | (cell - y * sc.width);
+}
+__device__ __forceinline__ u32 xy_index(const ScenarioDev &sc, u32 xy) { return (xy >> 16) * sc.width + (xy & 0xFFFFu); }
+// torus step of one axis: |d| <= R < size, one wrap suffices (R17)
+__device__ __forceinline__ u32 wrap_add(u32 x, int d, u32 size) {
+    int v = (int)x + d;
+    if (v < 0) v += (int)size; else if (v >= (int)size) v -= (int)size;
+    return (u32)v;
 }
 
 // DESIGN.md 2.5 step 2: dispersal of the event at stream position X from (loc, cell). Returns false on
-// resampling exhaustion. `resamples` counts rejected targets.
+// resampling exhaustion. `resamples` counts rejected targets. KIND 3: cell / cell2 are packed (y << 16 | x).
 template <int KIND>
 __device__ __forceinline__ bool disperse(const ScenarioDev &sc, u64 thr_m, u64 X, u32 cell, u32 &loc2, u32 &cell2,
                                          const GaussLut &gl, u32 &resamples) {
@@ -81,21 +120,16 @@ __device__ __forceinline__ bool disperse(const ScenarioDev &sc, u64 thr_m, u64 X
         loc2 = cell_prefix(sc, c2) + idx;
         return true;
     } else {  // EXPLICIT_GAUSSIAN: rounded normal on a torus, resample until habitat (R15-R17)
-        u32 x0, y0;
-        if (sc.width_shift != 0xFFFFFFFFu) { x0 = cell & (sc.width - 1); y0 = cell >> sc.width_shift; }
-        else { y0 = cell / sc.width; x0 = cell - y0 * sc.width; }
+        const u32 x0 = cell & 0xFFFFu, y0 = cell >> 16;
         for (u32 r = 0; r < NS_MAX_RESAMPLE; ++r) {
-            u64 x = draw_disp(X, r);
-            int dx = gauss_disp(gl, (u32)(x >> 32));
-            int dy = gauss_disp(gl, (u32)x);
-            int xx = (int)x0 + dx, yy = (int)y0 + dy;      // |d| <= R < min(width, height): one wrap suffices
-            if (xx < 0) xx += (int)sc.width; else if (xx >= (int)sc.width) xx -= (int)sc.width;
-            if (yy < 0) yy += (int)sc.height; else if (yy >= (int)sc.height) yy -= (int)sc.height;
-            u32 c2 = (u32)yy * sc.width + (u32)xx;
-            u32 d = cell_deme(sc, c2);
+            const u64 x = draw_disp(X, r);
+            const u32 xx = wrap_add(x0, gauss_disp(gl, (u32)(x >> 32)), sc.width);
+            const u32 yy = wrap_add(y0, gauss_disp(gl, (u32)x), sc.height);
+            const u32 c2 = yy * sc.width + xx;
+            const u32 d = cell_deme(sc, c2);
             if (d > 0) {
-                u32 idx = (d == 1u) ? 0u : mulhi64_u32(draw_index(X), d);
-                cell2 = c2;
+                const u32 idx = (d == 1u) ? 0u : mulhi64_u32(draw_index(X), d);
+                cell2 = (yy << 16) | xx;
                 loc2 = cell_prefix(sc, c2) + idx;
                 return true;
             }
@@ -105,30 +139,32 @@ __device__ __forceinline__ bool disperse(const ScenarioDev &sc, u64 thr_m, u64 X
     }
 }
 
-__device__ __forceinline__ u32 cache_slot(u32 loc, u32 k, u32 j, u32 mask) {
-    // slot hash only chooses a bucket; a hit always compares the full key
+__device__ __forceinline__ u32 cache_hash(u32 loc, u32 k, u32 j) {
+    // the hash only chooses a bucket (low bits) and whether the event probes at all (top 3 bits);
+    // a hit always compares the full key
     u32 h = loc * 0x9E3779B1u;
     h ^= (k + j * 0x7FEB352Du) * 0x85EBCA6Bu;
     h ^= h >> 15;
     h *= 0x2C1B3C6Du;
     h ^= h >> 13;
-    return h & mask;
+    return h;
 }
+__device__ __forceinline__ bool cache_probes(u32 h, u32 probe_mask) { return ((h >> 29) & probe_mask) == 0u; }
 
 // -ln tables in global memory (filled once per process from neglog_tables.inc), staged to smem per block
 __device__ unsigned short NEGLOG_Q_DEV[512];
 __device__ u64 NEGLOG_A_DEV[512];
 
-template <int KIND, bool DEDUP>
+template <int KIND, bool DEDUP, bool PERCELL>
 __global__ void __launch_bounds__(256) simulate_kernel(const ScenarioDev sc, const SimBuffers bf, const EpochArgs ep) {
     __shared__ unsigned short sQ[512];
     __shared__ u64 sA[512];
     __shared__ u32 sG[KIND == 3 ? 1024 : 1];
-    __shared__ unsigned short sGuide[KIND == 3 ? 256 : 1];
+    __shared__ uint2 sG2[KIND == 3 ? NS_G2_LEN : 1];
     for (u32 i = threadIdx.x; i < 512; i += blockDim.x) { sQ[i] = NEGLOG_Q_DEV[i]; sA[i] = NEGLOG_A_DEV[i]; }
-    if (KIND == 3) gauss_stage(sc, sG, sGuide);
+    if (KIND == 3) gauss_stage(sc, sG, sG2);
     __syncthreads();
-    GaussLut gl; gl.tg = sG; gl.guide = sGuide; gl.R = sc.R;
+    GaussLut gl; gl.tg = sG; gl.g2 = sG2; gl.R = sc.R;
 
     const u32 lane = threadIdx.x & 31u;
     const bool lane_on = lane < ep.lanes_per_warp;
@@ -167,7 +203,7 @@ __global__ void __launch_bounds__(256) simulate_kernel(const ScenarioDev sc, con
             } else {
                 X = prime(ep.key, loc, k);
                 T = 0; j = 0; need_prime = false;
-                if (sc.per_cell_turnover) { uint2 cs = __ldg(&sc.scale[cell]); Cm = cs.x; sh = cs.y; }
+                if (PERCELL) { uint2 cs = __ldg(&sc.scale[KIND == 3 ? xy_index(sc, cell) : cell]); Cm = cs.x; sh = cs.y; }
             }
         }
         {   // survivors of this epoch go to the output queue (warp-aggregated append)
@@ -198,7 +234,10 @@ __global__ void __launch_bounds__(256) simulate_kernel(const ScenarioDev sc, con
         // S5: duplicate-culling cache keyed on the full event identity. The 128-bit exchange is issued first and
         // its result consumed after the (side-effect free) speciation and dispersal draws, hiding the L2 round trip.
         uint4 old = make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu);
-        if (DEDUP) old = atomic_exch_128(&bf.cache[cache_slot(loc, k, j, bf.cache_mask)], make_uint4(loc, k, j, id));
+        if (DEDUP) {
+            const u32 h = cache_hash(loc, k, j);
+            if (cache_probes(h, ep.probe_mask)) old = atomic_exch_128(&bf.cache[h & bf.cache_mask], make_uint4(loc, k, j, id));
+        }
         // S2: speciation test on the event's SPEC lane
         const bool can_speciate = !(KIND == 1 && cell == 0);     // local community of the implicit model: nu = 0 (L1830)
         const bool speciates = can_speciate && bern(draw_spec(X), ep.thr_nu);

@@ -10,7 +10,7 @@ struct ScenarioDev {
     int kind;
     u32 width, height, ncells;
     u32 width_shift;           // log2(width) if width is a power of two, else 0xFFFFFFFF
-    u32 uniform_deme;          // != 0: every cell has this deme (no per-cell deme/prefix gathers needed)
+    u32 uniform_deme;          // != 0: every cell has this deme (host / init only; explicit kinds always carry the tables)
     u32 per_cell_turnover;     // 0: Cm_u/sh_u apply everywhere
     u32 Cm_u, sh_u;
     u64 n_locations;           // all indexed locations
@@ -62,6 +62,7 @@ struct EpochArgs {
     u32 k_stop;                // horizon: a lineage pauses when its interval index reaches k_stop
     u32 max_steps;             // 0 = unlimited
     u32 lanes_per_warp;        // lanes of each warp that hold lineages (32 = saturated; fewer in the tail)
+    u32 probe_mask;            // an event probes the dedup cache iff (hash >> 29) & probe_mask == 0 (0 = every event)
 };
 
 }  // namespace necsim

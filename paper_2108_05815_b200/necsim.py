@@ -29,7 +29,7 @@ class ScenarioDesc(C.Structure):
 class SimParams(C.Structure):
     _fields_ = [("block_threads", C.c_uint32), ("grid_blocks", C.c_uint32), ("dedup", C.c_uint32),
                 ("dedup_log2_slots", C.c_uint32), ("epoch_events", C.c_uint64), ("max_steps", C.c_uint64),
-                ("tail_threshold", C.c_uint32), ("reserved", C.c_uint32)]
+                ("tail_threshold", C.c_uint32), ("dedup_probe", C.c_uint32)]
 
 
 class Result(C.Structure):
@@ -111,11 +111,13 @@ def _dev_u32(torch, a, n=None):
     return torch.from_numpy(a.view(np.int32)).cuda()
 
 
-def make_params(block_threads=0, grid_blocks=0, dedup=None, dedup_log2_slots=0, epoch_events=0, max_steps=0, tail_threshold=0):
+def make_params(block_threads=0, grid_blocks=0, dedup=None, dedup_log2_slots=0, epoch_events=0, max_steps=0, tail_threshold=0,
+                dedup_probe=0):
     p = SimParams()
     p.block_threads, p.grid_blocks = block_threads, grid_blocks
     p.dedup = 0 if dedup is None else (1 if dedup else 2)
     p.dedup_log2_slots, p.epoch_events, p.max_steps, p.tail_threshold = dedup_log2_slots, epoch_events, max_steps, tail_threshold
+    p.dedup_probe = dedup_probe
     return p
 
 
