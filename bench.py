@@ -23,14 +23,15 @@ import numpy as np
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 from paper_2108_05815_b200 import inputs as I  # noqa: E402
+from paper_2108_05815_b200 import dist as D    # noqa: E402
 
 METRIC = "lineage_events_per_s"
 UNIT = "events/s"
 MAKERS = dict(c1=I.c1_nonspatial, c2=I.c2_implicit, c3=I.c3_matrix, c4=I.c4_gaussian, c5=I.c5_stress)
 SMALL = dict(zip(("c1", "c2", "c3", "c4", "c5"), range(5)))
-# Algorithmic integer instructions per executed event (counted on the straight-line
-# SASS of each primitive, weighted by the expected number of draws per event at mu = 2).
-I_EVENT = dict(c1=262, c2=270, c3=300, c4=345, c5=360)
+# Algorithmic integer instructions per executed event (minimal 32-bit instruction sequence of
+# each primitive, weighted by the expected number of draws per event at mu = 2 and the measured attempts per event).
+I_EVENT = dict(c1=230, c2=232, c3=252, c4=263, c5=272)
 # issue-slot peak: 148 SMs x 4 schedulers x 32 lanes x 1 instr/clk x sm_max_mhz (B300_MICROARCH "Pipe rates")
 def alu_peak(sm_count, sm_mhz):
     return sm_count * 4 * 32 * sm_mhz * 1e6
@@ -45,7 +46,7 @@ def cpu_sample(cfg, name, budget_events=30_000_000):
     n_ind = I.n_individuals(cfg)
     mask = np.ones(n_ind, np.uint8) if cfg["mask"] is None else np.asarray(cfg["mask"], np.uint8).copy()
     rng = np.random.Generator(np.random.PCG64(12345))
-    n_lin, max_steps = 2000, 15_000
+    n_lin, max_steps = 4000, 20_000
     idx = np.flatnonzero(mask)
     if len(idx) > n_lin:
         keep = rng.choice(idx, n_lin, replace=False)
@@ -142,7 +143,7 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     # weak scaling: every rank runs the same landscape with its own seed (independent replicate simulations,
     # the paper's repeated-runs use, L1240-1246); no data-path collective.
-    seed = cfg["seed"] + rank
+    seed = D.replica_seed(cfg["seed"], rank)
     sc = ns.Scenario(**I.scenario_kwargs(cfg))
     n_ind, n_s = sc.n_individuals, I.n_sampled(cfg)
     h_mask = None
@@ -178,10 +179,11 @@ def main():
     sampler = ClockSampler(local)
     sampler.start()
     barrier()
-    ms, ev, sim_ms, launches, epochs, res = 0.0, 0, 0.0, 0, 0, None
+    ms, ev, sim_ms, tail_ms, ev_tail, launches, epochs, res = 0.0, 0, 0.0, 0.0, 0, 0, 0, None
     for _ in range(args.steps):
         res = step_device()
         ms += res.ms_total; sim_ms += res.ms_simulate; ev += res.n_events_raw; launches += res.n_kernel_launches; epochs += res.n_epochs
+        tail_ms += res.ms_simulate_tail; ev_tail += res.n_events_tail
     barrier()
     clocks = sampler.stop()
     # end to end: host buffers in, host buffers out, copies inside the timed region
@@ -192,17 +194,10 @@ def main():
         res_h, dt = step_host()
         e2e_s += dt; e2e_ev += res_h.n_events_raw
     barrier()
-    t = torch.tensor([ms, e2e_s * 1e3, float(ev), float(e2e_ev), sim_ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        tmax = t.clone(); dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        tsum = t.clone(); dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
-        ms, e2e_ms, sim_ms = tmax[0].item(), tmax[1].item(), tmax[4].item()
-        ev_all, e2e_ev_all = tsum[2].item(), tsum[3].item()
-    else:
-        e2e_ms, ev_all, e2e_ev_all = e2e_s * 1e3, float(ev), float(e2e_ev)
+    (ms, e2e_ms, sim_ms), (ev_all, e2e_ev_all) = D.aggregate([ms, e2e_s * 1e3, sim_ms], [float(ev), float(e2e_ev)], device="cuda")
     if rank == 0:
         K = args.steps
-        value = ev_all / (ms * 1e-3)
+        value = D.throughput(ev_all, ms)
         prop = torch.cuda.get_device_properties(local)
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))) if os.path.exists(os.path.join(ROOT, "MEASURED_PEAKS.json")) else {}
         sm_max = float(peaks.get("sm_max_mhz", clocks.get("sm_max_mhz") or 1965.0))
@@ -223,7 +218,11 @@ def main():
                 "gpu_launches": int(launches),
                 "individuals_per_s": world * res.n_lineages / (ms / K * 1e-3),
                 "richness": int(res.richness), "epochs_per_step": epochs / K, "raw_events_per_step": ev / K,
-                "roofline": {"bound": "alu", "kernel": "simulate_kernel (all epochs of a step)", "achieved": achieved / 1e12, "peak": peak / 1e12,
+                "phases": {"saturated": {"events_per_s": (ev - ev_tail) / max((sim_ms - tail_ms) * 1e-3, 1e-9), "ms_per_step": (sim_ms - tail_ms) / K,
+                                         "events_per_step": (ev - ev_tail) / K, "kernel": "simulate_kernel (one lineage per lane)"},
+                           "tail": {"events_per_s": ev_tail / max(tail_ms * 1e-3, 1e-9), "ms_per_step": tail_ms / K, "events_per_step": ev_tail / K,
+                                    "kernel": "tail_kernel (one lineage per warp; bound by event latency x chain length, DESIGN.md 6.3)"}},
+                "roofline": {"bound": "alu", "kernel": "simulate_kernel + tail_kernel (all epochs of a step)", "achieved": achieved / 1e12, "peak": peak / 1e12,
                              "unit": "Tinstr/s", "frac": achieved / peak, "traffic": None, "instr_per_event": I_EVENT[name],
                              "peak_source": "derived: SMs x 4 schedulers x 32 lanes x sm_max_mhz (DESIGN.md section 6)",
                              "measured_int_peaks_Tinstr_s": {k: v / 1e12 for k, v in int_meas.items()}},

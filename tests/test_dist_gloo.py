@@ -1,0 +1,41 @@
+"""World-size-2 gloo test (CPU) of the N>1 host logic bench.py uses: replica seeds, sum of units, max of times."""
+import os
+import socket
+
+import torch
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+
+def _free_port():
+    s = socket.socket(); s.bind(("127.0.0.1", 0)); p = s.getsockname()[1]; s.close(); return p
+
+
+def _worker(rank, world, port, out):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    from paper_2108_05815_b200 import dist as D
+    seed = D.replica_seed(42, rank)
+    times, units = D.aggregate([10.0 + 5.0 * rank, 3.0 - rank], [1000.0 * (rank + 1), 7.0])
+    out[rank] = (seed, times, units, D.throughput(units[0], times[0]))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_two_rank_aggregation():
+    world, port = 2, _free_port()
+    mgr = mp.Manager()
+    out = mgr.dict()
+    mp.spawn(_worker, args=(world, port, out), nprocs=world, join=True)
+    assert out[0][0] == 42 and out[1][0] == 43
+    for r in range(world):
+        _, times, units, thr = out[r]
+        assert times == [15.0, 3.0]                 # max over ranks
+        assert units == [3000.0, 14.0]              # sum over ranks
+        assert abs(thr - 3000.0 / 0.015) < 1e-6
+
+
+def test_single_process_is_identity():
+    from paper_2108_05815_b200 import dist as D
+    assert D.aggregate([1.5], [2.0]) == ([1.5], [2.0])
+    assert D.replica_seed(2**64 - 1, 1) == 0

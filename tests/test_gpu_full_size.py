@@ -1,0 +1,68 @@
+"""Parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (default necsim_sim_params).
+
+(a) whole result against tests/golden/full_configs.json, written by tests/golden/gen_golden.py --full from the oracle
+    only: richness, a SHA-256 over every event field and every label (= element-by-element equality), first/last events;
+(b) sampled outputs the oracle computes one by one: for a few sampled individuals the oracle traces that single
+    lineage alone (no dedup involved) and the GPU's events[labels[i]] must be the speciation event it reaches.
+"""
+import hashlib
+import json
+import os
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+HERE = os.path.dirname(os.path.abspath(__file__))
+GOLDEN = os.path.join(HERE, "golden", "full_configs.json")
+
+
+def digest(res):
+    h = hashlib.sha256()
+    for name in ("loc", "k", "j", "f", "abundance"):
+        h.update(np.ascontiguousarray(res["events"][name]).tobytes())
+    h.update(np.ascontiguousarray(res["events"]["time"]).tobytes())
+    h.update(np.ascontiguousarray(res["labels"]).tobytes())
+    return h.hexdigest()
+
+
+@pytest.fixture(scope="module")
+def golden():
+    if not os.path.exists(GOLDEN):
+        pytest.skip("tests/golden/full_configs.json not generated")
+    return {g["name"]: g for g in json.load(open(GOLDEN))}
+
+
+@pytest.mark.parametrize("idx", range(5))
+def test_full_config_matches_oracle(O, golden, idx):
+    from paper_2108_05815_b200 import inputs as I, necsim as ns
+    cfg = [I.c1_nonspatial, I.c2_implicit, I.c3_matrix, I.c4_gaussian, I.c5_stress][idx]()
+    if cfg["name"] not in golden:
+        pytest.skip("no golden record for " + cfg["name"])
+    g = golden[cfg["name"]]
+    sc = ns.Scenario(**I.scenario_kwargs(cfg))
+    got = sc.simulate(cfg["seed"], cfg["nu"], cfg["mask"])
+    assert len(got["labels"]) == g["n_sampled"]
+    assert got["richness"] == g["richness"]
+    ev = got["events"]
+    rows = lambda a: [[int(e["loc"]), int(e["k"]), int(e["j"]), int(e["f"]), int(e["abundance"])] for e in a]
+    assert rows(ev[:5]) == g["first_events"] and rows(ev[-5:]) == g["last_events"]
+    assert [int(v) for v in got["labels"][:16]] == g["labels_head"]
+    assert digest(got) == g["digest"]
+    # properties that hold at any size
+    assert int(ev["abundance"].sum()) == g["n_sampled"] and (ev["abundance"] > 0).all()
+    key = np.stack([ev["k"].astype(np.uint64), ev["f"], ev["loc"].astype(np.uint64), ev["j"].astype(np.uint64)], axis=1)
+    assert all(tuple(key[i]) < tuple(key[i + 1]) for i in range(len(key) - 1))
+    assert got["stats"]["n_events_raw"] >= g["unique_events"]
+    # (b) single lineages, one by one
+    n_ind = sc.n_individuals
+    sampled = np.arange(n_ind) if cfg["mask"] is None else np.flatnonzero(cfg["mask"])
+    rng = np.random.default_rng(idx)
+    osc = O.Scenario(**I.scenario_kwargs(cfg))
+    for pos in rng.choice(len(sampled), 3, replace=False):
+        m = np.zeros(n_ind, np.uint8); m[sampled[pos]] = 1
+        one = osc.simulate(cfg["seed"], cfg["nu"], m, dedup=False)
+        e, mine = one["events"][0], ev[got["labels"][pos]]
+        assert (int(e["loc"]), int(e["k"]), int(e["j"]), int(e["f"])) == (int(mine["loc"]), int(mine["k"]), int(mine["j"]), int(mine["f"]))
+        assert e["time"] == mine["time"]
+    sc.close()
