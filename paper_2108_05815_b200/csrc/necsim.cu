@@ -455,6 +455,7 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
     const u32 warps_per_block = rp.block_threads / 32u;
     // one lineage per warp pays off once every active lineage can have a resident warp of its own
     const u32 tail_threshold = rp.tail_threshold ? rp.tail_threshold : tail_grid * warps_per_block;
+    const u32 full_cache_mask = rp.dedup ? ((1u << rp.dedup_log2_slots) - 1u) : 0u;
     u32 active = n_sampled, k_start = 0;
     uint4 *q_in = qa, *q_out = qb;
     float ms_sim = 0.f, ms_tail = 0.f;
@@ -483,6 +484,8 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
             if (lanes == 1) grid = (u32)std::min<u64>(full_grid, ((u64)active + warps_per_block - 1) / warps_per_block);
         }
         bf.q_in = q_in; bf.q_out = q_out; bf.q_in_count = active;
+        // a few thousand lineages need few slots: keep the tail's cache footprint (2 MiB) inside L2 next to the tables
+        bf.cache_mask = rp.dedup ? (tail ? std::min(full_cache_mask, (1u << 17) - 1u) : full_cache_mask) : 0u;
         CU(cudaMemsetAsync(bf.ctr, 0, 8, st));   // q_head, q_out
         CU(cudaEventRecord(scn->ev[2], st));
         (tail ? fn_tail : fn_main)<<<grid, rp.block_threads, 0, st>>>(sd, bf, ep);
