@@ -3,9 +3,11 @@
 // One lineage per lane (PAPER.md 5.2 L675-747: "each lineage simulated alone"). A lane whose lineage
 // ended (speciated / culled as a duplicate / reached the epoch's time horizon / step cap) takes the
 // next lineage from the device work queue: one atomicAdd per warp per refill (ballot + popc).
-// The loop body is a state machine that performs exactly one event-time draw per iteration for every
-// live lane (sum Exp draws from the interval start until the first partial sum
-// after the lineage's last event), so lanes of a warp only diverge on the rarer event branch.
+// Every lane is a small state machine: SEARCH (one exponential draw of the event-time search per pass, PAPER.md
+// L725-729: sum Exp draws from the interval start until the first partial sum after the lineage's last event) or
+// EVENT (duplicate probe + speciation test on the first pass, then one dispersal attempt per pass). Each loop
+// iteration the WARP runs the phase that more of its lanes are waiting for (a ballot decides), so both phases
+// execute densely instead of the rarer one running at a fraction of the lanes.
 #pragma once
 #include "sim_types.cuh"
 
@@ -155,6 +157,10 @@ __device__ __forceinline__ bool cache_probes(u32 h, u32 probe_mask) { return ((h
 __device__ unsigned short NEGLOG_Q_DEV[512];
 __device__ u64 NEGLOG_A_DEV[512];
 
+#define NS_ST_IDLE 0u
+#define NS_ST_SEARCH 1u     // needs draws of the event-time search (re-primes first when `need_prime`)
+#define NS_ST_EVENT 2u      // event (loc, k, j) found at offset T: `att` dispersal attempts rejected so far
+
 template <int KIND, bool DEDUP, bool PERCELL>
 __global__ void __launch_bounds__(256) simulate_kernel(const ScenarioDev sc, const SimBuffers bf, const EpochArgs ep) {
     __shared__ unsigned short sQ[512];
@@ -170,7 +176,8 @@ __global__ void __launch_bounds__(256) simulate_kernel(const ScenarioDev sc, con
     const bool lane_on = lane < ep.lanes_per_warp;
 
     // lineage state (registers)
-    bool has = false, need_prime = false, exhausted = false;
+    u32 st = NS_ST_IDLE, att = 0;
+    bool need_prime = false, exhausted = false;
     u32 id = 0, loc = 0, cell = 0, k = 0, steps = 0, j = 0, Cm = sc.Cm_u, sh = sc.sh_u;
     i64 f_last = -1;
     u64 X = 0, T = 0;
@@ -178,95 +185,124 @@ __global__ void __launch_bounds__(256) simulate_kernel(const ScenarioDev sc, con
 
     for (;;) {
         // ---- S4: refill idle lanes from the device work queue (one atomic per warp) -----------------
-        u32 need = __ballot_sync(NS_FULL, lane_on && !has);
+        const u32 need = __ballot_sync(NS_FULL, lane_on && st == NS_ST_IDLE);
         if (need != 0u && !exhausted) {
             u32 cnt = __popc(need), base = 0;
             if (lane == 0) base = atomicAdd(&bf.ctr->q_head, cnt);
             base = __shfl_sync(NS_FULL, base, 0);
-            if (lane_on && !has) {
+            if (lane_on && st == NS_ST_IDLE) {
                 u32 idx = base + __popc(need & lanemask_lt());
                 if (idx < bf.q_in_count) {
                     uint4 e = bf.q_in[idx];
                     id = e.x; loc = e.y; cell = e.z; steps = e.w;
-                    k = ep.k_start; f_last = -1; need_prime = true; has = true;
+                    k = ep.k_start; f_last = -1; need_prime = true; st = NS_ST_SEARCH;
                 }
             }
             exhausted = (base + cnt >= bf.q_in_count);
         }
-        if (!__any_sync(NS_FULL, has)) break;
+        const u32 n_search = __popc(__ballot_sync(NS_FULL, st == NS_ST_SEARCH));
+        const u32 n_event = __popc(__ballot_sync(NS_FULL, st == NS_ST_EVENT));
+        if ((n_search | n_event) == 0u) break;
 
-        // ---- S1a: (re-)prime on (loc, k); pause at the epoch horizon -------------------------------
-        bool pause = false;
-        if (has && need_prime) {
-            if (k == ep.k_stop) {
-                pause = true;
-            } else {
-                X = prime(ep.key, loc, k);
-                T = 0; j = 0; need_prime = false;
-                if (PERCELL) { uint2 cs = __ldg(&sc.scale[KIND == 3 ? xy_index(sc, cell) : cell]); Cm = cs.x; sh = cs.y; }
-            }
-        }
-        {   // survivors of this epoch go to the output queue (warp-aggregated append)
-            u32 pm = __ballot_sync(NS_FULL, pause);
-            if (pm) {
-                u32 base = 0;
-                if (lane == (u32)(__ffs(pm) - 1)) base = atomicAdd(&bf.ctr->q_out, __popc(pm));
-                base = __shfl_sync(NS_FULL, base, __ffs(pm) - 1);
-                if (pause) {
-                    bf.q_out[base + __popc(pm & lanemask_lt())] = make_uint4(id, loc, cell, steps);
-                    has = false;
+        if (n_event <= n_search) {
+            // ======== SEARCH phase ======================================================================
+            // S1a: (re-)prime on (loc, k); pause at the epoch horizon
+            bool pause = false;
+            if (st == NS_ST_SEARCH && need_prime) {
+                if (k == ep.k_stop) {
+                    pause = true;
+                } else {
+                    X = prime(ep.key, loc, k);
+                    T = 0; j = 0; need_prime = false;
+                    if (PERCELL) { uint2 cs = __ldg(&sc.scale[KIND == 3 ? xy_index(sc, cell) : cell]); Cm = cs.x; sh = cs.y; }
                 }
             }
-        }
-        if (!has) continue;
-
-        // ---- S1b: one exponential draw of the event-time search ------------------------------------
-        j += 1; X += NS_GAMMA;
-        T += scale_exp(neglog(draw_time(X), sQ, sA), Cm, sh);
-        if (T >= NS_TWO48) {                       // interval exhausted: cross and re-prime (L719, L727)
-            if (k == 0xFFFFFFFFu) { atomicMax(&bf.ctr->error, 3u); has = false; continue; }
-            k += 1; f_last = -1; need_prime = true;
-            continue;
-        }
-        if ((i64)T <= f_last) continue;            // not strictly later than the last event (L729)
-
-        // ---- event (loc, k, j) at offset T ----------------------------------------------------------
-        // S5: duplicate-culling cache keyed on the full event identity. The 128-bit exchange is issued first and
-        // its result consumed after the (side-effect free) speciation and dispersal draws, hiding the L2 round trip.
-        uint4 old = make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu);
-        if (DEDUP) {
-            const u32 h = cache_hash(loc, k, j);
-            if (cache_probes(h, ep.probe_mask)) old = atomic_exch_128(&bf.cache[h & bf.cache_mask], make_uint4(loc, k, j, id));
-        }
-        // S2: speciation test on the event's SPEC lane
-        const bool can_speciate = !(KIND == 1 && cell == 0);     // local community of the implicit model: nu = 0 (L1830)
-        const bool speciates = can_speciate && bern(draw_spec(X), ep.thr_nu);
-        // S3: dispersal to the parent's location
-        u32 loc2 = loc, cell2 = cell;
-        bool ok = true;
-        if (!speciates) ok = disperse<KIND>(sc, ep.thr_m, X, cell, loc2, cell2, gl, c_resamples);
-        if (DEDUP && old.x == loc && old.y == k && old.z == j && old.w != id) {
-            // another lineage executed this event: identical future (L687, L697) -> cull, link to it
-            bf.parent[id] = old.w; bf.state[id] = 2;
-            bf.term_loc[id] = loc; bf.term_k[id] = k; bf.term_j[id] = j; bf.term_f[id] = T; bf.steps[id] = steps;
-            c_culled++; has = false;
-            continue;
-        }
-        f_last = (i64)T; steps++; c_events++;
-        if (speciates) {
-            bf.state[id] = 1;
-            bf.term_loc[id] = loc; bf.term_k[id] = k; bf.term_j[id] = j; bf.term_f[id] = T; bf.steps[id] = steps;
-            bf.spec_ring[atomicAdd(&bf.ctr->n_spec, 1u)] = id;
-            atomicMax(&bf.ctr->j_max, j);
-            has = false;
-            continue;
-        }
-        if (!ok) { atomicMax(&bf.ctr->error, 3u); has = false; continue; }
-        loc = loc2; cell = cell2; need_prime = true;
-        if (ep.max_steps && steps >= ep.max_steps) {
-            bf.state[id] = 3;
-            bf.term_loc[id] = loc; bf.term_k[id] = k; bf.term_j[id] = j; bf.term_f[id] = T; bf.steps[id] = steps;
-            has = false;
+            {   // survivors of this epoch go to the output queue (warp-aggregated append)
+                u32 pm = __ballot_sync(NS_FULL, pause);
+                if (pm) {
+                    u32 base = 0;
+                    if (lane == (u32)(__ffs(pm) - 1)) base = atomicAdd(&bf.ctr->q_out, __popc(pm));
+                    base = __shfl_sync(NS_FULL, base, __ffs(pm) - 1);
+                    if (pause) {
+                        bf.q_out[base + __popc(pm & lanemask_lt())] = make_uint4(id, loc, cell, steps);
+                        st = NS_ST_IDLE;
+                    }
+                }
+            }
+            if (st == NS_ST_SEARCH) {
+                // S1b: one exponential draw of the event-time search
+                j += 1; X += NS_GAMMA;
+                T += scale_exp(neglog(draw_time(X), sQ, sA), Cm, sh);
+                if (T >= NS_TWO48) {                       // interval exhausted: cross and re-prime (L719, L727)
+                    if (k == 0xFFFFFFFFu) { atomicMax(&bf.ctr->error, 3u); st = NS_ST_IDLE; }
+                    else { k += 1; f_last = -1; need_prime = true; }
+                } else if ((i64)T > f_last) {              // strictly later than the last event (L729): the next event
+                    st = NS_ST_EVENT; att = 0;
+                }
+            }
+        } else if (st == NS_ST_EVENT) {
+            // ======== EVENT phase: event (loc, k, j) at offset T ==========================================
+            bool culled = false, speciates = false;
+            uint4 old = make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu);
+            if (att == 0) {
+                // S5: duplicate-culling cache keyed on the full event identity; the 128-bit exchange is issued first
+                // and consumed after the (side-effect free) speciation and dispersal draws of this pass
+                if (DEDUP) {
+                    const u32 h = cache_hash(loc, k, j);
+                    if (cache_probes(h, ep.probe_mask)) old = atomic_exch_128(&bf.cache[h & bf.cache_mask], make_uint4(loc, k, j, id));
+                }
+                // S2: speciation test on the event's SPEC lane (local community of the implicit model: nu = 0, L1830)
+                speciates = !(KIND == 1 && cell == 0) && bern(draw_spec(X), ep.thr_nu);
+            }
+            // S3: one dispersal attempt (KIND 0..2 always accept)
+            u32 loc2 = loc, cell2 = cell;
+            bool accept = true;
+            if (KIND != 3) {
+                u32 rs = 0;
+                disperse<KIND>(sc, ep.thr_m, X, cell, loc2, cell2, gl, rs);
+            } else {
+                const u64 x = draw_disp(X, att);
+                const u32 xx = wrap_add(cell & 0xFFFFu, gauss_disp(gl, (u32)(x >> 32)), sc.width);
+                const u32 yy = wrap_add(cell >> 16, gauss_disp(gl, (u32)x), sc.height);
+                const u32 c2 = yy * sc.width + xx;
+                const u32 d = cell_deme(sc, c2);
+                accept = d > 0u;
+                if (accept) {
+                    cell2 = (yy << 16) | xx;
+                    loc2 = cell_prefix(sc, c2) + ((d == 1u) ? 0u : mulhi64_u32(draw_index(X), d));
+                }
+            }
+            if (att == 0) {
+                if (DEDUP) culled = old.x == loc && old.y == k && old.z == j && old.w != id;
+                if (culled) {
+                    // another lineage executed this event: identical future (L687, L697) -> cull, link to it
+                    bf.parent[id] = old.w; bf.state[id] = 2;
+                    bf.term_loc[id] = loc; bf.term_k[id] = k; bf.term_j[id] = j; bf.term_f[id] = T; bf.steps[id] = steps;
+                    c_culled++; st = NS_ST_IDLE;
+                } else {
+                    f_last = (i64)T; steps++; c_events++;
+                    if (speciates) {
+                        bf.state[id] = 1;
+                        bf.term_loc[id] = loc; bf.term_k[id] = k; bf.term_j[id] = j; bf.term_f[id] = T; bf.steps[id] = steps;
+                        bf.spec_ring[atomicAdd(&bf.ctr->n_spec, 1u)] = id;
+                        atomicMax(&bf.ctr->j_max, j);
+                        st = NS_ST_IDLE;
+                    }
+                }
+            }
+            if (st == NS_ST_EVENT) {
+                if (accept) {
+                    loc = loc2; cell = cell2; need_prime = true; st = NS_ST_SEARCH;
+                    if (ep.max_steps && steps >= ep.max_steps) {
+                        bf.state[id] = 3;
+                        bf.term_loc[id] = loc; bf.term_k[id] = k; bf.term_j[id] = j; bf.term_f[id] = T; bf.steps[id] = steps;
+                        st = NS_ST_IDLE;
+                    }
+                } else {
+                    c_resamples++;
+                    if (++att >= NS_MAX_RESAMPLE) { atomicMax(&bf.ctr->error, 3u); st = NS_ST_IDLE; }
+                }
+            }
         }
     }
     // reduce the per-thread counters: warp shuffle, then one atomic per warp
