@@ -8,57 +8,18 @@
 //   - candidates: lanes 0..15 hold the points j = 1..16 of interval k (a segmented prefix sum gives the partial
 //     sums T_j), lanes 16..31 the FIRST point of intervals k+1..k+16 (the event if interval k is exhausted: a
 //     fresh interval's first point is its next event, L719-729);
-//   - every lane also evaluates the speciation draw and the first dispersal attempt of ITS candidate (with the
-//     habitat / prefix / turnover-scale gathers) while its -ln chain is in flight, so that when the winning
-//     candidate is known the event is already decided and the next search starts at once;
+//   - once the winning candidate is known, ONE hash evaluation across the lanes yields all the event's draws: lane 0
+//     the speciation draw, lane 1 the index draw, lane 2 the migration draw, lanes 3..31 the dispersal attempts
+//     r = 0..28 (R16), each with its habitat / prefix / turnover-scale gathers; a ballot picks the first accepted;
 //   - the duplicate-culling exchange of an event is issued when the event is selected and consumed one event
-//     later (never after another cache insertion: an unconfirmed lineage must not publish entries);
-//   - rejected dispersal targets fall back to eight attempts at a time.
+//     later (never after another cache insertion: an unconfirmed lineage must not publish entries).
 #pragma once
 #include "sim_kernel.cuh"
 
 namespace necsim {
 
-#define NS_TAIL_ATTEMPTS 8u
+#define NS_TAIL_ATTEMPTS 29u      // dispersal attempts evaluated per pass (lanes 3..31)
 
-// Dispersal of one candidate event (stream position X), written branch-free so that it schedules into the
-// latency of the candidate's -ln chain. KIND 0..2: the complete dispersal. KIND 3: attempt 0 only;
-// ok = target is habitat; exact = false where the table lookups need their rare exact path (then the caller
-// re-evaluates from attempt 0).
-template <int KIND, bool PERCELL>
-__device__ __forceinline__ void candidate_disperse(const ScenarioDev &sc, u64 thr_m, u64 X, u32 cell, const GaussLut &gl,
-                                                   u32 &loc2, u32 &cell2, u32 &Cm2, u32 &sh2, bool &ok, bool &exact) {
-    ok = true; exact = true;
-    u32 idx2 = 0;
-    if (KIND == 0) {
-        loc2 = mulhi64_u32(draw_disp(X, 0), (u32)sc.n_locations); cell2 = 0;
-    } else if (KIND == 1) {
-        const u64 x = draw_disp(X, 0);
-        const bool to_meta = (cell != 0) || bern(draw_migr(X), thr_m);
-        const u32 lm = sc.J_local + mulhi64_u32(x, sc.J_meta), ll = mulhi64_u32(x, sc.J_local);
-        loc2 = to_meta ? lm : ll; cell2 = to_meta ? 1u : 0u;
-    } else if (KIND == 2) {
-        const u64 x = draw_disp(X, 0);
-        const u32 n = sc.ncells, col = __umulhi((u32)(x >> 32), n);
-        const uint2 e = __ldg(&sc.alias[(size_t)cell * n + col]);
-        cell2 = ((u32)x < e.x) ? col : e.y;
-        const u32 d = __ldg(&sc.hab8[cell2]);
-        exact = d != 255u;
-        loc2 = __ldg(&sc.prefix[cell2]) + mulhi64_u32(draw_index(X), d);     // d = 1 gives index 0
-        idx2 = cell2;
-    } else {
-        const u64 x = draw_disp(X, 0);
-        bool e1, e2;
-        const u32 xx = wrap_add(cell & 0xFFFFu, gauss_disp_fast(gl, (u32)(x >> 32), e1), sc.width);
-        const u32 yy = wrap_add(cell >> 16, gauss_disp_fast(gl, (u32)x, e2), sc.height);
-        idx2 = yy * sc.width + xx;
-        cell2 = (yy << 16) | xx;
-        const u32 d = __ldg(&sc.hab8[idx2]);
-        ok = d > 0u; exact = e1 && e2 && d != 255u;
-        loc2 = __ldg(&sc.prefix[idx2]) + mulhi64_u32(draw_index(X), d);
-    }
-    if (PERCELL) { const uint2 cs = __ldg(&sc.scale[idx2]); Cm2 = cs.x; sh2 = cs.y; }
-}
 
 template <int KIND, bool DEDUP, bool PERCELL>
 __global__ void __launch_bounds__(256) tail_kernel(const ScenarioDev sc, const SimBuffers bf, const EpochArgs ep) {
@@ -72,7 +33,10 @@ __global__ void __launch_bounds__(256) tail_kernel(const ScenarioDev sc, const S
     GaussLut gl; gl.tg = sG; gl.g2 = sG2; gl.R = sc.R;
 
     const u32 lane = threadIdx.x & 31u, half = lane >> 4, sub = lane & 15u;
-    const u32 jj = half ? 1u : sub + 1u;                               // ordinal of this lane's candidate
+    const u32 jj = half ? 1u : sub + 1u;                               // ordinal of this lane's candidate point
+    // event draws, one per lane: draw = F((X ^ lane_xor) + lane_add)
+    const u64 lane_xor = lane == 0 ? NS_L_SPEC : lane == 1 ? NS_L_INDEX : lane == 2 ? NS_L_MIGR : NS_L_DISP;
+    const u32 att_lane = lane >= 3u ? lane - 3u : 0u;                  // dispersal attempt of this lane within a pass
     unsigned long long c_events = 0, c_culled = 0, c_resamples = 0;   // warp-uniform
 
     for (;;) {
@@ -115,16 +79,11 @@ __global__ void __launch_bounds__(256) tail_kernel(const ScenarioDev sc, const S
                 if (lane == 0) bf.q_out[atomicAdd(&bf.ctr->q_out, 1u)] = make_uint4(id, loc, cell, steps);
                 break;
             }
-            const bool can_speciate = !(KIND == 1 && cell == 0);      // local community of the implicit model: nu = 0 (L1830)
-            // ---- S1-S3 for this lane's candidate event, speculatively: time, speciation and dispersal draws --------
+            // ---- S1: candidate points of the event-time search ---------------------------------------------------
             const u64 kk64 = (u64)k + (half ? (u64)(1u + sub) : 0ull);
             const bool kvalid = kk64 < (u64)ep.k_stop;                // never look at or past the horizon
             u64 X = prime(ep.key, loc, (u32)kk64) + (u64)jj * NS_GAMMA;
             const u64 T1 = scale_exp(neglog(draw_time(X), sQ, sA), Cm, sh);
-            bool e_spec = can_speciate && bern(draw_spec(X), ep.thr_nu);
-            u32 e_loc2 = loc, e_cell2 = cell, e_Cm = Cm, e_sh = sh;
-            bool e_ok, e_exact;
-            candidate_disperse<KIND, PERCELL>(sc, ep.thr_m, X, cell, gl, e_loc2, e_cell2, e_Cm, e_sh, e_ok, e_exact);
             // partial sums over each 16-lane half (half 1 keeps its single draws: first points of fresh intervals)
             u64 T = T1;
 #pragma unroll
@@ -137,17 +96,19 @@ __global__ void __launch_bounds__(256) tail_kernel(const ScenarioDev sc, const S
             const u32 evm = __ballot_sync(NS_FULL, inside && (half ? kvalid : ((i64)T > f_last)));
             const u32 crm = __ballot_sync(NS_FULL, !inside);
             u32 j;
-            int src;
+            u64 Te, Xe;
             if (evm & 0xFFFFu) {                       // next event is in interval k
-                src = __ffs(evm & 0xFFFFu) - 1;
+                const int src = __ffs(evm & 0xFFFFu) - 1;
                 j = (u32)src + 1u;
+                Te = __shfl_sync(NS_FULL, T, src); Xe = __shfl_sync(NS_FULL, X, src);
             } else if (crm & 0xFFFFu) {                // interval k exhausted (L719, L727): first non-empty interval after it
                 const u32 gap = ep.k_stop - 1u - k;    // k < k_stop here
                 const u32 nvalid = gap < 16u ? gap : 16u;
                 const u32 hm = evm >> 16;
                 if (!hm) { k = k + 1u + nvalid; f_last = -1; continue; }   // all speculated intervals empty / beyond the horizon
-                src = 16 + __ffs(hm) - 1;
+                const int src = 16 + __ffs(hm) - 1;
                 k = k + 1u + (u32)(src - 16); j = 1u;
+                Te = __shfl_sync(NS_FULL, T, src); Xe = __shfl_sync(NS_FULL, X, src);
             } else {
                 // more than 16 points of interval k at or before f_last (large mu): continue the scan one draw at a time
                 u64 Tc = __shfl_sync(NS_FULL, T, 15), Xc = __shfl_sync(NS_FULL, X, 15);
@@ -160,19 +121,8 @@ __global__ void __launch_bounds__(256) tail_kernel(const ScenarioDev sc, const S
                     if ((i64)Tc > f_last) { found = true; break; }
                 }
                 if (!found) { k += 1u; f_last = -1; continue; }
-                // every lane evaluates the same candidate: lane 0 serves as the source below
-                j = jc; T = Tc; X = Xc; src = 0;
-                e_spec = can_speciate && bern(draw_spec(X), ep.thr_nu);
-                e_loc2 = loc; e_cell2 = cell; e_Cm = Cm; e_sh = sh;
-                candidate_disperse<KIND, PERCELL>(sc, ep.thr_m, X, cell, gl, e_loc2, e_cell2, e_Cm, e_sh, e_ok, e_exact);
+                j = jc; Te = Tc; Xe = Xc;
             }
-            const u64 Te = __shfl_sync(NS_FULL, T, src);
-            const u32 flags = __shfl_sync(NS_FULL, (e_spec ? 1u : 0u) | (e_ok ? 2u : 0u) | (e_exact ? 4u : 0u), src);
-            u32 loc2 = __shfl_sync(NS_FULL, e_loc2, src), cell2 = __shfl_sync(NS_FULL, e_cell2, src);
-            u32 Cm2 = Cm, sh2 = sh;
-            if (PERCELL) { Cm2 = __shfl_sync(NS_FULL, e_Cm, src); sh2 = __shfl_sync(NS_FULL, e_sh, src); }
-            const bool speciates = flags & 1u;
-            bool ok = (flags & 6u) == 6u;              // accepted by the fast path
 
             // ---- event (loc, k, j) at offset Te --------------------------------------------------------------
             // S5: the previous probing event's exchange is consumed before this event may publish a cache entry
@@ -187,41 +137,58 @@ __global__ void __launch_bounds__(256) tail_kernel(const ScenarioDev sc, const S
                 }
             }
             if (!probes) { steps++; c_events++; }
-            if (KIND >= 2 && !speciates && !ok) {
-                // S3 slow path: exact lookups; attempts r0.. eight at a time (R16). Attempt 0 is known rejected when
-                // the fast path was exact.
-                const u64 Xe = __shfl_sync(NS_FULL, X, src);
-                if (KIND == 2) {
-                    u32 rs = 0;
-                    ok = disperse<2>(sc, ep.thr_m, Xe, cell, loc2, cell2, gl, rs);
+            // S2 + S3: all draws of the event in one hash evaluation across the lanes
+            const u64 xb = Xe ^ lane_xor;
+            u64 u = hashF(xb + (u64)att_lane * NS_GAMMA);
+            const bool can_speciate = !(KIND == 1 && cell == 0);      // local community of the implicit model: nu = 0 (L1830)
+            const u32 bm = __ballot_sync(NS_FULL, bern(u, lane == 2 ? ep.thr_m : ep.thr_nu));
+            const bool speciates = can_speciate && (bm & 1u);
+            u32 loc2 = loc, cell2 = cell, Cm2 = Cm, sh2 = sh;
+            bool ok = true;
+            if (!speciates) {
+                if (KIND == 0) {
+                    loc2 = mulhi64_u32(__shfl_sync(NS_FULL, u, 3), (u32)sc.n_locations); cell2 = 0;
+                } else if (KIND == 1) {
+                    const u64 x = __shfl_sync(NS_FULL, u, 3);
+                    const bool to_meta = (cell != 0) || (bm & 4u);
+                    if (to_meta) { loc2 = sc.J_local + mulhi64_u32(x, sc.J_meta); cell2 = 1; }
+                    else { loc2 = mulhi64_u32(x, sc.J_local); cell2 = 0; }
+                } else if (KIND == 2) {
+                    const u64 x = __shfl_sync(NS_FULL, u, 3), xi = __shfl_sync(NS_FULL, u, 1);
+                    const u32 n = sc.ncells, col = __umulhi((u32)(x >> 32), n);
+                    const uint2 e = __ldg(&sc.alias[(size_t)cell * n + col]);
+                    cell2 = ((u32)x < e.x) ? col : e.y;
+                    const u32 d = cell_deme(sc, cell2);
+                    loc2 = cell_prefix(sc, cell2) + ((d == 1u) ? 0u : mulhi64_u32(xi, d));
                     if (PERCELL) { const uint2 cs = __ldg(&sc.scale[cell2]); Cm2 = cs.x; sh2 = cs.y; }
                 } else {
-                    const u64 xi = draw_index(Xe);
+                    const u64 xi = __shfl_sync(NS_FULL, u, 1);
                     const u32 x0 = cell & 0xFFFFu, y0 = cell >> 16;
-                    for (u32 r0 = (flags & 4u) ? 1u : 0u; r0 < NS_MAX_RESAMPLE; r0 += NS_TAIL_ATTEMPTS) {
+                    ok = false;
+                    for (u32 r0 = 0; r0 < NS_MAX_RESAMPLE; r0 += NS_TAIL_ATTEMPTS) {
                         u32 c2 = 0, d = 0, pf = 0;
                         uint2 cs = make_uint2(Cm, sh);
-                        if (lane < NS_TAIL_ATTEMPTS) {
-                            const u64 x = draw_disp(Xe, r0 + lane);
-                            const u32 xx = wrap_add(x0, gauss_disp(gl, (u32)(x >> 32)), sc.width);
-                            const u32 yy = wrap_add(y0, gauss_disp(gl, (u32)x), sc.height);
+                        if (lane >= 3u) {   // attempt r0 + lane - 3 (R16: redraw the whole (dx, dy) pair)
+                            const u32 xx = wrap_add(x0, gauss_disp(gl, (u32)(u >> 32)), sc.width);
+                            const u32 yy = wrap_add(y0, gauss_disp(gl, (u32)u), sc.height);
                             const u32 ci = yy * sc.width + xx;
                             c2 = (yy << 16) | xx;
                             d = cell_deme(sc, ci);
                             pf = cell_prefix(sc, ci);                       // speculative: same round trip as the habitat test
                             if (PERCELL) cs = __ldg(&sc.scale[ci]);
                         }
-                        const u32 okm = __ballot_sync(NS_FULL, lane < NS_TAIL_ATTEMPTS && d > 0);
+                        const u32 okm = __ballot_sync(NS_FULL, lane >= 3u && d > 0u);
                         if (okm) {
                             const int w = __ffs(okm) - 1;    // first accepted attempt = the sequential algorithm's choice
                             c2 = __shfl_sync(NS_FULL, c2, w); d = __shfl_sync(NS_FULL, d, w); pf = __shfl_sync(NS_FULL, pf, w);
-                            Cm2 = __shfl_sync(NS_FULL, cs.x, w); sh2 = __shfl_sync(NS_FULL, cs.y, w);
+                            if (PERCELL) { Cm2 = __shfl_sync(NS_FULL, cs.x, w); sh2 = __shfl_sync(NS_FULL, cs.y, w); }
                             cell2 = c2;
                             loc2 = pf + ((d == 1u) ? 0u : mulhi64_u32(xi, d));
-                            c_resamples += r0 + (u32)w;
+                            c_resamples += r0 + (u32)w - 3u;
                             ok = true;
                             break;
                         }
+                        u = hashF(xb + (u64)(r0 + NS_TAIL_ATTEMPTS + att_lane) * NS_GAMMA);   // next 29 attempts
                     }
                 }
             }
