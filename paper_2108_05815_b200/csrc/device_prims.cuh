@@ -40,10 +40,15 @@ typedef int64_t i64;
 
 // one Feistel round: p = a*M; (a, b) <- (hi32(p) ^ b ^ K, lo32(p))   [1 IMAD.WIDE.U32 + 1 LOP3]
 __host__ __device__ __forceinline__ void feistel(u32 &a, u32 &b, u32 M, u32 K) {
-    u64 p = (u64)a * (u64)M;
-    u32 na = (u32)(p >> 32) ^ b ^ K;
-    b = (u32)p;
-    a = na;
+    // written as separate low / high products: nvcc fuses them into ONE IMAD.WIDE.U32 (the u64 form costs an extra add)
+#ifdef __CUDA_ARCH__
+    const u32 lo = a * M, hi = __umulhi(a, M);
+#else
+    const u64 p = (u64)a * (u64)M;
+    const u32 lo = (u32)p, hi = (u32)(p >> 32);
+#endif
+    a = hi ^ b ^ K;
+    b = lo;
 }
 
 // F: fixed-key 64-bit bijection, rounds 6..11
