@@ -103,21 +103,37 @@ __device__ __forceinline__ u32 mulhi64_u32(u64 x, u32 d) {
 }
 __device__ __forceinline__ bool bern(u64 x, u64 thr) { return (x >> 11) < thr; }
 
-// fixed-point -ln: Q8.56 of -ln(U), U = M * 2^-(z+50). tQ/tA: 512-entry tables (shared memory)
+// Shared-memory reads by 32-bit shared-window address. Tables handed to device functions as generic pointers make the
+// compiler rebuild the window base (S2R + LEA) at every access; a plain address register does not.
+struct SmemTables {
+    u32 q, a;      // -ln tables: Q[512] u16, A[512] u64
+    u32 tg, g2;    // rounded-normal thresholds u32[<=1024], guide uint2[2048]
+};
+__device__ __forceinline__ u32 smem_addr(const void *p) {
+    u32 a = (u32)__cvta_generic_to_shared(p), r;
+    asm volatile("mov.u32 %0, %1;" : "=r"(r) : "r"(a));   // opaque: keep the address in a register, do not rebuild it per access
+    return r;
+}
+__device__ __forceinline__ u32 lds_u16(u32 addr) { u32 v; asm("ld.shared.u16 %0, [%1];" : "=r"(v) : "r"(addr)); return v; }
+__device__ __forceinline__ u32 lds_u32(u32 addr) { u32 v; asm("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr)); return v; }
+__device__ __forceinline__ u64 lds_u64(u32 addr) { u64 v; asm("ld.shared.u64 %0, [%1];" : "=l"(v) : "r"(addr)); return v; }
+__device__ __forceinline__ uint2 lds_v2(u32 addr) { uint2 v; asm("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(addr)); return v; }
+
+// fixed-point -ln: Q8.56 of -ln(U), U = M * 2^-(z+50). Tables: 512 entries in shared memory
 #define NS_LN2_56 49946518145322873ull
-__device__ __forceinline__ u64 neglog(u64 x, const unsigned short *__restrict__ tQ, const u64 *__restrict__ tA) {
+__device__ __forceinline__ u64 neglog(u64 x, const SmemTables &sm) {
     u32 z = (u32)__clzll((long long)x);         // 64 for x = 0
     u64 y = (z >= 64) ? 0ull : (x << z);
     u64 M = (y >> 14) | 1ull;
     u32 i = (u32)(y >> 54) & 511u;
-    u64 P = M * (u64)tQ[i];
+    u64 P = M * (u64)lds_u16(sm.q + 2u * i);
     u64 r = P & ((1ull << 61) - 1);
     u32 t = (u32)(r >> 21);
     u32 h1 = 0x55555555u - (t >> 10);
     u32 h2 = 0x80000000u - (__umulhi(t, h1) >> 8);
     u64 u = (u64)__umulhi(t, h2);
     u64 c = ((u64)t * u) >> 24;
-    u64 G = tA[i] + ((r >> 5) - c);
+    u64 G = lds_u64(sm.a + 8u * i) + ((r >> 5) - c);
     u64 Lz = (u64)(z + 1) * NS_LN2_56;
     return Lz > G ? Lz - G : 0ull;
 }

@@ -623,7 +623,8 @@ __global__ void debug_neglog_kernel(const u64 *x, u64 *out, u64 n) {
     for (u32 i = threadIdx.x; i < 512; i += blockDim.x) { sQ[i] = NEGLOG_Q_DEV[i]; sA[i] = NEGLOG_A_DEV[i]; }
     __syncthreads();
     u64 i = (u64)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) out[i] = neglog(x[i], sQ, sA);
+    SmemTables smt; smt.q = smem_addr(sQ); smt.a = smem_addr(sA); smt.tg = smt.g2 = 0;
+    if (i < n) out[i] = neglog(x[i], smt);
 }
 __global__ void debug_next_event_kernel(SeedKey key, const u32 *loc, const u32 *k, const i64 *f_last, const u32 *Cm, const u32 *sh, u32 *k_out,
                                         u32 *j_out, u64 *T_out, int *rc, u64 n) {
@@ -631,6 +632,7 @@ __global__ void debug_next_event_kernel(SeedKey key, const u32 *loc, const u32 *
     __shared__ u64 sA[512];
     for (u32 i = threadIdx.x; i < 512; i += blockDim.x) { sQ[i] = NEGLOG_Q_DEV[i]; sA[i] = NEGLOG_A_DEV[i]; }
     __syncthreads();
+    SmemTables smt; smt.q = smem_addr(sQ); smt.a = smem_addr(sA); smt.tg = smt.g2 = 0;
     u64 i = (u64)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     u32 kk = k[i];
@@ -641,7 +643,7 @@ __global__ void debug_next_event_kernel(SeedKey key, const u32 *loc, const u32 *
         bool crossed = false;
         for (;;) {
             j += 1; X += NS_GAMMA;
-            T += scale_exp(neglog(draw_time(X), sQ, sA), Cm[i], sh[i]);
+            T += scale_exp(neglog(draw_time(X), smt), Cm[i], sh[i]);
             if (T >= NS_TWO48) { crossed = true; break; }
             if ((i64)T > fl) { k_out[i] = kk; j_out[i] = j; T_out[i] = T; rc[i] = 0; return; }
         }
@@ -657,7 +659,7 @@ __global__ void debug_disperse_kernel(const ScenarioDev sc, SeedKey key, u64 thr
     __shared__ uint2 sG2[KIND == 3 ? NS_G2_LEN : 1];
     if (KIND == 3) gauss_stage(sc, sG, sG2);
     __syncthreads();
-    GaussLut gl; gl.tg = sG; gl.g2 = sG2; gl.R = sc.R;
+    GaussLut gl; gl.tg = smem_addr(sG); gl.g2 = smem_addr(sG2); gl.R = sc.R;
     u64 i = (u64)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     u32 cell = (KIND == 1) ? (loc[i] >= sc.J_local ? 1u : 0u) : cell_of_loc(sc, loc[i]);

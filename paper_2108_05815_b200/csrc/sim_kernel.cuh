@@ -29,25 +29,24 @@ __device__ __forceinline__ u32 lanemask_lt() {
 #define NS_G2_BITS 11
 #define NS_G2_LEN (1u << NS_G2_BITS)
 struct GaussLut {
-    const u32 *tg;
-    const uint2 *g2;
+    u32 tg, g2;    // shared-window addresses of the thresholds and the guide
     int R;
 };
-// exact for every u; `fast` = false when the rare forward scan was needed
+// exact for every u
 __device__ __forceinline__ int gauss_disp(const GaussLut &g, u32 u) {
-    const uint2 e = g.g2[u >> (32 - NS_G2_BITS)];
+    const uint2 e = lds_v2(g.g2 + 8u * (u >> (32 - NS_G2_BITS)));
     u32 pos = e.x & 0xFFFFu;
     if (e.x >> 16) {
         const u32 n = 2u * (u32)g.R;
-        while (pos < n && g.tg[pos] <= u) ++pos;
+        while (pos < n && lds_u32(g.tg + 4u * pos) <= u) ++pos;
     } else {
         pos += (e.y <= u) ? 1u : 0u;
     }
     return (int)pos - g.R;
 }
-// branch-free variant for speculative candidates: `exact` = false where the forward scan would be needed
+// branch-free variant: `exact` = false where the forward scan would be needed
 __device__ __forceinline__ int gauss_disp_fast(const GaussLut &g, u32 u, bool &exact) {
-    const uint2 e = g.g2[u >> (32 - NS_G2_BITS)];
+    const uint2 e = lds_v2(g.g2 + 8u * (u >> (32 - NS_G2_BITS)));
     exact = (e.x >> 16) == 0u;
     return (int)((e.x & 0xFFFFu) + ((e.y <= u) ? 1u : 0u)) - g.R;
 }
@@ -170,7 +169,8 @@ __global__ void __launch_bounds__(256) simulate_kernel(const ScenarioDev sc, con
     for (u32 i = threadIdx.x; i < 512; i += blockDim.x) { sQ[i] = NEGLOG_Q_DEV[i]; sA[i] = NEGLOG_A_DEV[i]; }
     if (KIND == 3) gauss_stage(sc, sG, sG2);
     __syncthreads();
-    GaussLut gl; gl.tg = sG; gl.g2 = sG2; gl.R = sc.R;
+    GaussLut gl; gl.tg = smem_addr(sG); gl.g2 = smem_addr(sG2); gl.R = sc.R;
+    SmemTables smt; smt.q = smem_addr(sQ); smt.a = smem_addr(sA); smt.tg = gl.tg; smt.g2 = gl.g2;
 
     const u32 lane = threadIdx.x & 31u;
     const bool lane_on = lane < ep.lanes_per_warp;
@@ -232,7 +232,7 @@ __global__ void __launch_bounds__(256) simulate_kernel(const ScenarioDev sc, con
             if (st == NS_ST_SEARCH) {
                 // S1b: one exponential draw of the event-time search
                 j += 1; X += NS_GAMMA;
-                T += scale_exp(neglog(draw_time(X), sQ, sA), Cm, sh);
+                T += scale_exp(neglog(draw_time(X), smt), Cm, sh);
                 if (T >= NS_TWO48) {                       // interval exhausted: cross and re-prime (L719, L727)
                     if (k == 0xFFFFFFFFu) { atomicMax(&bf.ctr->error, 3u); st = NS_ST_IDLE; }
                     else { k += 1; f_last = -1; need_prime = true; }

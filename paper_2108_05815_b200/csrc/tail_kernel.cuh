@@ -30,7 +30,8 @@ __global__ void __launch_bounds__(256) tail_kernel(const ScenarioDev sc, const S
     for (u32 i = threadIdx.x; i < 512; i += blockDim.x) { sQ[i] = NEGLOG_Q_DEV[i]; sA[i] = NEGLOG_A_DEV[i]; }
     if (KIND == 3) gauss_stage(sc, sG, sG2);
     __syncthreads();
-    GaussLut gl; gl.tg = sG; gl.g2 = sG2; gl.R = sc.R;
+    GaussLut gl; gl.tg = smem_addr(sG); gl.g2 = smem_addr(sG2); gl.R = sc.R;
+    SmemTables smt; smt.q = smem_addr(sQ); smt.a = smem_addr(sA); smt.tg = gl.tg; smt.g2 = gl.g2;
 
     const u32 lane = threadIdx.x & 31u, half = lane >> 4, sub = lane & 15u;
     const u32 jj = half ? 1u : sub + 1u;                               // ordinal of this lane's candidate point
@@ -83,7 +84,7 @@ __global__ void __launch_bounds__(256) tail_kernel(const ScenarioDev sc, const S
             const u64 kk64 = (u64)k + (half ? (u64)(1u + sub) : 0ull);
             const bool kvalid = kk64 < (u64)ep.k_stop;                // never look at or past the horizon
             u64 X = prime(ep.key, loc, (u32)kk64) + (u64)jj * NS_GAMMA;
-            const u64 T1 = scale_exp(neglog(draw_time(X), sQ, sA), Cm, sh);
+            const u64 T1 = scale_exp(neglog(draw_time(X), smt), Cm, sh);
             // partial sums over each 16-lane half (half 1 keeps its single draws: first points of fresh intervals)
             u64 T = T1;
 #pragma unroll
@@ -116,7 +117,7 @@ __global__ void __launch_bounds__(256) tail_kernel(const ScenarioDev sc, const S
                 bool found = false;
                 for (;;) {
                     jc += 1u; Xc += NS_GAMMA;
-                    Tc += scale_exp(neglog(draw_time(Xc), sQ, sA), Cm, sh);
+                    Tc += scale_exp(neglog(draw_time(Xc), smt), Cm, sh);
                     if (Tc >= NS_TWO48) break;
                     if ((i64)Tc > f_last) { found = true; break; }
                 }
