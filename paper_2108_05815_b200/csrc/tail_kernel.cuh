@@ -21,6 +21,22 @@ namespace necsim {
 #define NS_TAIL_ATTEMPTS 29u      // dispersal attempts evaluated per pass (lanes 3..31)
 
 
+// one level of the inclusive prefix sum over 16-lane segments: T += T of the lane `o` below, where that lane is in the
+// same segment (the shuffle's own predicate says so): 2 SHFL + 2 predicated adds
+__device__ __forceinline__ void seg16_scan_step(u32 &lo, u32 &hi, u32 o) {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        ".reg .b32 tl, th;\n\t"
+        "shfl.sync.up.b32 tl|p, %0, %2, 0x1000, 0xffffffff;\n\t"
+        "shfl.sync.up.b32 th, %1, %2, 0x1000, 0xffffffff;\n\t"
+        "@p add.cc.u32 %0, %0, tl;\n\t"
+        "@p addc.u32 %1, %1, th;\n\t"
+        "}"
+        : "+r"(lo), "+r"(hi)
+        : "r"(o));
+}
+
 template <int KIND, bool DEDUP, bool PERCELL>
 __global__ void __launch_bounds__(256) tail_kernel(const ScenarioDev sc, const SimBuffers bf, const EpochArgs ep) {
     __shared__ unsigned short sQ[512];
@@ -33,11 +49,15 @@ __global__ void __launch_bounds__(256) tail_kernel(const ScenarioDev sc, const S
     GaussLut gl; gl.tg = smem_addr(sG); gl.g2 = smem_addr(sG2); gl.R = sc.R;
     SmemTables smt; smt.q = smem_addr(sQ); smt.a = smem_addr(sA); smt.tg = gl.tg; smt.g2 = gl.g2;
 
-    const u32 lane = threadIdx.x & 31u, half = lane >> 4, sub = lane & 15u;
+    u32 lane;
+    asm volatile("mov.u32 %0, %%laneid;" : "=r"(lane));                // opaque: kept in a register, not re-read per use
+    const u32 half = lane >> 4, sub = lane & 15u;
     const u32 jj = half ? 1u : sub + 1u;                               // ordinal of this lane's candidate point
+    const u64 cand_add = (u64)jj * NS_GAMMA;                           // stream position of the candidate: s + jj * GAMMA
     // event draws, one per lane: draw = F((X ^ lane_xor) + lane_add)
     const u64 lane_xor = lane == 0 ? NS_L_SPEC : lane == 1 ? NS_L_INDEX : lane == 2 ? NS_L_MIGR : NS_L_DISP;
     const u32 att_lane = lane >= 3u ? lane - 3u : 0u;                  // dispersal attempt of this lane within a pass
+    const u64 att_add = (u64)att_lane * NS_GAMMA;
     unsigned long long c_events = 0, c_culled = 0, c_resamples = 0;   // warp-uniform
 
     for (;;) {
@@ -83,16 +103,13 @@ __global__ void __launch_bounds__(256) tail_kernel(const ScenarioDev sc, const S
             // ---- S1: candidate points of the event-time search ---------------------------------------------------
             const u64 kk64 = (u64)k + (half ? (u64)(1u + sub) : 0ull);
             const bool kvalid = kk64 < (u64)ep.k_stop;                // never look at or past the horizon
-            u64 X = prime(ep.key, loc, (u32)kk64) + (u64)jj * NS_GAMMA;
+            u64 X = prime(ep.key, loc, (u32)kk64) + cand_add;
             const u64 T1 = scale_exp(neglog(draw_time(X), smt), Cm, sh);
             // partial sums over each 16-lane half (half 1 keeps its single draws: first points of fresh intervals)
-            u64 T = T1;
-#pragma unroll
-            for (int o = 1; o < 16; o <<= 1) {
-                const u64 t = __shfl_up_sync(NS_FULL, T, o, 16);
-                if ((int)sub >= o) T += t;
-            }
-            if (half) T = T1;
+            u32 t_lo = (u32)T1, t_hi = (u32)(T1 >> 32);
+            seg16_scan_step(t_lo, t_hi, 1); seg16_scan_step(t_lo, t_hi, 2);
+            seg16_scan_step(t_lo, t_hi, 4); seg16_scan_step(t_lo, t_hi, 8);
+            const u64 T = half ? T1 : (((u64)t_hi << 32) | t_lo);
             const bool inside = T < NS_TWO48;
             const u32 evm = __ballot_sync(NS_FULL, inside && (half ? kvalid : ((i64)T > f_last)));
             const u32 crm = __ballot_sync(NS_FULL, !inside);
@@ -140,7 +157,7 @@ __global__ void __launch_bounds__(256) tail_kernel(const ScenarioDev sc, const S
             if (!probes) { steps++; c_events++; }
             // S2 + S3: all draws of the event in one hash evaluation across the lanes
             const u64 xb = Xe ^ lane_xor;
-            u64 u = hashF(xb + (u64)att_lane * NS_GAMMA);
+            u64 u = hashF(xb + att_add);
             const bool can_speciate = !(KIND == 1 && cell == 0);      // local community of the implicit model: nu = 0 (L1830)
             const u32 bm = __ballot_sync(NS_FULL, bern(u, lane == 2 ? ep.thr_m : ep.thr_nu));
             const bool speciates = can_speciate && (bm & 1u);
@@ -170,8 +187,11 @@ __global__ void __launch_bounds__(256) tail_kernel(const ScenarioDev sc, const S
                         u32 c2 = 0, d = 0, pf = 0;
                         uint2 cs = make_uint2(Cm, sh);
                         if (lane >= 3u) {   // attempt r0 + lane - 3 (R16: redraw the whole (dx, dy) pair)
-                            const u32 xx = wrap_add(x0, gauss_disp(gl, (u32)(u >> 32)), sc.width);
-                            const u32 yy = wrap_add(y0, gauss_disp(gl, (u32)u), sc.height);
+                            bool e1, e2;
+                            int dx = gauss_disp_fast(gl, (u32)(u >> 32), e1), dy = gauss_disp_fast(gl, (u32)u, e2);
+                            if (!(e1 && e2)) { dx = gauss_disp(gl, (u32)(u >> 32)); dy = gauss_disp(gl, (u32)u); }   // rare: crowded tail buckets
+                            const u32 xx = wrap_add(x0, dx, sc.width);
+                            const u32 yy = wrap_add(y0, dy, sc.height);
                             const u32 ci = yy * sc.width + xx;
                             c2 = (yy << 16) | xx;
                             d = cell_deme(sc, ci);
@@ -189,7 +209,7 @@ __global__ void __launch_bounds__(256) tail_kernel(const ScenarioDev sc, const S
                             ok = true;
                             break;
                         }
-                        u = hashF(xb + (u64)(r0 + NS_TAIL_ATTEMPTS + att_lane) * NS_GAMMA);   // next 29 attempts
+                        u = hashF(xb + att_add + (u64)(r0 + NS_TAIL_ATTEMPTS) * NS_GAMMA);   // next 29 attempts
                     }
                 }
             }
