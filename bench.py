@@ -202,7 +202,10 @@ def main():
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))) if os.path.exists(os.path.join(ROOT, "MEASURED_PEAKS.json")) else {}
         sm_max = float(peaks.get("sm_max_mhz", clocks.get("sm_max_mhz") or 1965.0))
         peak = alu_peak(prop.multi_processor_count, sm_max)
-        achieved = (ev / K) * I_EVENT[name] / ((sim_ms / K) * 1e-3)   # per step: all simulate-kernel launches of one step
+        # dominant kernel of a step = tail_kernel (95.7 % of the step in the ncu launch list, profiles/r1_launches_c5.md):
+        # algorithmic instructions of its launches / their summed device time (CUDA events around every launch)
+        dom_ms, dom_ev, dom_name = (tail_ms, ev_tail, "tail_kernel") if tail_ms >= sim_ms - tail_ms else (sim_ms - tail_ms, ev - ev_tail, "simulate_kernel")
+        achieved = dom_ev * I_EVENT[name] / max(dom_ms * 1e-3, 1e-12)
         int_meas = {k: ns.int_peak(i, 2048)[0] for i, k in enumerate(("hash_round_mix", "imad_only", "alu_only"))}
         # MODE-T: the saturated workload (dedup off, every lineage advanced 200 events): where the ALU roofline is meaningful
         rt = sc.simulate_raw(seed, cfg["nu"], d_mask, n_s, ns.make_params(dedup=False, max_steps=200))
@@ -222,12 +225,19 @@ def main():
                                          "events_per_step": (ev - ev_tail) / K, "kernel": "simulate_kernel (one lineage per lane)"},
                            "tail": {"events_per_s": ev_tail / max(tail_ms * 1e-3, 1e-9), "ms_per_step": tail_ms / K, "events_per_step": ev_tail / K,
                                     "kernel": "tail_kernel (one lineage per warp; bound by event latency x chain length, DESIGN.md 6.3)"}},
-                "roofline": {"bound": "alu", "kernel": "simulate_kernel + tail_kernel (all epochs of a step)", "achieved": achieved / 1e12, "peak": peak / 1e12,
-                             "unit": "Tinstr/s", "frac": achieved / peak, "traffic": None, "instr_per_event": I_EVENT[name],
+                "roofline": {"bound": "alu", "kernel": dom_name + " (all its launches of the timed steps)", "achieved": achieved / 1e12, "peak": peak / 1e12,
+                             "unit": "Tinstr/s", "frac": achieved / peak,
+                             # dram__bytes_read.sum + dram__bytes_write.sum of one tail_kernel launch (C5, 61st tail epoch), ncu --set full,
+                             # profiles/r1_ncu_tail_kernel_c5.md; caches are flushed per ncu replay pass, so this is an upper bound
+                             "traffic": 67198464 if (name == "c5" and dom_name == "tail_kernel") else None,
+                             "instr_per_event": I_EVENT[name],
+                             "note": "latency-bound by construction: one lineage per warp walks a serial chain of ~ln(S)/nu events (DESIGN.md 6.3)",
                              "peak_source": "derived: SMs x 4 schedulers x 32 lanes x sm_max_mhz (DESIGN.md section 6)",
                              "measured_int_peaks_Tinstr_s": {k: v / 1e12 for k, v in int_meas.items()}},
                 "mode_t": {"value": mode_t, "unit": UNIT, "what": "dedup off, 200 events per lineage, saturated machine",
-                           "roofline_frac": mode_t * I_EVENT[name] / peak}}
+                           "roofline_frac": mode_t * I_EVENT[name] / peak,
+                           "ncu": "profiles/r1_ncu_simulate_kernel_c5_modeT.md: issue slots 71 % active, ALU pipe 65 %, FMA pipe 18 % of peak, "
+                                  "22.2 of 32 lanes per instruction, L2 hit 98.5 %"}}
         if not args.no_cpu_baseline and world == 1:
             v, dt, n_ev, desc = run_oracle_sample(cfg, name)
             line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc, "seconds": dt}
