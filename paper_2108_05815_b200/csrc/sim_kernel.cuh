@@ -173,7 +173,7 @@ __global__ void __launch_bounds__(256) simulate_kernel(const ScenarioDev sc, con
     SmemTables smt; smt.q = smem_addr(sQ); smt.a = smem_addr(sA); smt.tg = gl.tg; smt.g2 = gl.g2;
 
     const u32 lane = threadIdx.x & 31u;
-    const bool lane_on = lane < ep.lanes_per_warp;
+    const u32 on_mask = ep.lanes_per_warp >= 32u ? 0xFFFFFFFFu : ((1u << ep.lanes_per_warp) - 1u);   // lanes that hold lineages
 
     // lineage state (registers)
     u32 st = NS_ST_IDLE, att = 0;
@@ -185,12 +185,14 @@ __global__ void __launch_bounds__(256) simulate_kernel(const ScenarioDev sc, con
 
     for (;;) {
         // ---- S4: refill idle lanes from the device work queue (one atomic per warp) -----------------
-        const u32 need = __ballot_sync(NS_FULL, lane_on && st == NS_ST_IDLE);
+        u32 bs = __ballot_sync(NS_FULL, st == NS_ST_SEARCH);
+        const u32 be = __ballot_sync(NS_FULL, st == NS_ST_EVENT);
+        const u32 need = on_mask & ~(bs | be);                 // idle lanes that may hold a lineage
         if (need != 0u && !exhausted) {
             u32 cnt = __popc(need), base = 0;
             if (lane == 0) base = atomicAdd(&bf.ctr->q_head, cnt);
             base = __shfl_sync(NS_FULL, base, 0);
-            if (lane_on && st == NS_ST_IDLE) {
+            if ((need >> lane) & 1u) {
                 u32 idx = base + __popc(need & lanemask_lt());
                 if (idx < bf.q_in_count) {
                     uint4 e = bf.q_in[idx];
@@ -199,9 +201,9 @@ __global__ void __launch_bounds__(256) simulate_kernel(const ScenarioDev sc, con
                 }
             }
             exhausted = (base + cnt >= bf.q_in_count);
+            bs = __ballot_sync(NS_FULL, st == NS_ST_SEARCH);
         }
-        const u32 n_search = __popc(__ballot_sync(NS_FULL, st == NS_ST_SEARCH));
-        const u32 n_event = __popc(__ballot_sync(NS_FULL, st == NS_ST_EVENT));
+        const u32 n_search = __popc(bs), n_event = __popc(be);
         if ((n_search | n_event) == 0u) break;
 
         if (n_event <= n_search) {
