@@ -460,11 +460,15 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
     uint4 *q_in = qa, *q_out = qb;
     float ms_sim = 0.f, ms_tail = 0.f;
     u64 n_epochs = 0, n_tail_epochs = 0, ev_before = 0, ev_tail = 0;
+    const bool params_default_epoch = !(params && params->epoch_events);
     while (active > 0) {
         u32 k_stop;
         if (rp.epoch_events == 0) k_stop = 0xFFFFFFFFu;
         else {
-            double span = (double)rp.epoch_events / ((double)active * scn->mu_max);
+            // tail epochs are latency-bound and their warps stay roughly synchronous in simulated time: longer epochs cost
+            // no dedup hits and amortise the end-of-epoch imbalance (spread of events per lineage ~ 1/sqrt(span))
+            const double w = (double)rp.epoch_events * ((active <= tail_threshold && params_default_epoch) ? 8.0 : 1.0);
+            double span = w / ((double)active * scn->mu_max);
             u64 sp = span < 1.0 ? 1ull : (span > 1e9 ? 1000000000ull : (u64)span);
             u64 h = (u64)k_start + sp;
             k_stop = h >= 0xFFFFFFFFull ? 0xFFFFFFFFu : (u32)h;
