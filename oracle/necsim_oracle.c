@@ -153,6 +153,57 @@ int orc_next_event(const u32 K[6], u32 loc, u32 *k, i64 f_last, u32 Cm, u32 sh, 
 }
 
 /* ------------------------------------------------------------------------------------------- */
+/* Poisson / order-statistics event-time sampler (paper 5.2.3 L733-741, C.5 L1940-1954) */
+/* ------------------------------------------------------------------------------------------- */
+#define L_COUNT 0x9b05688c2b3e6c1full /* frac sqrt 13 */
+#define L_THIN 0x1f83d9abfb41bd6bull  /* frac sqrt 17 */
+#define ORC_NMAX 256
+/* PC[n] = min(floor(P(N <= n) * 2^64), 2^64 - 1), N ~ Poisson(mu): pmf recurrence in binary64 (libm exp) */
+void orc_poisson_table(double mu, u64 *PC) {
+    double p = exp(-mu), cdf = 0.0;
+    for (int n = 0; n < ORC_NMAX; ++n) {
+        if (n > 0) p = p * mu / (double)n;
+        cdf = cdf + p;
+        PC[n] = (cdf >= 1.0) ? 0xFFFFFFFFFFFFFFFFull : (u64)ldexp(cdf, 64);   /* cdf < 1: ldexp exact, conversion truncates */
+    }
+}
+/* number of points of the rate-mu_max stream of (loc, k): N = #{n : c >= PC[n]}, c = F(s ^ L_COUNT) */
+u32 orc_poisson_count(const u64 *PC, u64 s) {
+    u64 c = orc_F(s ^ L_COUNT);
+    u32 n = 0;
+    for (int i = 0; i < ORC_NMAX; ++i) if (c >= PC[i]) ++n;
+    return n;
+}
+/* thinning threshold of a cell: point i survives iff thin == 2^32-1 or lo32(F(X_i ^ L_THIN)) < thin */
+u32 orc_thin_threshold(double mu_cell, double mu_max) {
+    if (mu_cell >= mu_max) return 0xFFFFFFFFu;
+    double v = floor((mu_cell / mu_max) * 4294967296.0);
+    return (v >= 4294967295.0) ? 0xFFFFFFFFu : (u32)v;
+}
+/* next point of loc's stream strictly after (k, f_last): all N points of an interval are uniform offsets (order
+ * statistics of a Poisson process, L735-741); the next event is the surviving point with the smallest (f, i), f > f_last.
+ * Same contract as orc_next_event. */
+int orc_next_event_poisson(const u32 K[6], const u64 *PC, u32 thin, u32 loc, u32 *k, i64 f_last, u32 k_stop,
+                           u32 *j_out, u64 *T_out, u64 *s_out) {
+    for (;;) {
+        if (*k == k_stop) return 1;
+        u64 s = orc_prime(K, loc, *k);
+        u32 N = orc_poisson_count(PC, s);
+        u32 best_i = 0; u64 best_f = 0;
+        for (u32 i = 1; i <= N; ++i) {
+            u64 X = s + (u64)i * GAMMA;
+            u64 f = orc_F(X) >> 16;                                      /* Q0.48 offset in units of delta_t */
+            if (thin != 0xFFFFFFFFu && (u32)orc_F(X ^ L_THIN) >= thin) continue;   /* thinned out (rate lambda_cell < lambda_max) */
+            if ((i64)f <= f_last) continue;                              /* strictly later (L729) */
+            if (best_i == 0 || f < best_f) { best_i = i; best_f = f; }   /* ties: smallest i */
+        }
+        if (best_i) { *j_out = best_i; *T_out = best_f; *s_out = s; return 0; }
+        if (*k == 0xFFFFFFFFu) return -2;
+        *k += 1; f_last = -1;
+    }
+}
+
+/* ------------------------------------------------------------------------------------------- */
 /* dispersal tables                                                             */
 /* ------------------------------------------------------------------------------------------- */
 /* rounded-normal thresholds (R15; paper L1216 "discretised normal distribution"). TG has 2R entries. */
@@ -221,13 +272,16 @@ typedef struct orc_scenario {
     /* gaussian */
     double sigma; int R; u32 *TG;
     double delta_t;
+    int sampler;         /* 0 exponential (2.4), 1 Poisson / order statistics (2.7) */
+    u64 *PC; u32 *thin;  /* Poisson: cdf thresholds of mu_max; per-cell thinning threshold */
+    double mu_max; double *lam; /* lambda per cell (as given) */
 } orc_scenario;
 
 static void set_err(char *err, int errlen, const char *msg) { if (err && errlen > 0) { strncpy(err, msg, (size_t)errlen - 1); err[errlen - 1] = 0; } }
 
 void orc_scenario_destroy(orc_scenario *sc) {
     if (!sc) return;
-    free(sc->deme); free(sc->prefix); free(sc->Cm); free(sc->sh); free(sc->thresh); free(sc->alias); free(sc->TG);
+    free(sc->deme); free(sc->prefix); free(sc->Cm); free(sc->sh); free(sc->thresh); free(sc->alias); free(sc->TG); free(sc->PC); free(sc->thin); free(sc->lam);
     free(sc);
 }
 
@@ -253,6 +307,7 @@ orc_scenario *orc_scenario_create(int kind, u32 width, u32 height, const u32 *de
     u32 n = sc->ncells;
     sc->deme = (u32 *)malloc(sizeof(u32) * n); sc->prefix = (u32 *)malloc(sizeof(u32) * ((size_t)n + 1));
     sc->Cm = (u32 *)malloc(sizeof(u32) * n); sc->sh = (u32 *)malloc(sizeof(u32) * n);
+    sc->lam = (double *)calloc(n, sizeof(double));
     u64 tot = 0;
     for (u32 c = 0; c < n; ++c) {
         u32 d;
@@ -260,6 +315,7 @@ orc_scenario *orc_scenario_create(int kind, u32 width, u32 height, const u32 *de
         else d = deme ? deme[c] : uniform_deme;
         sc->deme[c] = d; sc->prefix[c] = (u32)tot; tot += d;
         double lam = (turnover && kind != ORC_SPATIALLY_IMPLICIT) ? turnover[c] : uniform_turnover;
+        sc->lam[c] = lam;
         if (d > 0 || !turnover) {
             if (orc_turnover_scale(lam, delta_t, &sc->Cm[c], &sc->sh[c]) != 0) { set_err(err, errlen, "turnover*delta_t out of range"); orc_scenario_destroy(sc); return NULL; }
         } else { sc->Cm[c] = 0; sc->sh[c] = 0; }
@@ -289,6 +345,23 @@ orc_scenario *orc_scenario_create(int kind, u32 width, u32 height, const u32 *de
 }
 
 u64 orc_scenario_num_individuals(const orc_scenario *sc) { return sc->n_sampleable; }
+/* chooses the event-time sampler (DESIGN.md 2.4 / 2.7). Results depend on it: same law, different realisation. */
+int orc_scenario_set_sampler(orc_scenario *sc, int sampler) {
+    if (sampler != 0 && sampler != 1) return -1;
+    sc->sampler = sampler;
+    if (sampler == 1 && !sc->PC) {
+        double mu_max = 0.0;
+        for (u32 c = 0; c < sc->ncells; ++c) if (sc->deme[c]) { double mu = sc->lam[c] * sc->delta_t; if (mu > mu_max) mu_max = mu; }
+        sc->mu_max = mu_max;
+        sc->PC = (u64 *)malloc(sizeof(u64) * ORC_NMAX);
+        orc_poisson_table(mu_max, sc->PC);
+        sc->thin = (u32 *)malloc(sizeof(u32) * sc->ncells);
+        for (u32 c = 0; c < sc->ncells; ++c) sc->thin[c] = sc->deme[c] ? orc_thin_threshold(sc->lam[c] * sc->delta_t, mu_max) : 0u;
+    }
+    return 0;
+}
+const u64 *orc_scenario_poisson(const orc_scenario *sc, double *mu_max) { *mu_max = sc->mu_max; return sc->PC; }
+u32 orc_scenario_thin(const orc_scenario *sc, u32 cell) { return sc->thin ? sc->thin[cell] : 0xFFFFFFFFu; }
 const u32 *orc_scenario_thresh(const orc_scenario *sc) { return sc->thresh; }
 const u32 *orc_scenario_alias(const orc_scenario *sc) { return sc->alias; }
 const u32 *orc_scenario_gauss(const orc_scenario *sc, int *R) { *R = sc->R; return sc->TG; }
@@ -460,7 +533,9 @@ int orc_simulate(const orc_scenario *sc, u64 seed, double nu, const uint8_t *mas
             if (state[id] != 0) continue;
             for (;;) {
                 u32 j; u64 T, s;
-                int r = orc_next_event(K, loc[id], &kk[id], ff[id], sc->Cm[cell[id]], sc->sh[cell[id]], k_stop, &j, &T, &s);
+                int r = sc->sampler == 1
+                    ? orc_next_event_poisson(K, sc->PC, sc->thin[cell[id]], loc[id], &kk[id], ff[id], k_stop, &j, &T, &s)
+                    : orc_next_event(K, loc[id], &kk[id], ff[id], sc->Cm[cell[id]], sc->sh[cell[id]], k_stop, &j, &T, &s);
                 if (r == 1) { ff[id] = -1; break; }          /* reached the horizon: pause (fresh at k_stop) */
                 if (r < 0) { rc = r; break; }
                 /* event (loc, k, j) at offset T */
@@ -553,6 +628,16 @@ void orc_batch_next_event(u64 seed, const u32 *loc, const u32 *k, const i64 *f_l
     for (u64 i = 0; i < n; ++i) {
         u32 kk = k[i]; u64 s;
         rc[i] = orc_next_event(K, loc[i], &kk, f_last[i], Cm[i], sh[i], 0xFFFFFFFFu, &j_out[i], &T_out[i], &s);
+        k_out[i] = kk;
+    }
+}
+/* Poisson sampler: rc[i] as orc_next_event_poisson with the scenario's table and the thinning threshold of cell[i] */
+void orc_batch_next_event_poisson(const orc_scenario *sc, u64 seed, const u32 *loc, const u32 *cell, const u32 *k, const i64 *f_last,
+                                  u32 *k_out, u32 *j_out, u64 *T_out, int *rc, u64 n) {
+    u32 K[6]; orc_key_schedule(seed, K);
+    for (u64 i = 0; i < n; ++i) {
+        u32 kk = k[i]; u64 s;
+        rc[i] = orc_next_event_poisson(K, sc->PC, sc->thin[cell[i]], loc[i], &kk, f_last[i], 0xFFFFFFFFu, &j_out[i], &T_out[i], &s);
         k_out[i] = kk;
     }
 }

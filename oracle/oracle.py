@@ -116,7 +116,7 @@ class Scenario:
     """Mirror of the paper's scenario = habitat + turnover + dispersal (+ sizes)."""
 
     def __init__(self, kind, width=1, height=1, deme=None, uniform_deme=0, turnover=None, uniform_turnover=1.0,
-                 matrix=None, sigma=0.0, local_size=0, meta_size=0, migration=0.0, delta_t=2.0):
+                 matrix=None, sigma=0.0, local_size=0, meta_size=0, migration=0.0, delta_t=2.0, sampler=0):
         self.kind = kind
         d = None if deme is None else np.ascontiguousarray(deme, dtype=np.uint32).ravel()
         t = None if turnover is None else np.ascontiguousarray(turnover, dtype=np.float64).ravel()
@@ -127,6 +127,10 @@ class Scenario:
                                             float(delta_t), err, 256)
         if not self._h:
             raise ValueError("oracle scenario: " + err.value.decode())
+        L = lib(); L.orc_scenario_set_sampler.restype = C.c_int; L.orc_scenario_set_sampler.argtypes = [C.c_void_p, C.c_int]
+        if L.orc_scenario_set_sampler(self._h, int(sampler)) != 0:
+            raise ValueError("oracle scenario: unknown sampler")
+        self.sampler = int(sampler)
         self.delta_t = float(delta_t)
         self.ncells = 2 if kind == SPATIALLY_IMPLICIT else width * height
 
@@ -142,6 +146,26 @@ class Scenario:
         th = np.ctypeslib.as_array(C.cast(lib().orc_scenario_thresh(self._h), C.POINTER(C.c_uint32)), shape=(n, n)).copy()
         al = np.ctypeslib.as_array(C.cast(lib().orc_scenario_alias(self._h), C.POINTER(C.c_uint32)), shape=(n, n)).copy()
         return th, al
+
+    def poisson_table(self):
+        """(mu_max, PC[256]) of the Poisson sampler."""
+        L = lib(); L.orc_scenario_poisson.restype = C.c_void_p; L.orc_scenario_poisson.argtypes = [C.c_void_p, C.c_void_p]
+        mu = C.c_double(); p = L.orc_scenario_poisson(self._h, C.byref(mu))
+        return mu.value, np.ctypeslib.as_array(C.cast(p, C.POINTER(C.c_uint64)), shape=(256,)).copy()
+
+    def thin(self, cell):
+        L = lib(); L.orc_scenario_thin.restype = C.c_uint32; L.orc_scenario_thin.argtypes = [C.c_void_p, C.c_uint32]
+        return L.orc_scenario_thin(self._h, int(cell))
+
+    def batch_next_event_poisson(self, seed, loc, cell, k, f_last):
+        loc = np.ascontiguousarray(loc, dtype=np.uint32); n = len(loc)
+        cell = _u32(cell, n); k = _u32(k, n)
+        f_last = np.ascontiguousarray(np.broadcast_to(np.asarray(f_last, dtype=np.int64), (n,)))
+        ko = np.zeros(n, np.uint32); jo = np.zeros(n, np.uint32); To = np.zeros(n, np.uint64); rc = np.zeros(n, np.int32)
+        L = lib(); L.orc_batch_next_event_poisson.restype = None
+        L.orc_batch_next_event_poisson.argtypes = [C.c_void_p, C.c_uint64] + [C.c_void_p] * 8 + [C.c_uint64]
+        L.orc_batch_next_event_poisson(self._h, int(seed), _ptr(loc), _ptr(cell), _ptr(k), _ptr(f_last), _ptr(ko), _ptr(jo), _ptr(To), _ptr(rc), n)
+        return ko, jo, To, rc
 
     def disperse(self, seed, loc, k, j):
         out = C.c_uint32()

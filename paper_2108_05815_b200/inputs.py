@@ -8,7 +8,7 @@ of the method (no hashing, no sampling of events): only numpy recipes that produ
 Every config is a plain dict:
   kind, width, height, deme (u32[ncells] or None), uniform_deme, turnover (f64[ncells] or None),
   uniform_turnover, matrix (f64[ncells, ncells] or None), sigma, local_size, meta_size, migration,
-  delta_t, nu, seed, mask (u8[n_individuals] or None), name
+  delta_t, sampler (0 exponential, 1 Poisson event-time sampler), nu, seed, mask (u8[n_individuals] or None), name
 """
 import math
 import numpy as np
@@ -19,7 +19,7 @@ NONSPATIAL, SPATIALLY_IMPLICIT, EXPLICIT_MATRIX, EXPLICIT_GAUSSIAN = 0, 1, 2, 3
 def _base(name, kind, **kw):
     cfg = dict(name=name, kind=kind, width=1, height=1, deme=None, uniform_deme=0, turnover=None,
                uniform_turnover=1.0, matrix=None, sigma=0.0, local_size=0, meta_size=0, migration=0.0,
-               delta_t=2.0, nu=1e-3, seed=42, mask=None)
+               delta_t=2.0, nu=1e-3, seed=42, mask=None, sampler=0)
     cfg.update(kw)
     return cfg
 
@@ -121,7 +121,7 @@ def n_sampled(cfg):
 
 
 SCENARIO_KEYS = ("kind", "width", "height", "deme", "uniform_deme", "turnover", "uniform_turnover", "matrix",
-                 "sigma", "local_size", "meta_size", "migration", "delta_t")
+                 "sigma", "local_size", "meta_size", "migration", "delta_t", "sampler")
 
 
 def scenario_kwargs(cfg):
