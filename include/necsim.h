@@ -48,6 +48,8 @@ extern "C" {
 typedef struct necsim_scenario_desc {
     int32_t kind;             /* NECSIM_NONSPATIAL .. NECSIM_EXPLICIT_GAUSSIAN */
     uint32_t width, height;   /* NONSPATIAL: 1x1. SPATIALLY_IMPLICIT: ignored */
+    uint32_t sampler;         /* event-time sampler: 0 = exponential, 1 = Poisson / order
+                                 statistics (L733-741). Same law, different realisation */
     const uint32_t *deme;     /* HOST [width*height] deme size per cell, 0 = not habitat; NULL = uniform_deme */
     uint32_t uniform_deme;
     const double *turnover;   /* HOST [width*height] lambda per cell (> 0, finite; read for habitat cells); NULL = uniform */
@@ -186,6 +188,12 @@ int necsim_debug_disperse(const necsim_scenario *scn, uint64_t seed, const uint3
  * [ncells*ncells], rounded-normal thresholds [2R] (*R_out = R), per-cell turnover scale Cm/sh [ncells] */
 int necsim_debug_tables(const necsim_scenario *scn, uint32_t *h_thresh, uint32_t *h_alias, uint32_t *h_gauss, int32_t *R_out,
                         uint32_t *h_Cm, uint32_t *h_sh, void *cuda_stream);
+/* Poisson sampler: event-time search over arrays; d_cell[i] = cell of d_loc[i] (thinning threshold) */
+int necsim_debug_next_event_poisson(const necsim_scenario *scn, uint64_t seed, const uint32_t *d_loc, const uint32_t *d_cell, const uint32_t *d_k,
+                                    const int64_t *d_f_last, uint32_t *d_k_out, uint32_t *d_j_out, uint64_t *d_T_out, int32_t *d_rc, uint64_t n,
+                                    void *cuda_stream);
+/* copies the Poisson cdf thresholds PC[256] and the per-cell thinning thresholds [ncells] to HOST (any may be NULL) */
+int necsim_debug_poisson_table(const necsim_scenario *scn, uint64_t *h_pc, uint32_t *h_thin, double *mu_max, void *cuda_stream);
 /* integer-pipe peak micro-benchmark: runs `iters` iterations of an unrolled chain of
  * independent IMAD.WIDE / LOP3 / SHF / IADD3 on every SM; kind 0 = mixed hash-like, 1 = IMAD only,
  * 2 = ALU (LOP3/SHF/IADD3) only. Returns thread-level integer instructions per second. */

@@ -36,7 +36,10 @@ typedef int64_t i64;
 #define NS_L_DISP 0x3c6ef372fe94f82bull
 #define NS_L_INDEX 0xa54ff53a5f1d36f1ull
 #define NS_L_MIGR 0x510e527fade682d1ull
+#define NS_L_COUNT 0x9b05688c2b3e6c1full
+#define NS_L_THIN 0x1f83d9abfb41bd6bull
 #define NS_TWO48 (1ull << 48)
+#define NS_POIS_N 256u
 
 // one Feistel round: p = a*M; (a, b) <- (hi32(p) ^ b ^ K, lo32(p))   [1 IMAD.WIDE.U32 + 1 LOP3]
 __host__ __device__ __forceinline__ void feistel(u32 &a, u32 &b, u32 M, u32 K) {
@@ -108,6 +111,7 @@ __device__ __forceinline__ bool bern(u64 x, u64 thr) { return (x >> 11) < thr; }
 struct SmemTables {
     u32 q, a;      // -ln tables: Q[512] u16, A[512] u64
     u32 tg, g2;    // rounded-normal thresholds u32[<=1024], guide uint2[2048]
+    u32 pc, pg;    // Poisson cdf thresholds u64[256], guide u16[256] on the top byte of the draw
 };
 __device__ __forceinline__ u32 smem_addr(const void *p) {
     u32 a = (u32)__cvta_generic_to_shared(p), r;
@@ -137,6 +141,18 @@ __device__ __forceinline__ u64 neglog(u64 x, const SmemTables &sm) {
     u64 Lz = (u64)(z + 1) * NS_LN2_56;
     return Lz > G ? Lz - G : 0ull;
 }
+
+// Poisson sampler: N = #{n : c >= PC[n]}, c = F(s ^ L_COUNT). pg[b] = #{n : PC[n] < b << 56} starts a short
+// forward scan over the non-decreasing thresholds.
+__device__ __forceinline__ u32 poisson_count(u64 s, const SmemTables &sm) {
+    const u64 c = hashF(s ^ NS_L_COUNT);
+    u32 n = lds_u16(sm.pg + 2u * (u32)(c >> 56));
+    while (n < NS_POIS_N && lds_u64(sm.pc + 8u * n) <= c) ++n;
+    return n;
+}
+// offset of point X and whether it exists for a cell with thinning threshold `thin`
+__device__ __forceinline__ u64 poisson_offset(u64 X) { return hashF(X) >> 16; }
+__device__ __forceinline__ bool poisson_kept(u64 X, u32 thin) { return thin == 0xFFFFFFFFu || (u32)hashF(X ^ NS_L_THIN) < thin; }
 
 // E / mu in Q16.48: bits of the exact 96-bit product E * Cm
 __device__ __forceinline__ u64 scale_exp(u64 E, u32 Cm, u32 sh) {

@@ -107,7 +107,7 @@ struct necsim_scenario {
 };
 
 struct ScenarioLayout {
-    size_t off_hab8, off_deme32, off_prefix, off_scale, off_alias, off_gauss, total;
+    size_t off_hab8, off_deme32, off_prefix, off_pois, off_thin, off_scale, off_alias, off_gauss, total;
     u32 ncells, gauss_len;
     int R;
     bool uniform_deme, need_deme32, per_cell_turnover;
@@ -117,11 +117,12 @@ static int scenario_layout(const necsim_scenario_desc *d, ScenarioLayout &L) {
     if (!d) return fail(NECSIM_ERR_INVALID_ARG, "desc is NULL");
     memset(&L, 0, sizeof(L));
     if (d->kind < 0 || d->kind > 3) return fail(NECSIM_ERR_INVALID_ARG, "unknown scenario kind");
+    if (d->sampler > 1) return fail(NECSIM_ERR_INVALID_ARG, "unknown event-time sampler");
     if (!(d->delta_t > 0.0) || !std::isfinite(d->delta_t)) return fail(NECSIM_ERR_INVALID_ARG, "delta_t must be > 0 and finite");
     if (d->kind == NECSIM_SPATIALLY_IMPLICIT) {
         if (d->local_size == 0 || d->meta_size == 0 || d->local_size + d->meta_size >= (1ull << 32) || !(d->migration >= 0.0 && d->migration <= 1.0))
             return fail(NECSIM_ERR_INVALID_ARG, "implicit: bad sizes or migration");
-        L.ncells = 2; L.uniform_deme = false; L.total = 256;
+        L.ncells = 2; L.uniform_deme = false; L.off_pois = 0; L.total = d->sampler ? align256(8 * NS_POIS_N) : 256;
         return NECSIM_OK;
     }
     if (d->width == 0 || d->height == 0 || (u64)d->width * d->height >= (1ull << 32)) return fail(NECSIM_ERR_INVALID_ARG, "bad width/height");
@@ -139,6 +140,10 @@ static int scenario_layout(const necsim_scenario_desc *d, ScenarioLayout &L) {
         L.off_prefix = off; off = align256(off + 4 * ((size_t)L.ncells + 1));
     }
     if (L.per_cell_turnover) { L.off_scale = off; off = align256(off + 8 * (size_t)L.ncells); }
+    if (d->sampler) {
+        L.off_pois = off; off = align256(off + 8 * NS_POIS_N);
+        if (L.per_cell_turnover) { L.off_thin = off; off = align256(off + 4 * (size_t)L.ncells); }
+    }
     if (d->kind == NECSIM_EXPLICIT_MATRIX) {
         if (!d->dispersal_matrix) return fail(NECSIM_ERR_INVALID_ARG, "matrix missing");
         L.off_alias = off; off = align256(off + 8 * (size_t)L.ncells * L.ncells);
@@ -276,6 +281,31 @@ extern "C" int necsim_create_scenario(const necsim_scenario_desc *d, void *d_wor
             sd.gauss = (const u32 *)(base + L.off_gauss); sd.R = L.R; sd.gauss_len = L.gauss_len;
         }
     }
+    sd.sampler = d->sampler;
+    if (d->sampler) {   // Poisson sampler tables: cdf thresholds of mu_max; per-cell thinning thresholds
+        std::vector<u64> pc(NS_POIS_N);
+        double p = exp(-mu_max), cdf = 0.0;
+        for (u32 nn = 0; nn < NS_POIS_N; ++nn) {
+            if (nn > 0) p = p * mu_max / (double)nn;
+            cdf = cdf + p;
+            pc[nn] = (cdf >= 1.0) ? 0xFFFFFFFFFFFFFFFFull : (u64)ldexp(cdf, 64);
+        }
+        CU(cudaMemcpyAsync(base + L.off_pois, pc.data(), 8 * NS_POIS_N, cudaMemcpyHostToDevice, st));
+        sd.pois = (const u64 *)(base + L.off_pois);
+        if (L.per_cell_turnover) {
+            std::vector<u32> thin(n);
+            for (u32 c = 0; c < n; ++c) {
+                const u32 dm = L.uniform_deme ? sd.uniform_deme : d->deme[c];
+                const double mu = d->turnover[c] * d->delta_t;
+                if (dm == 0) thin[c] = 0;
+                else if (mu >= mu_max) thin[c] = 0xFFFFFFFFu;
+                else thin[c] = to_thresh32(mu / mu_max);
+            }
+            CU(cudaMemcpyAsync(base + L.off_thin, thin.data(), 4 * (size_t)n, cudaMemcpyHostToDevice, st));
+            sd.thin = (const u32 *)(base + L.off_thin);
+        }
+        CU(cudaStreamSynchronize(st));
+    }
     rc = upload_neglog_tables(st);
     if (rc) return rc;
     CU(cudaStreamSynchronize(st));
@@ -370,18 +400,22 @@ extern "C" int necsim_simulate_workspace_size(const necsim_scenario *scn, uint64
 }
 
 typedef void (*EpochKernel)(const ScenarioDev, const SimBuffers, const EpochArgs);
+template <int KIND, bool PERCELL, int SAMP>
+static EpochKernel pick_kernel3(bool dedup, bool tail) {
+    if (tail) return dedup ? (EpochKernel)tail_kernel<KIND, true, PERCELL, SAMP> : (EpochKernel)tail_kernel<KIND, false, PERCELL, SAMP>;
+    return dedup ? (EpochKernel)simulate_kernel<KIND, true, PERCELL, SAMP> : (EpochKernel)simulate_kernel<KIND, false, PERCELL, SAMP>;
+}
 template <int KIND, bool PERCELL>
-static EpochKernel pick_kernel2(bool dedup, bool tail) {
-    if (tail) return dedup ? (EpochKernel)tail_kernel<KIND, true, PERCELL> : (EpochKernel)tail_kernel<KIND, false, PERCELL>;
-    return dedup ? (EpochKernel)simulate_kernel<KIND, true, PERCELL> : (EpochKernel)simulate_kernel<KIND, false, PERCELL>;
+static EpochKernel pick_kernel2(int sampler, bool dedup, bool tail) {
+    return sampler ? pick_kernel3<KIND, PERCELL, 1>(dedup, tail) : pick_kernel3<KIND, PERCELL, 0>(dedup, tail);
 }
 // per-cell turnover exists for the explicit kinds only
-static EpochKernel pick_kernel(int kind, bool percell, bool dedup, bool tail) {
+static EpochKernel pick_kernel(int kind, bool percell, int sampler, bool dedup, bool tail) {
     switch (kind) {
-    case 0: return pick_kernel2<0, false>(dedup, tail);
-    case 1: return pick_kernel2<1, false>(dedup, tail);
-    case 2: return percell ? pick_kernel2<2, true>(dedup, tail) : pick_kernel2<2, false>(dedup, tail);
-    default: return percell ? pick_kernel2<3, true>(dedup, tail) : pick_kernel2<3, false>(dedup, tail);
+    case 0: return pick_kernel2<0, false>(sampler, dedup, tail);
+    case 1: return pick_kernel2<1, false>(sampler, dedup, tail);
+    case 2: return percell ? pick_kernel2<2, true>(sampler, dedup, tail) : pick_kernel2<2, false>(sampler, dedup, tail);
+    default: return percell ? pick_kernel2<3, true>(sampler, dedup, tail) : pick_kernel2<3, false>(sampler, dedup, tail);
     }
 }
 static int occupancy_for(EpochKernel fn, u32 block) {
@@ -444,8 +478,8 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
     ep.thr_nu = thr53(nu);
     ep.thr_m = thr53(scn->migration);
     ep.max_steps = (u32)rp.max_steps;
-    const EpochKernel fn_main = pick_kernel(sd.kind, sd.per_cell_turnover != 0, rp.dedup, false);
-    const EpochKernel fn_tail = pick_kernel(sd.kind, sd.per_cell_turnover != 0, rp.dedup, true);
+    const EpochKernel fn_main = pick_kernel(sd.kind, sd.per_cell_turnover != 0, (int)sd.sampler, rp.dedup, false);
+    const EpochKernel fn_tail = pick_kernel(sd.kind, sd.per_cell_turnover != 0, (int)sd.sampler, rp.dedup, true);
     const int occ = occupancy_for(fn_main, rp.block_threads);
     const int occ_tail = occupancy_for(fn_tail, rp.block_threads);
     ep.probe_mask = rp.probe_mask;
@@ -674,6 +708,33 @@ __global__ void debug_disperse_kernel(const ScenarioDev sc, SeedKey key, u64 thr
     loc_out[i] = l2;
 }
 
+__global__ void debug_next_event_poisson_kernel(const ScenarioDev sc, SeedKey key, const u32 *loc, const u32 *cell, const u32 *k, const i64 *f_last,
+                                                u32 *k_out, u32 *j_out, u64 *T_out, int *rc, u64 n) {
+    __shared__ unsigned short sPG[256];
+    __shared__ u64 sP[256];
+    poisson_stage(sc, sP, sPG);
+    SmemTables smt; smt.q = smt.a = smt.tg = smt.g2 = 0; smt.pc = smem_addr(sP); smt.pg = smem_addr(sPG);
+    u64 i = (u64)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const u32 thin = sc.thin ? sc.thin[cell[i]] : 0xFFFFFFFFu;
+    u32 kk = k[i];
+    i64 fl = f_last[i];
+    for (;;) {
+        const u64 s = prime(key, loc[i], kk);
+        const u32 N = poisson_count(s, smt);
+        u32 bi = 0; u64 bf = 0, X = s;
+        for (u32 q = 1; q <= N; ++q) {
+            X += NS_GAMMA;
+            const u64 f = poisson_offset(X);
+            if (!poisson_kept(X, thin)) continue;
+            if ((i64)f > fl && (bi == 0u || f < bf)) { bi = q; bf = f; }
+        }
+        if (bi) { k_out[i] = kk; j_out[i] = bi; T_out[i] = bf; rc[i] = 0; return; }
+        if (kk == 0xFFFFFFFFu) { k_out[i] = kk; j_out[i] = 0; T_out[i] = 0; rc[i] = -3; return; }
+        kk += 1; fl = -1;
+    }
+}
+
 static inline u32 grid_for(u64 n, u32 block) { return (u32)((n + block - 1) / block); }
 
 extern "C" int necsim_debug_draw(uint64_t seed, int lane, const uint32_t *d_loc, const uint32_t *d_k, const uint32_t *d_j, const uint32_t *d_r,
@@ -746,6 +807,31 @@ extern "C" int necsim_debug_tables(const necsim_scenario *scn, uint32_t *h_thres
             for (size_t i = 0; i < n; ++i) { if (h_Cm) h_Cm[i] = sd.Cm_u; if (h_sh) h_sh[i] = sd.sh_u; }
         }
     }
+    return NECSIM_OK;
+}
+
+extern "C" int necsim_debug_next_event_poisson(const necsim_scenario *scn, uint64_t seed, const uint32_t *d_loc, const uint32_t *d_cell,
+                                               const uint32_t *d_k, const int64_t *d_f_last, uint32_t *d_k_out, uint32_t *d_j_out,
+                                               uint64_t *d_T_out, int32_t *d_rc, uint64_t n, void *cuda_stream) {
+    if (!scn) return fail(NECSIM_ERR_INVALID_ARG, "NULL scenario");
+    if (!scn->dev.sampler) return fail(NECSIM_ERR_INVALID_ARG, "the scenario does not use the Poisson sampler");
+    if (n == 0) return NECSIM_OK;
+    debug_next_event_poisson_kernel<<<grid_for(n, 256), 256, 0, (cudaStream_t)cuda_stream>>>(scn->dev, key_schedule(seed), d_loc, d_cell, d_k,
+                                                                                             (const i64 *)d_f_last, d_k_out, d_j_out, d_T_out, d_rc, n);
+    CU(cudaGetLastError());
+    return NECSIM_OK;
+}
+extern "C" int necsim_debug_poisson_table(const necsim_scenario *scn, uint64_t *h_pc, uint32_t *h_thin, double *mu_max, void *cuda_stream) {
+    if (!scn) return fail(NECSIM_ERR_INVALID_ARG, "NULL scenario");
+    if (!scn->dev.sampler) return fail(NECSIM_ERR_INVALID_ARG, "the scenario does not use the Poisson sampler");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (mu_max) *mu_max = scn->mu_max;
+    if (h_pc) CU(cudaMemcpyAsync(h_pc, scn->dev.pois, 8 * NS_POIS_N, cudaMemcpyDeviceToHost, st));
+    if (h_thin) {
+        if (scn->dev.thin) CU(cudaMemcpyAsync(h_thin, scn->dev.thin, 4 * (size_t)scn->dev.ncells, cudaMemcpyDeviceToHost, st));
+        else for (u32 c = 0; c < scn->dev.ncells; ++c) h_thin[c] = 0xFFFFFFFFu;
+    }
+    CU(cudaStreamSynchronize(st));
     return NECSIM_OK;
 }
 

@@ -156,21 +156,36 @@ __device__ __forceinline__ bool cache_probes(u32 h, u32 probe_mask) { return ((h
 __device__ unsigned short NEGLOG_Q_DEV[512];
 __device__ u64 NEGLOG_A_DEV[512];
 
+// stages the Poisson cdf thresholds and their top-byte guide (call by all threads of the block; ends with __syncthreads)
+__device__ __forceinline__ void poisson_stage(const ScenarioDev &sc, u64 *sP, unsigned short *sPG) {
+    for (u32 i = threadIdx.x; i < NS_POIS_N; i += blockDim.x) sP[i] = sc.pois[i];
+    __syncthreads();
+    for (u32 b = threadIdx.x; b < 256u; b += blockDim.x) {
+        const u64 lim = (u64)b << 56;
+        u32 n = 0;
+        while (n < NS_POIS_N && sP[n] < lim) ++n;
+        sPG[b] = (unsigned short)n;
+    }
+    __syncthreads();
+}
+
 #define NS_ST_IDLE 0u
 #define NS_ST_SEARCH 1u     // needs draws of the event-time search (re-primes first when `need_prime`)
 #define NS_ST_EVENT 2u      // event (loc, k, j) found at offset T: `att` dispersal attempts rejected so far
 
-template <int KIND, bool DEDUP, bool PERCELL>
+// SAMP: 0 = exponential event-time sampler, 1 = Poisson / order statistics (2.7)
+template <int KIND, bool DEDUP, bool PERCELL, int SAMP>
 __global__ void __launch_bounds__(256) simulate_kernel(const ScenarioDev sc, const SimBuffers bf, const EpochArgs ep) {
-    __shared__ unsigned short sQ[512];
-    __shared__ u64 sA[512];
+    __shared__ unsigned short sQ[SAMP == 0 ? 512 : 256];      // SAMP 1: the Poisson guide
+    __shared__ u64 sA[SAMP == 0 ? 512 : 256];                 // SAMP 1: the Poisson cdf thresholds
     __shared__ u32 sG[KIND == 3 ? 1024 : 1];
     __shared__ uint2 sG2[KIND == 3 ? NS_G2_LEN : 1];
-    for (u32 i = threadIdx.x; i < 512; i += blockDim.x) { sQ[i] = NEGLOG_Q_DEV[i]; sA[i] = NEGLOG_A_DEV[i]; }
+    if (SAMP == 0) for (u32 i = threadIdx.x; i < 512; i += blockDim.x) { sQ[i] = NEGLOG_Q_DEV[i]; sA[i] = NEGLOG_A_DEV[i]; }
+    else poisson_stage(sc, sA, sQ);
     if (KIND == 3) gauss_stage(sc, sG, sG2);
     __syncthreads();
     GaussLut gl; gl.tg = smem_addr(sG); gl.g2 = smem_addr(sG2); gl.R = sc.R;
-    SmemTables smt; smt.q = smem_addr(sQ); smt.a = smem_addr(sA); smt.tg = gl.tg; smt.g2 = gl.g2;
+    SmemTables smt; smt.q = smem_addr(sQ); smt.a = smem_addr(sA); smt.tg = gl.tg; smt.g2 = gl.g2; smt.pc = smt.a; smt.pg = smt.q;
 
     const u32 lane = threadIdx.x & 31u;
     const u32 on_mask = ep.lanes_per_warp >= 32u ? 0xFFFFFFFFu : ((1u << ep.lanes_per_warp) - 1u);   // lanes that hold lineages
@@ -216,7 +231,12 @@ __global__ void __launch_bounds__(256) simulate_kernel(const ScenarioDev sc, con
                 } else {
                     X = prime(ep.key, loc, k);
                     T = 0; j = 0; need_prime = false;
-                    if (PERCELL) { uint2 cs = __ldg(&sc.scale[KIND == 3 ? xy_index(sc, cell) : cell]); Cm = cs.x; sh = cs.y; }
+                    if (SAMP == 0) {
+                        if (PERCELL) { uint2 cs = __ldg(&sc.scale[KIND == 3 ? xy_index(sc, cell) : cell]); Cm = cs.x; sh = cs.y; }
+                    } else {   // sh = number of points of this interval, Cm = thinning threshold of the cell, att = best point so far
+                        sh = poisson_count(X, smt); att = 0;
+                        if (PERCELL) Cm = __ldg(&sc.thin[KIND == 3 ? xy_index(sc, cell) : cell]);
+                    }
                 }
             }
             {   // survivors of this epoch go to the output queue (warp-aggregated append)
@@ -231,7 +251,21 @@ __global__ void __launch_bounds__(256) simulate_kernel(const ScenarioDev sc, con
                     }
                 }
             }
-            if (st == NS_ST_SEARCH) {
+            if (SAMP == 1 && st == NS_ST_SEARCH) {
+                // S1b (Poisson): one point of the interval per pass; keep the earliest one after f_last (ties: smallest i)
+                if (j < sh) {
+                    j += 1; X += NS_GAMMA;
+                    const u64 f = poisson_offset(X);
+                    const bool kept = PERCELL ? poisson_kept(X, Cm) : true;
+                    if (kept && (i64)f > f_last && (att == 0u || f < T)) { T = f; att = j; }
+                }
+                if (j >= sh) {                             // interval scanned
+                    if (att) { X -= (u64)(sh - att) * NS_GAMMA; j = att; att = 0; st = NS_ST_EVENT; }
+                    else if (k == 0xFFFFFFFFu) { atomicMax(&bf.ctr->error, 3u); st = NS_ST_IDLE; }
+                    else { k += 1; f_last = -1; need_prime = true; }
+                }
+            }
+            if (SAMP == 0 && st == NS_ST_SEARCH) {
                 // S1b: one exponential draw of the event-time search
                 j += 1; X += NS_GAMMA;
                 T += scale_exp(neglog(draw_time(X), smt), Cm, sh);

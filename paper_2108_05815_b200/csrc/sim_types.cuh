@@ -21,6 +21,9 @@ struct ScenarioDev {
     const u32 *prefix;         // [ncells+1] exclusive prefix sum of deme
     const uint2 *scale;        // [ncells] (Cm, sh) when per_cell_turnover
     const uint2 *alias;        // [ncells*ncells] (thresh, alias) for EXPLICIT_MATRIX
+    const u64 *pois;           // [256] Poisson cdf thresholds of mu_max (sampler 1)
+    const u32 *thin;           // [ncells] thinning thresholds (sampler 1 with per-cell turnover)
+    u32 sampler;               // 0 exponential, 1 Poisson / order statistics
     const u32 *gauss;          // [gauss_len] rounded-normal thresholds, padded with 0xFFFFFFFF to a power of two
     int R;                     // displacement range: dx in [-R, R]
     u32 gauss_len;             // power of two >= 2R

@@ -37,17 +37,77 @@ __device__ __forceinline__ void seg16_scan_step(u32 &lo, u32 &hi, u32 o) {
         : "r"(o));
 }
 
-template <int KIND, bool DEDUP, bool PERCELL>
+// per-cell rate data: exponential sampler -> (Cm, sh) of 1/(lambda dt); Poisson sampler -> (thinning threshold, unused)
+template <int SAMP>
+__device__ __forceinline__ uint2 load_rate(const ScenarioDev &sc, u32 idx) {
+    if (SAMP == 0) return __ldg(&sc.scale[idx]);
+    return make_uint2(__ldg(&sc.thin[idx]), 0u);
+}
+
+__device__ __forceinline__ u64 shfl_xor_u64(u64 v, int m) { return __shfl_xor_sync(NS_FULL, v, m); }
+
+// Poisson sampler, one search round of one lineage across the warp: lanes 0..15 the points 1..16 of
+// interval k, lanes 16..23 / 24..31 the points 1..8 of intervals k+1 / k+2. A butterfly min over (offset, ordinal) keys
+// finds the earliest existing point after f_last in the first non-empty interval. Returns true with (k, j, Te, Xe) set;
+// false after advancing k past intervals without a next event (the caller loops).
+template <bool PERCELL>
+__device__ __forceinline__ bool tail_search_poisson(const SeedKey &key, const SmemTables &smt, u32 lane, u32 loc, u32 &k, i64 &f_last,
+                                                    u32 k_stop, u32 thin, u32 &j, u64 &Te, u64 &Xe) {
+    const u32 seg = lane < 16u ? 0u : (lane < 24u ? 1u : 2u);
+    const u32 i = (lane < 16u ? lane : (lane & 7u)) + 1u;
+    const u64 kk64 = (u64)k + seg;
+    const bool kvalid = kk64 < (u64)k_stop;
+    const u64 s = prime(key, loc, (u32)kk64);
+    const u32 N = poisson_count(s, smt);
+    const u64 X = s + (u64)i * NS_GAMMA;
+    const u64 f = poisson_offset(X);
+    if (__ballot_sync(NS_FULL, kvalid && N > (seg ? 8u : 16u))) {
+        // more points than lanes somewhere (large mu): scan interval k one point at a time (every lane the same)
+        const u64 s0 = __shfl_sync(NS_FULL, s, 0);
+        const u32 N0 = __shfl_sync(NS_FULL, N, 0);
+        u32 bi = 0; u64 bf = 0, Xi = s0;
+        for (u32 q = 1; q <= N0; ++q) {
+            Xi += NS_GAMMA;
+            const u64 fq = poisson_offset(Xi);
+            if (PERCELL && !poisson_kept(Xi, thin)) continue;
+            if ((i64)fq > f_last && (bi == 0u || fq < bf)) { bi = q; bf = fq; }
+        }
+        if (!bi) { k += 1u; f_last = -1; return false; }
+        j = bi; Te = bf; Xe = s0 + (u64)bi * NS_GAMMA;
+        return true;
+    }
+    bool ok = kvalid && i <= N && (seg != 0u || (i64)f > f_last);
+    if (PERCELL) ok = ok && poisson_kept(X, thin);
+    u64 m = ok ? ((f << 8) | (u64)i) : ~0ull;
+    m = min(m, shfl_xor_u64(m, 1)); m = min(m, shfl_xor_u64(m, 2)); m = min(m, shfl_xor_u64(m, 4));
+    const u64 m16 = min(m, shfl_xor_u64(m, 8));
+    const u64 m0 = __shfl_sync(NS_FULL, m16, 0), m1 = __shfl_sync(NS_FULL, m, 16), m2 = __shfl_sync(NS_FULL, m, 24);
+    u64 best; u32 dk, base;
+    if (m0 != ~0ull) { best = m0; dk = 0u; base = 0u; }
+    else if (m1 != ~0ull) { best = m1; dk = 1u; base = 16u; }
+    else if (m2 != ~0ull) { best = m2; dk = 2u; base = 24u; }
+    else {   // no next event in the (up to three) intervals before the horizon
+        const u32 gap = k_stop - k;
+        k += gap < 3u ? gap : 3u; f_last = -1;
+        return false;
+    }
+    j = (u32)best & 255u; Te = best >> 8; k += dk;
+    Xe = __shfl_sync(NS_FULL, X, (int)(base + j - 1u));
+    return true;
+}
+
+template <int KIND, bool DEDUP, bool PERCELL, int SAMP>
 __global__ void __launch_bounds__(256) tail_kernel(const ScenarioDev sc, const SimBuffers bf, const EpochArgs ep) {
-    __shared__ unsigned short sQ[512];
-    __shared__ u64 sA[512];
+    __shared__ unsigned short sQ[SAMP == 0 ? 512 : 256];      // SAMP 1: the Poisson guide
+    __shared__ u64 sA[SAMP == 0 ? 512 : 256];                 // SAMP 1: the Poisson cdf thresholds
     __shared__ u32 sG[KIND == 3 ? 1024 : 1];
     __shared__ uint2 sG2[KIND == 3 ? NS_G2_LEN : 1];
-    for (u32 i = threadIdx.x; i < 512; i += blockDim.x) { sQ[i] = NEGLOG_Q_DEV[i]; sA[i] = NEGLOG_A_DEV[i]; }
+    if (SAMP == 0) for (u32 i = threadIdx.x; i < 512; i += blockDim.x) { sQ[i] = NEGLOG_Q_DEV[i]; sA[i] = NEGLOG_A_DEV[i]; }
+    else poisson_stage(sc, sA, sQ);
     if (KIND == 3) gauss_stage(sc, sG, sG2);
     __syncthreads();
     GaussLut gl; gl.tg = smem_addr(sG); gl.g2 = smem_addr(sG2); gl.R = sc.R;
-    SmemTables smt; smt.q = smem_addr(sQ); smt.a = smem_addr(sA); smt.tg = gl.tg; smt.g2 = gl.g2;
+    SmemTables smt; smt.q = smem_addr(sQ); smt.a = smem_addr(sA); smt.tg = gl.tg; smt.g2 = gl.g2; smt.pc = smt.a; smt.pg = smt.q;
 
     u32 lane;
     asm volatile("mov.u32 %0, %%laneid;" : "=r"(lane));                // opaque: kept in a register, not re-read per use
@@ -70,7 +130,7 @@ __global__ void __launch_bounds__(256) tail_kernel(const ScenarioDev sc, const S
         const u32 id = qe.x;
         u32 loc = qe.y, cell = qe.z, steps = qe.w, k = ep.k_start, Cm = sc.Cm_u, sh = sc.sh_u;
         i64 f_last = -1;
-        if (PERCELL) { uint2 cs = __ldg(&sc.scale[KIND == 3 ? xy_index(sc, cell) : cell]); Cm = cs.x; sh = cs.y; }
+        if (PERCELL) { uint2 cs = load_rate<SAMP>(sc, KIND == 3 ? xy_index(sc, cell) : cell); Cm = cs.x; sh = cs.y; }
         // pending duplicate check: the exchange of the last probing event (lane 0 holds its result)
         bool pend = false;
         uint4 pold = make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu);
@@ -100,46 +160,51 @@ __global__ void __launch_bounds__(256) tail_kernel(const ScenarioDev sc, const S
                 if (lane == 0) bf.q_out[atomicAdd(&bf.ctr->q_out, 1u)] = make_uint4(id, loc, cell, steps);
                 break;
             }
-            // ---- S1: candidate points of the event-time search ---------------------------------------------------
-            const u64 kk64 = (u64)k + (half ? (u64)(1u + sub) : 0ull);
-            const bool kvalid = kk64 < (u64)ep.k_stop;                // never look at or past the horizon
-            u64 X = prime(ep.key, loc, (u32)kk64) + cand_add;
-            const u64 T1 = scale_exp(neglog(draw_time(X), smt), Cm, sh);
-            // partial sums over each 16-lane half (half 1 keeps its single draws: first points of fresh intervals)
-            u32 t_lo = (u32)T1, t_hi = (u32)(T1 >> 32);
-            seg16_scan_step(t_lo, t_hi, 1); seg16_scan_step(t_lo, t_hi, 2);
-            seg16_scan_step(t_lo, t_hi, 4); seg16_scan_step(t_lo, t_hi, 8);
-            const u64 T = half ? T1 : (((u64)t_hi << 32) | t_lo);
-            const bool inside = T < NS_TWO48;
-            const u32 evm = __ballot_sync(NS_FULL, inside && (half ? kvalid : ((i64)T > f_last)));
-            const u32 crm = __ballot_sync(NS_FULL, !inside);
             u32 j;
             u64 Te, Xe;
-            if (evm & 0xFFFFu) {                       // next event is in interval k
-                const int src = __ffs(evm & 0xFFFFu) - 1;
-                j = (u32)src + 1u;
-                Te = __shfl_sync(NS_FULL, T, src); Xe = __shfl_sync(NS_FULL, X, src);
-            } else if (crm & 0xFFFFu) {                // interval k exhausted (L719, L727): first non-empty interval after it
-                const u32 gap = ep.k_stop - 1u - k;    // k < k_stop here
-                const u32 nvalid = gap < 16u ? gap : 16u;
-                const u32 hm = evm >> 16;
-                if (!hm) { k = k + 1u + nvalid; f_last = -1; continue; }   // all speculated intervals empty / beyond the horizon
-                const int src = 16 + __ffs(hm) - 1;
-                k = k + 1u + (u32)(src - 16); j = 1u;
-                Te = __shfl_sync(NS_FULL, T, src); Xe = __shfl_sync(NS_FULL, X, src);
+            if (SAMP == 1) {
+                // S1 (Poisson sampler, Cm = thinning threshold of the cell)
+                if (!tail_search_poisson<PERCELL>(ep.key, smt, lane, loc, k, f_last, ep.k_stop, Cm, j, Te, Xe)) continue;
             } else {
-                // more than 16 points of interval k at or before f_last (large mu): continue the scan one draw at a time
-                u64 Tc = __shfl_sync(NS_FULL, T, 15), Xc = __shfl_sync(NS_FULL, X, 15);
-                u32 jc = 16u;
-                bool found = false;
-                for (;;) {
-                    jc += 1u; Xc += NS_GAMMA;
-                    Tc += scale_exp(neglog(draw_time(Xc), smt), Cm, sh);
-                    if (Tc >= NS_TWO48) break;
-                    if ((i64)Tc > f_last) { found = true; break; }
+                // ---- S1: candidate points of the event-time search ---------------------------------------------------
+                const u64 kk64 = (u64)k + (half ? (u64)(1u + sub) : 0ull);
+                const bool kvalid = kk64 < (u64)ep.k_stop;                // never look at or past the horizon
+                u64 X = prime(ep.key, loc, (u32)kk64) + cand_add;
+                const u64 T1 = scale_exp(neglog(draw_time(X), smt), Cm, sh);
+                // partial sums over each 16-lane half (half 1 keeps its single draws: first points of fresh intervals)
+                u32 t_lo = (u32)T1, t_hi = (u32)(T1 >> 32);
+                seg16_scan_step(t_lo, t_hi, 1); seg16_scan_step(t_lo, t_hi, 2);
+                seg16_scan_step(t_lo, t_hi, 4); seg16_scan_step(t_lo, t_hi, 8);
+                const u64 T = half ? T1 : (((u64)t_hi << 32) | t_lo);
+                const bool inside = T < NS_TWO48;
+                const u32 evm = __ballot_sync(NS_FULL, inside && (half ? kvalid : ((i64)T > f_last)));
+                const u32 crm = __ballot_sync(NS_FULL, !inside);
+                if (evm & 0xFFFFu) {                       // next event is in interval k
+                    const int src = __ffs(evm & 0xFFFFu) - 1;
+                    j = (u32)src + 1u;
+                    Te = __shfl_sync(NS_FULL, T, src); Xe = __shfl_sync(NS_FULL, X, src);
+                } else if (crm & 0xFFFFu) {                // interval k exhausted (L719, L727): first non-empty interval after it
+                    const u32 gap = ep.k_stop - 1u - k;    // k < k_stop here
+                    const u32 nvalid = gap < 16u ? gap : 16u;
+                    const u32 hm = evm >> 16;
+                    if (!hm) { k = k + 1u + nvalid; f_last = -1; continue; }   // all speculated intervals empty / beyond the horizon
+                    const int src = 16 + __ffs(hm) - 1;
+                    k = k + 1u + (u32)(src - 16); j = 1u;
+                    Te = __shfl_sync(NS_FULL, T, src); Xe = __shfl_sync(NS_FULL, X, src);
+                } else {
+                    // more than 16 points of interval k at or before f_last (large mu): continue the scan one draw at a time
+                    u64 Tc = __shfl_sync(NS_FULL, T, 15), Xc = __shfl_sync(NS_FULL, X, 15);
+                    u32 jc = 16u;
+                    bool found = false;
+                    for (;;) {
+                        jc += 1u; Xc += NS_GAMMA;
+                        Tc += scale_exp(neglog(draw_time(Xc), smt), Cm, sh);
+                        if (Tc >= NS_TWO48) break;
+                        if ((i64)Tc > f_last) { found = true; break; }
+                    }
+                    if (!found) { k += 1u; f_last = -1; continue; }
+                    j = jc; Te = Tc; Xe = Xc;
                 }
-                if (!found) { k += 1u; f_last = -1; continue; }
-                j = jc; Te = Tc; Xe = Xc;
             }
 
             // ---- event (loc, k, j) at offset Te --------------------------------------------------------------
@@ -178,7 +243,7 @@ __global__ void __launch_bounds__(256) tail_kernel(const ScenarioDev sc, const S
                     cell2 = ((u32)x < e.x) ? col : e.y;
                     const u32 d = cell_deme(sc, cell2);
                     loc2 = cell_prefix(sc, cell2) + ((d == 1u) ? 0u : mulhi64_u32(xi, d));
-                    if (PERCELL) { const uint2 cs = __ldg(&sc.scale[cell2]); Cm2 = cs.x; sh2 = cs.y; }
+                    if (PERCELL) { const uint2 cs = load_rate<SAMP>(sc, cell2); Cm2 = cs.x; sh2 = cs.y; }
                 } else {
                     const u64 xi = __shfl_sync(NS_FULL, u, 1);
                     const u32 x0 = cell & 0xFFFFu, y0 = cell >> 16;
@@ -196,7 +261,7 @@ __global__ void __launch_bounds__(256) tail_kernel(const ScenarioDev sc, const S
                             c2 = (yy << 16) | xx;
                             d = cell_deme(sc, ci);
                             pf = cell_prefix(sc, ci);                       // speculative: same round trip as the habitat test
-                            if (PERCELL) cs = __ldg(&sc.scale[ci]);
+                            if (PERCELL) cs = load_rate<SAMP>(sc, ci);
                         }
                         const u32 okm = __ballot_sync(NS_FULL, lane >= 3u && d > 0u);
                         if (okm) {

@@ -16,11 +16,11 @@ LIB_PATH = os.path.join(_HERE, "csrc", "libnecsim_b200.so")
 EXPORTS = ["necsim_scenario_workspace_size", "necsim_create_scenario", "necsim_scenario_num_individuals",
            "necsim_simulate_workspace_size", "necsim_simulate", "necsim_simulate_host", "necsim_destroy", "necsim_last_error",
            "necsim_debug_draw", "necsim_debug_neglog", "necsim_debug_next_event", "necsim_debug_disperse", "necsim_debug_tables",
-           "necsim_debug_int_peak"]
+           "necsim_debug_int_peak", "necsim_debug_next_event_poisson", "necsim_debug_poisson_table"]
 
 
 class ScenarioDesc(C.Structure):
-    _fields_ = [("kind", C.c_int32), ("width", C.c_uint32), ("height", C.c_uint32), ("deme", C.c_void_p),
+    _fields_ = [("kind", C.c_int32), ("width", C.c_uint32), ("height", C.c_uint32), ("sampler", C.c_uint32), ("deme", C.c_void_p),
                 ("uniform_deme", C.c_uint32), ("turnover", C.c_void_p), ("uniform_turnover", C.c_double),
                 ("dispersal_matrix", C.c_void_p), ("sigma", C.c_double), ("local_size", C.c_uint64),
                 ("meta_size", C.c_uint64), ("migration", C.c_double), ("delta_t", C.c_double)]
@@ -81,6 +81,8 @@ def lib():
         L.necsim_debug_disperse.argtypes = [vp, u64, vp, vp, vp, vp, u64, vp]
         L.necsim_debug_tables.argtypes = [vp] * 8
         L.necsim_debug_int_peak.argtypes = [C.c_int, u32, vp, vp, vp]
+        L.necsim_debug_next_event_poisson.argtypes = [vp, u64] + [vp] * 8 + [u64, vp]
+        L.necsim_debug_poisson_table.argtypes = [vp] * 5
         _lib = L
     return _lib
 
@@ -125,13 +127,13 @@ class Scenario:
     """necsim_create_scenario / necsim_simulate / necsim_destroy (include/necsim.h)."""
 
     def __init__(self, kind, width=1, height=1, deme=None, uniform_deme=0, turnover=None, uniform_turnover=1.0, matrix=None,
-                 sigma=0.0, local_size=0, meta_size=0, migration=0.0, delta_t=2.0):
+                 sigma=0.0, local_size=0, meta_size=0, migration=0.0, delta_t=2.0, sampler=0):
         torch = _torch()
         L = lib()
         self._h = None
         d = ScenarioDesc()
         keep = []
-        d.kind, d.width, d.height = int(kind), int(width), int(height)
+        d.kind, d.width, d.height, d.sampler = int(kind), int(width), int(height), int(sampler)
         if deme is not None:
             a = np.ascontiguousarray(deme, dtype=np.uint32).ravel(); keep.append(a); d.deme = a.ctypes.data
         d.uniform_deme = int(uniform_deme)
@@ -220,6 +222,23 @@ class Scenario:
         return out
 
     # ---- test-only -----------------------------------------------------------------------------------
+    def debug_next_event_poisson(self, seed, loc, cell, k, f_last):
+        torch = _torch()
+        loc = np.ascontiguousarray(loc, dtype=np.uint32); n = len(loc)
+        dl, dc, dk = _dev_u32(torch, loc), _dev_u32(torch, cell, n), _dev_u32(torch, k, n)
+        df = torch.from_numpy(np.ascontiguousarray(np.broadcast_to(np.asarray(f_last, dtype=np.int64), (n,)))).cuda()
+        ko = torch.empty(n, dtype=torch.int32, device="cuda"); jo = torch.empty_like(ko); rc = torch.empty_like(ko)
+        To = torch.empty(n, dtype=torch.int64, device="cuda")
+        _check(lib().necsim_debug_next_event_poisson(self._h, int(seed), dl.data_ptr(), dc.data_ptr(), dk.data_ptr(), df.data_ptr(), ko.data_ptr(),
+                                                     jo.data_ptr(), To.data_ptr(), rc.data_ptr(), n, _stream_ptr(torch)))
+        return (ko.cpu().numpy().view(np.uint32), jo.cpu().numpy().view(np.uint32), To.cpu().numpy().view(np.uint64), rc.cpu().numpy())
+
+    def debug_poisson_table(self):
+        torch = _torch()
+        pc = np.zeros(256, np.uint64); thin = np.zeros(self.ncells, np.uint32); mu = C.c_double()
+        _check(lib().necsim_debug_poisson_table(self._h, _hptr(pc), _hptr(thin), C.byref(mu), _stream_ptr(torch)))
+        return mu.value, pc, thin
+
     def debug_disperse(self, seed, loc, k, j):
         torch = _torch()
         loc = np.ascontiguousarray(loc, dtype=np.uint32); n = len(loc)
