@@ -252,8 +252,9 @@ __global__ void __launch_bounds__(256) simulate_kernel(const ScenarioDev sc, con
                 }
             }
             if (SAMP == 1 && st == NS_ST_SEARCH) {
-                // S1b (Poisson): one point of the interval per pass; keep the earliest one after f_last (ties: smallest i)
-                if (j < sh) {
+                // S1b (Poisson): scan the interval's points; keep the earliest one after f_last (ties: smallest i)
+#pragma unroll 1
+                for (u32 q = 0; q < 4u && j < sh; ++q) {   // up to four points per pass: amortises the phase scheduling
                     j += 1; X += NS_GAMMA;
                     const u64 f = poisson_offset(X);
                     const bool kept = PERCELL ? poisson_kept(X, Cm) : true;
