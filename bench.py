@@ -110,7 +110,7 @@ def reference_arm(args, cfg, name):
     v = float(np.mean(vals))
     print(json.dumps({"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": len(vals), "warmup": args.warmup,
                       "ms_per_step": 1e3 * float(np.mean(secs)), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-                      "dtype": "int64", "data": "synthetic", "config": {"workload": cfg["name"], "sample": desc},
+                      "dtype": "int64", "data": "synthetic", "config": {"workload": cfg["name"], "event_time_sampler": args.sampler, "sample": desc},
                       "cpu_baseline": {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc},
                       "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
 
@@ -123,10 +123,13 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="c5", choices=sorted(MAKERS))
     ap.add_argument("--small", action="store_true", help="the reduced config of the same kind (for testing the harness)")
+    ap.add_argument("--sampler", default="exp", choices=["exp", "poisson"],
+                    help="event-time sampler of the scenario (DESIGN.md 2.4 / 2.7): same law, different realisation")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     name = args.config
     cfg = make_cfg(name, args.small)
+    cfg["sampler"] = 1 if args.sampler == "poisson" else 0
     if args.impl == "reference":
         return reference_arm(args, cfg, name)
 
@@ -212,7 +215,7 @@ def main():
         mode_t = rt.n_events_raw / (rt.ms_simulate * 1e-3)
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": args.warmup, "ms_per_step": ms / K,
                 "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int64", "data": "synthetic",
-                "config": {"workload": cfg["name"], "n_lineages": int(res.n_lineages), "nu": cfg["nu"], "mode": "MODE-S (dedup on, to completion)",
+                "config": {"workload": cfg["name"], "event_time_sampler": args.sampler, "n_lineages": int(res.n_lineages), "nu": cfg["nu"], "mode": "MODE-S (dedup on, to completion)",
                            "l2": "256 MiB flush write between steps", "parallelism": "replicas x%d" % world},
                 "clocks": clocks,
                 "e2e": {"value": e2e_ev_all / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms / K,

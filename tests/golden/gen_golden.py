@@ -2,6 +2,7 @@
 
     python tests/golden/gen_golden.py            # rng_vectors.txt, neglog_vectors.txt, small_configs.json
     python tests/golden/gen_golden.py --full     # additionally full_configs.json (minutes to hours of CPU)
+    python tests/golden/gen_golden.py --full-poisson   # additionally full_configs_poisson.json (sampler = 1)
 """
 import json
 import os
@@ -57,10 +58,10 @@ def summarise(cfg, res):
                 labels_head=[int(v) for v in res["labels"][:16]])
 
 
-def configs(which, fname, epoch_events=0):
+def configs(which, fname, epoch_events=0, sampler=0):
     out = []
     for cfg in which:
-        sc = O.Scenario(**I.scenario_kwargs(cfg))
+        sc = O.Scenario(**dict(I.scenario_kwargs(cfg), sampler=sampler))
         res = sc.simulate(cfg["seed"], cfg["nu"], cfg["mask"], dedup=True, epoch_events=epoch_events)
         out.append(summarise(cfg, res))
         print(out[-1]["name"], out[-1]["richness"], out[-1]["unique_events"], flush=True)
@@ -74,3 +75,5 @@ if __name__ == "__main__":
     configs(I.small_configs(), "small_configs.json")
     if "--full" in sys.argv:
         configs(I.full_configs(), "full_configs.json", epoch_events=50_000_000)
+    if "--full-poisson" in sys.argv:      # the Poisson event-time sampler on the same five configs
+        configs(I.full_configs(), "full_configs_poisson.json", epoch_events=50_000_000, sampler=1)

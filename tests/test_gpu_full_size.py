@@ -14,7 +14,8 @@ import pytest
 
 pytestmark = pytest.mark.gpu
 HERE = os.path.dirname(os.path.abspath(__file__))
-GOLDEN = os.path.join(HERE, "golden", "full_configs.json")
+GOLDEN = {0: os.path.join(HERE, "golden", "full_configs.json"),             # exponential event-time sampler
+          1: os.path.join(HERE, "golden", "full_configs_poisson.json")}     # Poisson / order statistics (2.7)
 
 
 def digest(res):
@@ -26,21 +27,23 @@ def digest(res):
     return h.hexdigest()
 
 
-@pytest.fixture(scope="module")
-def golden():
-    if not os.path.exists(GOLDEN):
-        pytest.skip("tests/golden/full_configs.json not generated")
-    return {g["name"]: g for g in json.load(open(GOLDEN))}
+def load_golden(sampler):
+    if not os.path.exists(GOLDEN[sampler]):
+        pytest.skip(os.path.basename(GOLDEN[sampler]) + " not generated")
+    return {g["name"]: g for g in json.load(open(GOLDEN[sampler]))}
 
 
+@pytest.mark.parametrize("sampler", [0, 1])
 @pytest.mark.parametrize("idx", range(5))
-def test_full_config_matches_oracle(O, golden, idx):
+def test_full_config_matches_oracle(O, idx, sampler):
+    golden = load_golden(sampler)
     from paper_2108_05815_b200 import inputs as I, necsim as ns
     cfg = [I.c1_nonspatial, I.c2_implicit, I.c3_matrix, I.c4_gaussian, I.c5_stress][idx]()
     if cfg["name"] not in golden:
         pytest.skip("no golden record for " + cfg["name"])
     g = golden[cfg["name"]]
-    sc = ns.Scenario(**I.scenario_kwargs(cfg))
+    kw = dict(I.scenario_kwargs(cfg), sampler=sampler)
+    sc = ns.Scenario(**kw)
     got = sc.simulate(cfg["seed"], cfg["nu"], cfg["mask"])
     assert len(got["labels"]) == g["n_sampled"]
     assert got["richness"] == g["richness"]
@@ -58,7 +61,7 @@ def test_full_config_matches_oracle(O, golden, idx):
     n_ind = sc.n_individuals
     sampled = np.arange(n_ind) if cfg["mask"] is None else np.flatnonzero(cfg["mask"])
     rng = np.random.default_rng(idx)
-    osc = O.Scenario(**I.scenario_kwargs(cfg))
+    osc = O.Scenario(**kw)
     for pos in rng.choice(len(sampled), 3, replace=False):
         m = np.zeros(n_ind, np.uint8); m[sampled[pos]] = 1
         one = osc.simulate(cfg["seed"], cfg["nu"], m, dedup=False)
