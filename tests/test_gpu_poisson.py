@@ -46,7 +46,8 @@ def test_tables_and_search_primitive(ns, O, I):
         mu, pc, thin = g.debug_poisson_table()
         omu, opc = o.poisson_table()
         assert mu == omu and np.array_equal(pc, opc)
-        assert all(int(thin[c]) == o.thin(int(c)) for c in rng.integers(0, g.ncells, min(g.ncells, 50)))
+        hab_cells = np.arange(g.ncells) if kw.get("deme") is None else np.flatnonzero(np.asarray(kw["deme"]).ravel() > 0)
+        assert all(int(thin[c]) == o.thin(int(c)) for c in rng.choice(hab_cells, min(len(hab_cells), 50)))   # habitat cells only
         n = 20_001
         cell = rng.integers(0, g.ncells, n).astype(np.uint32)
         if kw["kind"] >= I.EXPLICIT_MATRIX and kw.get("deme") is not None:
