@@ -165,6 +165,18 @@ int necsim_simulate_host(necsim_scenario *scn, uint64_t seed, double nu, const u
                          uint64_t n_sampled_capacity, const necsim_sim_params *params, void *d_workspace /*DEVICE*/, size_t bytes,
                          void *cuda_stream, necsim_result *out, necsim_event *h_events /*HOST*/, uint32_t *h_labels /*HOST*/);
 
+/*
+ * Merge of the species tables of isolated partitions ("IsolatedIndividuals / IsolatedLandscape", replay
+ * L2511-2532): lineages simulated separately (other GPUs, other calls, later additions, L1485) reach the same
+ * speciation events where they coalesce, so the union of the partitions' tables, made unique, is the table of the whole
+ * sample. d_events_in: DEVICE [n] concatenation of d_events arrays; d_events_out: DEVICE [n] capacity, receives the
+ * merged table sorted by (k, f, loc, j) with abundances added up; d_map: DEVICE [n], rank in the merged table of every
+ * input record (a partition's labels are translated by map[offset_of_partition + label]); *richness: HOST out.
+ */
+int necsim_merge_workspace_size(uint64_t n, size_t *device_bytes /*HOST out*/);
+int necsim_merge_species(const necsim_event *d_events_in /*DEVICE*/, uint64_t n, void *d_workspace /*DEVICE*/, size_t bytes, void *cuda_stream,
+                         necsim_event *d_events_out /*DEVICE*/, uint32_t *d_map /*DEVICE*/, uint64_t *richness /*HOST out*/);
+
 /* Frees the host-side handle (NULL is a no-op). The device workspace belongs to the caller. */
 int necsim_destroy(necsim_scenario *scn);
 

@@ -190,6 +190,28 @@ __global__ void __launch_bounds__(256) label_kernel(const SimBuffers bf, u32 n, 
     }
 }
 
+// ---- merge of species tables from isolated partitions -------
+// AoS species records -> the SoA key arrays the radix passes read; perm = identity
+__global__ void __launch_bounds__(256) merge_unpack_kernel(const necsim_event *__restrict__ in, u32 n, const SimBuffers bf, u32 *__restrict__ perm) {
+    u32 i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const necsim_event e = in[i];
+    bf.term_loc[i] = e.loc; bf.term_k[i] = e.k; bf.term_j[i] = e.j; bf.term_f[i] = e.f;
+    perm[i] = i;
+}
+// sorted + head-flag-scanned records -> merged table (abundances add up), map[input record] = rank in the merged table
+__global__ void __launch_bounds__(256) merge_write_kernel(const SimBuffers bf, const u32 *__restrict__ perm, u32 n, const u32 *__restrict__ uidx,
+                                                          const necsim_event *__restrict__ in, necsim_event *__restrict__ out, u32 *__restrict__ map) {
+    u32 i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const u32 id = perm[i];
+    const bool head = (i == 0) || !same_event(bf, id, perm[i - 1]);
+    const u32 e = head ? uidx[i] : uidx[i] - 1u;
+    map[id] = e;
+    if (head) { out[e].loc = in[id].loc; out[e].k = in[id].k; out[e].j = in[id].j; out[e].f = in[id].f; out[e].time = in[id].time; }
+    atomicAdd(&out[e].abundance, in[id].abundance);
+}
+
 __global__ void copy_u32_kernel(u32 *a, const u32 *src, u32 n) {
     u32 i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i < n) a[i] = src[i];

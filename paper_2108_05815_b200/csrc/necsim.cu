@@ -637,6 +637,56 @@ extern "C" int necsim_simulate_host(necsim_scenario *scn, uint64_t seed, double 
 }
 
 // ---------------------------------------------------------------------------------------------------
+// merge of species tables (NEXT-2: isolated partitions + merge)
+// ---------------------------------------------------------------------------------------------------
+struct MergeLayout { size_t off_loc, off_k, off_j, off_f, off_pa, off_pb, off_flag, off_hist, off_cnt, total; u32 nb; };
+static void merge_layout(u64 n, MergeLayout &L) {
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off = align256(off + bytes); return o; };
+    L.nb = (u32)((n + NS_SORT_TILE - 1) / NS_SORT_TILE); if (L.nb == 0) L.nb = 1;
+    L.off_loc = take(4 * n); L.off_k = take(4 * n); L.off_j = take(4 * n); L.off_f = take(8 * n);
+    L.off_pa = take(4 * n); L.off_pb = take(4 * n); L.off_flag = take(4 * n); L.off_hist = take(4 * 256 * (size_t)L.nb); L.off_cnt = take(256);
+    L.total = off;
+}
+extern "C" int necsim_merge_workspace_size(uint64_t n, size_t *device_bytes) {
+    if (!device_bytes || n == 0 || n >= (1ull << 32)) return fail(NECSIM_ERR_INVALID_ARG, "n must be in [1, 2^32)");
+    MergeLayout L; merge_layout(n, L); *device_bytes = L.total;
+    return NECSIM_OK;
+}
+extern "C" int necsim_merge_species(const necsim_event *d_in, uint64_t n64, void *d_workspace, size_t bytes, void *cuda_stream,
+                                    necsim_event *d_out, uint32_t *d_map, uint64_t *richness) {
+    if (!d_in || !d_out || !d_map || !richness || n64 == 0 || n64 >= (1ull << 32)) return fail(NECSIM_ERR_INVALID_ARG, "bad argument");
+    MergeLayout L; merge_layout(n64, L);
+    if (!d_workspace || bytes < L.total) return fail(NECSIM_ERR_WORKSPACE_TOO_SMALL, "merge workspace too small");
+    if (((uintptr_t)d_workspace & 255u) != 0) return fail(NECSIM_ERR_INVALID_ARG, "workspace must be 256-byte aligned");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const u32 n = (u32)n64, g256 = (n + 255) / 256;
+    uint8_t *base = (uint8_t *)d_workspace;
+    SimBuffers bf; memset(&bf, 0, sizeof(bf));
+    bf.term_loc = (u32 *)(base + L.off_loc); bf.term_k = (u32 *)(base + L.off_k); bf.term_j = (u32 *)(base + L.off_j); bf.term_f = (u64 *)(base + L.off_f);
+    u32 *pa = (u32 *)(base + L.off_pa), *pb = (u32 *)(base + L.off_pb), *flag = (u32 *)(base + L.off_flag), *hist = (u32 *)(base + L.off_hist);
+    u32 *cnt = (u32 *)(base + L.off_cnt);
+    CU(cudaMemsetAsync(d_out, 0, sizeof(necsim_event) * (size_t)n, st));
+    merge_unpack_kernel<<<g256, 256, 0, st>>>(d_in, n, bf, pa);
+    u32 *src = pa, *dst = pb;
+    for (u32 b = 0; b < 18; ++b) {   // all 18 key bytes: the tables are small (thousands of records)
+        radix_hist_kernel<<<L.nb, 256, 0, st>>>(bf, src, n, b, hist, L.nb);
+        scan_exclusive_kernel<<<1, 1024, 0, st>>>(hist, 256 * L.nb, NULL);
+        radix_scatter_kernel<<<L.nb, 256, 0, st>>>(bf, src, dst, n, b, hist, L.nb);
+        std::swap(src, dst);
+    }
+    unique_flag_kernel<<<g256, 256, 0, st>>>(bf, src, n, flag);
+    scan_exclusive_kernel<<<1, 1024, 0, st>>>(flag, n, cnt);
+    merge_write_kernel<<<g256, 256, 0, st>>>(bf, src, n, flag, d_in, d_out, d_map);
+    CU(cudaGetLastError());
+    u32 h_cnt = 0;
+    CU(cudaMemcpyAsync(&h_cnt, cnt, 4, cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    *richness = h_cnt;
+    return NECSIM_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------
 // test-only exports: device primitives over arrays
 // ---------------------------------------------------------------------------------------------------
 __global__ void debug_draw_kernel(SeedKey key, int lane_kind, const u32 *loc, const u32 *k, const u32 *j, const u32 *r, u64 *out, u64 n) {

@@ -23,6 +23,57 @@ def aggregate(times_ms, units, device="cpu"):
     return t.tolist(), u.tolist()
 
 
+def shard_mask(mask, n_individuals, rank, world):
+    """Rank `rank`'s share of the sample: a contiguous range of the sampled individuals in canonical order (cells row-major:
+    spatially coherent, the paper's IsolatedLandscape partitioning). Returns a uint8 numpy mask."""
+    import numpy as np
+    m = np.ones(n_individuals, np.uint8) if mask is None else (np.asarray(mask) != 0).astype(np.uint8)
+    idx = np.flatnonzero(m)
+    lo, hi = (len(idx) * rank) // world, (len(idx) * (rank + 1)) // world
+    out = np.zeros(n_individuals, np.uint8)
+    out[idx[lo:hi]] = 1
+    return out
+
+
+def gather_tables(local, record_bytes=32):
+    """All-gathers variable-length byte tensors (one species table per rank). Returns (concatenation in rank order,
+    per-rank record offsets). The one exchange step of the partitioned path: sizes, then padded tables."""
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return local, [0]
+    world = dist.get_world_size()
+    n = torch.tensor([local.numel()], dtype=torch.int64, device=local.device)
+    sizes = [torch.zeros_like(n) for _ in range(world)]
+    dist.all_gather(sizes, n)
+    sizes = [int(s.item()) for s in sizes]
+    pad = torch.zeros(max(max(sizes), 1), dtype=torch.uint8, device=local.device)
+    pad[: local.numel()] = local
+    bufs = [torch.empty_like(pad) for _ in range(world)]
+    dist.all_gather(bufs, pad)
+    cat = torch.cat([b[:s] for b, s in zip(bufs, sizes)])
+    offsets, acc = [], 0
+    for s in sizes:
+        offsets.append(acc // record_bytes); acc += s
+    return cat, offsets
+
+
+def simulate_partitioned(scenario, seed, nu, mask=None, rank=0, world=1, params=None):
+    """Isolated partitions + merge: this rank simulates its share of the sample with no
+    communication, then ONE all-gather of the species tables and a device-side merge (necsim_merge_species) give the table
+    of the whole sample. Returns dict(events: CUDA uint8 [S * 32] merged table, labels: CUDA int64 [local lineages] indices
+    into it, richness, local: the rank's Result)."""
+    from . import necsim as ns
+    m = shard_mask(mask, scenario.n_individuals, rank, world)
+    if int(m.sum()) == 0:
+        local_tab = torch.empty(0, dtype=torch.uint8, device="cuda"); labels = torch.empty(0, dtype=torch.int64, device="cuda"); res = None
+    else:
+        res = scenario.simulate_raw(seed, nu, torch.from_numpy(m).cuda(), int(m.sum()), params)
+        tab, lab = scenario.result_tensors(res)
+        local_tab, labels = tab.clone(), lab.to(torch.int64)
+    cat, offsets = gather_tables(local_tab)
+    merged, dmap = ns.merge_species(cat)
+    return dict(events=merged, labels=dmap[offsets[rank if len(offsets) > 1 else 0] + labels], richness=merged.numel() // 32, local=res)
+
+
 def throughput(units_total, time_ms_max):
     """Whole-job units per second: everything all ranks processed over the slowest rank's time."""
     return units_total / (time_ms_max * 1e-3)

@@ -16,7 +16,8 @@ LIB_PATH = os.path.join(_HERE, "csrc", "libnecsim_b200.so")
 EXPORTS = ["necsim_scenario_workspace_size", "necsim_create_scenario", "necsim_scenario_num_individuals",
            "necsim_simulate_workspace_size", "necsim_simulate", "necsim_simulate_host", "necsim_destroy", "necsim_last_error",
            "necsim_debug_draw", "necsim_debug_neglog", "necsim_debug_next_event", "necsim_debug_disperse", "necsim_debug_tables",
-           "necsim_debug_int_peak", "necsim_debug_next_event_poisson", "necsim_debug_poisson_table"]
+           "necsim_debug_int_peak", "necsim_debug_next_event_poisson", "necsim_debug_poisson_table",
+           "necsim_merge_workspace_size", "necsim_merge_species"]
 
 
 class ScenarioDesc(C.Structure):
@@ -83,6 +84,8 @@ def lib():
         L.necsim_debug_int_peak.argtypes = [C.c_int, u32, vp, vp, vp]
         L.necsim_debug_next_event_poisson.argtypes = [vp, u64] + [vp] * 8 + [u64, vp]
         L.necsim_debug_poisson_table.argtypes = [vp] * 5
+        L.necsim_merge_workspace_size.argtypes = [u64, vp]
+        L.necsim_merge_species.argtypes = [vp, u64, vp, C.c_size_t, vp, vp, vp, vp]
         _lib = L
     return _lib
 
@@ -195,6 +198,12 @@ class Scenario:
                                           _hptr(h_labels)))
         return res
 
+    def result_tensors(self, res):
+        """CUDA views (no copy) of a Result's species table (uint8 [richness * 32]) and labels (int32 [n_lineages]) inside the workspace."""
+        ws = self._sim_ws
+        eo, lo = int(res.d_events) - ws.data_ptr(), int(res.d_labels) - ws.data_ptr()
+        return ws[eo:eo + int(res.richness) * 32], ws[lo:lo + int(res.n_lineages) * 4].view(_torch().int32)
+
     def simulate(self, seed, nu, mask=None, per_lineage=False, **param_kw):
         """Convenience: numpy mask in, numpy results out. dict(events, labels, richness, stats[, per_lineage, steps, state])."""
         torch = _torch()
@@ -269,6 +278,24 @@ def _read(ws, ptr, nbytes, dtype):
     off = int(ptr) - ws.data_ptr()
     assert 0 <= off and off + nbytes <= ws.numel(), "result pointer outside the workspace"
     return ws[off:off + nbytes].cpu().numpy().view(dtype).copy()
+
+
+def merge_species(d_events):
+    """necsim_merge_species: d_events = CUDA uint8 tensor holding n necsim_event records (the concatenated species tables
+    of isolated partitions). Returns (merged table as a CUDA uint8 tensor [richness * 32], map as a CUDA int64 tensor [n])."""
+    torch = _torch()
+    assert d_events.is_cuda and d_events.dtype == torch.uint8 and d_events.numel() % 32 == 0
+    n = d_events.numel() // 32
+    d_events = d_events.contiguous()
+    nbytes = C.c_size_t()
+    _check(lib().necsim_merge_workspace_size(n, C.byref(nbytes)))
+    ws = torch.empty(nbytes.value, dtype=torch.uint8, device="cuda")
+    out = torch.empty(n * 32, dtype=torch.uint8, device="cuda")
+    dmap = torch.empty(n, dtype=torch.int32, device="cuda")
+    rich = C.c_uint64()
+    _check(lib().necsim_merge_species(C.c_void_p(d_events.data_ptr()), n, C.c_void_p(ws.data_ptr()), ws.numel(), _stream_ptr(torch),
+                                      C.c_void_p(out.data_ptr()), C.c_void_p(dmap.data_ptr()), C.byref(rich)))
+    return out[: rich.value * 32], dmap.to(torch.int64)
 
 
 # ---- vectorised device primitives (test-only exports) ------------------------------------------------

@@ -17,6 +17,10 @@ def _worker(rank, world, port, out):
     from paper_2108_05815_b200 import dist as D
     seed = D.replica_seed(42, rank)
     times, units = D.aggregate([10.0 + 5.0 * rank, 3.0 - rank], [1000.0 * (rank + 1), 7.0])
+    # the exchange step of the partitioned path: variable-length tables, rank order, record offsets
+    tab = torch.full((32 * (rank + 2),), rank + 1, dtype=torch.uint8)
+    cat, offsets = D.gather_tables(tab)
+    assert offsets == [0, 2] and cat.numel() == 32 * 5 and bool((cat[:64] == 1).all()) and bool((cat[64:] == 2).all())
     out[rank] = (seed, times, units, D.throughput(units[0], times[0]))
     dist.barrier()
     dist.destroy_process_group()
@@ -33,6 +37,20 @@ def test_two_rank_aggregation():
         assert times == [15.0, 3.0]                 # max over ranks
         assert units == [3000.0, 14.0]              # sum over ranks
         assert abs(thr - 3000.0 / 0.015) < 1e-6
+
+
+def test_shard_mask_partitions_the_sample():
+    import numpy as np
+    from paper_2108_05815_b200 import dist as D
+    rng = np.random.default_rng(0)
+    mask = (rng.random(1000) < 0.3).astype(np.uint8)
+    for world in (1, 2, 7):
+        parts = [D.shard_mask(mask, 1000, r, world) for r in range(world)]
+        assert np.array_equal(np.sum(parts, axis=0), mask)                     # disjoint cover of the sample
+        firsts = [np.flatnonzero(p)[0] for p in parts if p.any()]
+        assert firsts == sorted(firsts)                                        # contiguous ranges in canonical order
+        assert max(int(p.sum()) for p in parts) - min(int(p.sum()) for p in parts) <= 1
+    assert np.array_equal(D.shard_mask(None, 10, 1, 2), np.array([0] * 5 + [1] * 5, np.uint8))
 
 
 def test_single_process_is_identity():
