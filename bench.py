@@ -97,6 +97,18 @@ class ClockSampler(threading.Thread):
         return dict(sm_mhz=float(np.median(sm)) if sm else None, sm_max_mhz=max(mx) if mx else None, reasons=sorted(reasons), samples=len(sm))
 
 
+def unique_events(cfg, args):
+    """Distinct events (loc, k, j) of the workload, counted by the oracle's full-size run (tests/golden/, written by
+    tests/golden/gen_golden.py from oracle/ only); raw events / this = redundant work left by the lossy dedup cache."""
+    f = os.path.join(ROOT, "tests", "golden", "full_configs_poisson.json" if args.sampler == "poisson" else "full_configs.json")
+    if args.small or not os.path.exists(f):
+        return None
+    for g in json.load(open(f)):
+        if g["name"] == cfg["name"]:
+            return g["unique_events"]
+    return None
+
+
 def reference_arm(args, cfg, name):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -224,6 +236,7 @@ def main():
                 "gpu_launches": int(launches),
                 "individuals_per_s": world * res.n_lineages / (ms / K * 1e-3),
                 "richness": int(res.richness), "epochs_per_step": epochs / K, "raw_events_per_step": ev / K,
+                "unique_events": unique_events(cfg, args), "redundancy": (ev / K) / unique_events(cfg, args) if unique_events(cfg, args) else None,
                 "phases": {"saturated": {"events_per_s": (ev - ev_tail) / max((sim_ms - tail_ms) * 1e-3, 1e-9), "ms_per_step": (sim_ms - tail_ms) / K,
                                          "events_per_step": (ev - ev_tail) / K, "kernel": "simulate_kernel (one lineage per lane)"},
                            "tail": {"events_per_s": ev_tail / max(tail_ms * 1e-3, 1e-9), "ms_per_step": tail_ms / K, "events_per_step": ev_tail / K,

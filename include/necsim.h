@@ -77,7 +77,7 @@ typedef struct necsim_sim_params {
     uint64_t max_steps;        /* 0 = unlimited; else a lineage stops after this many executed events
                                   ("unfinished": label 0xFFFFFFFF) -- the MODE-T throughput workload */
     uint32_t tail_threshold;   /* switch to the low-latency tail kernel when active lineages <= this; 0 = default */
-    uint32_t dedup_probe;      /* 0 = default; else 1 + log2 of the probe period: 1 = every event, 2 = every 2nd, 3 = every 4th,
+    uint32_t dedup_probe;      /* 0 = default (4); else 1 + log2 of the probe period: 1 = every event, 2 = every 2nd, 3 = every 4th,
                                   4 = every 8th event (chosen by a hash of the event identity) probes the cache (PAPER.md L942-946:
                                   the paper probes every step_slice steps) */
 } necsim_sim_params;

@@ -358,7 +358,7 @@ static int resolve_params(const necsim_scenario *scn, const necsim_sim_params *p
     if (r.max_steps > 0xFFFFFFFFull) return fail(NECSIM_ERR_INVALID_ARG, "max_steps must fit 32 bits");
     r.tail_threshold = p->tail_threshold;
     if (p->dedup_probe > 4) return fail(NECSIM_ERR_INVALID_ARG, "dedup_probe must be in [0, 4]");
-    r.probe_mask = p->dedup_probe ? ((1u << (p->dedup_probe - 1u)) - 1u) : 3u;   // default: every 4th event probes
+    r.probe_mask = p->dedup_probe ? ((1u << (p->dedup_probe - 1u)) - 1u) : 7u;   // default: every 8th event probes
     (void)scn;
     return NECSIM_OK;
 }
@@ -487,8 +487,8 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
     const u32 full_grid = rp.grid_blocks ? rp.grid_blocks : (u32)(occ * scn->sm_count);
     const u32 tail_grid = rp.grid_blocks ? rp.grid_blocks : (u32)(occ_tail * scn->sm_count);
     const u32 warps_per_block = rp.block_threads / 32u;
-    // one lineage per warp pays off once every active lineage can have a resident warp of its own
-    const u32 tail_threshold = rp.tail_threshold ? rp.tail_threshold : tail_grid * warps_per_block;
+    // one lineage per warp pays off from about two lineages per resident warp downwards (measured on C5: sweep in DESIGN.md 5)
+    const u32 tail_threshold = rp.tail_threshold ? rp.tail_threshold : 2u * tail_grid * warps_per_block;
     const u32 full_cache_mask = rp.dedup ? ((1u << rp.dedup_log2_slots) - 1u) : 0u;
     u32 active = n_sampled, k_start = 0;
     uint4 *q_in = qa, *q_out = qb;
@@ -501,7 +501,7 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
         else {
             // tail epochs are latency-bound and their warps stay roughly synchronous in simulated time: longer epochs cost
             // no dedup hits and amortise the end-of-epoch imbalance (spread of events per lineage ~ 1/sqrt(span))
-            const double w = (double)rp.epoch_events * ((active <= tail_threshold && params_default_epoch) ? 8.0 : 1.0);
+            const double w = (double)rp.epoch_events * ((active <= tail_threshold && params_default_epoch) ? 64.0 : 1.0);
             double span = w / ((double)active * scn->mu_max);
             u64 sp = span < 1.0 ? 1ull : (span > 1e9 ? 1000000000ull : (u64)span);
             u64 h = (u64)k_start + sp;
