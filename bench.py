@@ -243,17 +243,18 @@ def main():
                                     "kernel": "tail_kernel (one lineage per warp; bound by event latency x chain length, DESIGN.md 6.3)"}},
                 "roofline": {"bound": "alu", "kernel": dom_name + " (all its launches of the timed steps)", "achieved": achieved / 1e12, "peak": peak / 1e12,
                              "unit": "Tinstr/s", "frac": achieved / peak,
-                             # dram__bytes_read.sum + dram__bytes_write.sum of one tail_kernel launch (C5, 61st tail epoch), ncu --set full,
-                             # profiles/r1_ncu_tail_kernel_c5.md; caches are flushed per ncu replay pass, so this is an upper bound
-                             "traffic": 67198464 if (name == "c5" and dom_name == "tail_kernel") else None,
+                             # dram__bytes_read.sum + dram__bytes_write.sum of one tail_kernel launch (C5, exponential sampler, 13th tail
+                             # epoch, 50 ms), ncu --set full, profiles/r1_ncu_tail_kernel_c5.md; caches are flushed per ncu replay pass,
+                             # so this is an upper bound
+                             "traffic": 1422595056 if (name == "c5" and dom_name == "tail_kernel" and args.sampler == "exp") else None,
                              "instr_per_event": I_EVENT[name],
                              "note": "latency-bound by construction: one lineage per warp walks a serial chain of ~ln(S)/nu events (DESIGN.md 6.3)",
                              "peak_source": "derived: SMs x 4 schedulers x 32 lanes x sm_max_mhz (DESIGN.md section 6)",
                              "measured_int_peaks_Tinstr_s": {k: v / 1e12 for k, v in int_meas.items()}},
                 "mode_t": {"value": mode_t, "unit": UNIT, "what": "dedup off, 200 events per lineage, saturated machine",
                            "roofline_frac": mode_t * I_EVENT[name] / peak,
-                           "ncu": "profiles/r1_ncu_simulate_kernel_c5_modeT.md: issue slots 71 % active, ALU pipe 65 %, FMA pipe 18 % of peak, "
-                                  "22.2 of 32 lanes per instruction, L2 hit 98.5 %"}}
+                           "ncu": "profiles/r1_ncu_simulate_kernel_c5_modeT.md (exponential sampler): issue slots 70 % active, ALU pipe 66 %, "
+                                  "FMA pipe 18 % of peak, 22.1 of 32 lanes per instruction, L2 hit 98.6 %"}}
         if not args.no_cpu_baseline and world == 1:
             v, dt, n_ev, desc = run_oracle_sample(cfg, name)
             line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc, "seconds": dt}
