@@ -257,8 +257,9 @@ __global__ void __launch_bounds__(256) simulate_kernel(const ScenarioDev sc, con
                 for (u32 q = 0; q < 4u && j < sh; ++q) {   // up to four points per pass: amortises the phase scheduling
                     j += 1; X += NS_GAMMA;
                     const u64 f = poisson_offset(X);
-                    const bool kept = PERCELL ? poisson_kept(X, Cm) : true;
-                    if (kept && (i64)f > f_last && (att == 0u || f < T)) { T = f; att = j; }
+                    if ((i64)f > f_last && (att == 0u || f < T)) {         // a better candidate: only now pay for the thinning draw
+                        if (!PERCELL || poisson_kept(X, Cm)) { T = f; att = j; }
+                    }
                 }
                 if (j >= sh) {                             // interval scanned
                     if (att) { X -= (u64)(sh - att) * NS_GAMMA; j = att; att = 0; st = NS_ST_EVENT; }
