@@ -27,17 +27,19 @@ from paper_2108_05815_b200 import dist as D    # noqa: E402
 
 METRIC = "lineage_events_per_s"
 UNIT = "events/s"
-MAKERS = dict(c1=I.c1_nonspatial, c2=I.c2_implicit, c3=I.c3_matrix, c4=I.c4_gaussian, c5=I.c5_stress)
+MAKERS = dict(c1=I.c1_nonspatial, c2=I.c2_implicit, c3=I.c3_matrix, c4=I.c4_gaussian, c5=I.c5_stress, c6=I.c6_bigdeme)
 SMALL = dict(zip(("c1", "c2", "c3", "c4", "c5"), range(5)))
 # Algorithmic integer instructions per executed event (minimal 32-bit instruction sequence of
 # each primitive, weighted by the expected number of draws per event at mu = 2 and the measured attempts per event).
-I_EVENT = dict(c1=230, c2=232, c3=252, c4=263, c5=272)
+I_EVENT = dict(c1=230, c2=232, c3=252, c4=263, c5=272, c6=259)   # c6: one attempt + 5 % resampling, index draw, deme32 gather
 # issue-slot peak: 148 SMs x 4 schedulers x 32 lanes x 1 instr/clk x sm_max_mhz (B300_MICROARCH "Pipe rates")
 def alu_peak(sm_count, sm_mhz):
     return sm_count * 4 * 32 * sm_mhz * 1e6
 
 
 def make_cfg(name, small):
+    if name == "c6":                                     # SURVEY NEXT-4 shape; --small: demes of ~360
+        return I.c6_bigdeme(deme_mean=360, sample=0.05) if small else I.c6_bigdeme()
     return I.small_configs()[SMALL[name]] if small else MAKERS[name]()
 
 

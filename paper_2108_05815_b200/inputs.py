@@ -108,6 +108,23 @@ def c5_stress(side=4096, deme=4, sigma=5.0, nu=1e-6, sample=0.1, seed=42, noise_
                  nu=nu, seed=seed, mask=mask)
 
 
+def c6_bigdeme(width=180, height=64, deme_mean=36_000, sigma=2.0, nu=1e-3, sample=0.01, seed=42, deme_seed=5, mask_seed=6):
+    """SURVEY NEXT-4 workload shape: few cells with enormous demes (the paper's fg0size12 map is 180 x 64 cells holding
+    4.2e9 individuals; this stand-in keeps the grid and scales the demes so that the sample mask stays
+    below 1 GB): log-normal deme sizes, 5 % non-habitat cells, rounded Gaussian dispersal, a thin uniform sample."""
+    rng = np.random.Generator(np.random.PCG64(deme_seed))
+    n = width * height
+    deme = np.maximum(rng.lognormal(mean=math.log(deme_mean) - 0.125, sigma=0.5, size=n), 300.0).astype(np.uint32)
+    deme[rng.random(n) < 0.05] = 0
+    n_ind = int(deme.astype(np.uint64).sum())
+    rng2 = np.random.Generator(np.random.PCG64(mask_seed))
+    mask = (rng2.random(n_ind) < sample).astype(np.uint8)
+    if mask.sum() == 0:
+        mask[0] = 1
+    return _base("C6-bigdeme-%dx%d" % (width, height), EXPLICIT_GAUSSIAN, width=width, height=height, deme=deme, sigma=sigma,
+                 nu=nu, seed=seed, mask=mask)
+
+
 def n_individuals(cfg):
     if cfg["kind"] == SPATIALLY_IMPLICIT:
         return int(cfg["local_size"])

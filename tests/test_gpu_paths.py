@@ -71,6 +71,19 @@ def test_rare_paths(ns, O, I, kernel):
         sc.close()
 
 
+def test_bigdeme_shape_next4(ns, O, I):
+    """few cells with enormous demes (every deme >= 255: the deme32 gather on every dispersal)."""
+    cfg = I.c6_bigdeme(width=24, height=21, deme_mean=2000, sigma=1.0, nu=5e-3, sample=0.02, seed=3)
+    kw = I.scenario_kwargs(cfg)
+    ref = O.Scenario(**kw).simulate(cfg["seed"], cfg["nu"], cfg["mask"], dedup=True)
+    sc = ns.Scenario(**kw)
+    for knobs in (dict(), dict(tail_threshold=1), dict(tail_threshold=0xFFFFFFFF)):
+        same(sc.simulate(cfg["seed"], cfg["nu"], cfg["mask"], **knobs), ref)
+    sc.close()
+    kw1 = dict(kw, sampler=1)
+    same(ns.Scenario(**kw1).simulate(cfg["seed"], cfg["nu"], cfg["mask"]), O.Scenario(**kw1).simulate(cfg["seed"], cfg["nu"], cfg["mask"], dedup=True))
+
+
 @pytest.mark.parametrize("kernel", sorted(KERNELS))
 def test_step_cap_with_dedup_and_no_migration(ns, O, I, kernel):
     kw = dict(kind=I.SPATIALLY_IMPLICIT, local_size=300, meta_size=1000, migration=0.0)
