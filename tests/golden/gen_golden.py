@@ -70,10 +70,13 @@ def configs(which, fname, epoch_events=0, sampler=0):
 
 
 if __name__ == "__main__":
-    rng_vectors()
-    neglog_vectors()
-    configs(I.small_configs(), "small_configs.json")
+    if not any(a.startswith("--full") for a in sys.argv[1:]):
+        rng_vectors()
+        neglog_vectors()
+        configs(I.small_configs(), "small_configs.json")
     if "--full" in sys.argv:
         configs(I.full_configs(), "full_configs.json", epoch_events=50_000_000)
+    if "--full-c6" in sys.argv:           # SURVEY NEXT-4 big-deme workload at full size (about 10 minutes of CPU)
+        configs([I.c6_bigdeme()], "full_config_c6.json", epoch_events=50_000_000)
     if "--full-poisson" in sys.argv:      # the Poisson event-time sampler on the same five configs
         configs(I.full_configs(), "full_configs_poisson.json", epoch_events=50_000_000, sampler=1)

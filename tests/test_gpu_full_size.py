@@ -69,3 +69,21 @@ def test_full_config_matches_oracle(O, idx, sampler):
         assert (int(e["loc"]), int(e["k"]), int(e["j"]), int(e["f"])) == (int(mine["loc"]), int(mine["k"]), int(mine["j"]), int(mine["f"]))
         assert e["time"] == mine["time"]
     sc.close()
+
+
+def test_bigdeme_full_size_matches_oracle(O):
+    """SURVEY NEXT-4 workload (bench.py --config c6) at full size against tests/golden/full_config_c6.json (oracle only)."""
+    from paper_2108_05815_b200 import inputs as I, necsim as ns
+    f = os.path.join(HERE, "golden", "full_config_c6.json")
+    if not os.path.exists(f):
+        pytest.skip("full_config_c6.json not generated")
+    g = json.load(open(f))[0]
+    cfg = I.c6_bigdeme()
+    assert g["name"] == cfg["name"]
+    sc = ns.Scenario(**I.scenario_kwargs(cfg))
+    got = sc.simulate(cfg["seed"], cfg["nu"], cfg["mask"])
+    assert got["richness"] == g["richness"] and len(got["labels"]) == g["n_sampled"]
+    assert [int(v) for v in got["labels"][:16]] == g["labels_head"]
+    assert digest(got) == g["digest"]
+    assert got["stats"]["n_events_raw"] >= g["unique_events"]
+    sc.close()
