@@ -105,7 +105,9 @@ def unique_events(cfg, args):
     f = os.path.join(ROOT, "tests", "golden", "full_configs_poisson.json" if args.sampler == "poisson" else "full_configs.json")
     if args.small or not os.path.exists(f):
         return None
-    for g in json.load(open(f)):
+    extra = os.path.join(ROOT, "tests", "golden", "full_config_c6.json")
+    records = json.load(open(f)) + (json.load(open(extra)) if (args.sampler == "exp" and os.path.exists(extra)) else [])
+    for g in records:
         if g["name"] == cfg["name"]:
             return g["unique_events"]
     return None
