@@ -80,6 +80,11 @@ typedef struct necsim_sim_params {
     uint32_t dedup_probe;      /* 0 = default (4); else 1 + log2 of the probe period: 1 = every event, 2 = every 2nd, 3 = every 4th,
                                   4 = every 8th event (chosen by a hash of the event identity) probes the cache (PAPER.md L942-946:
                                   the paper probes every step_slice steps) */
+    uint32_t record_events;    /* 1 = also produce the full event stream (PAPER.md 6.2 L813-906, 7.1.3 L958-967):
+                                  every distinct executed event (speciation and dispersal), sorted by (k, f, loc, j) */
+    uint32_t reserved;
+    uint64_t event_ring_capacity;   /* records one epoch may produce (incl. redundant ones); 0 = 2^24. Each takes 36 bytes of workspace */
+    uint64_t event_stream_capacity; /* distinct events of the whole run; 0 = 2^26. Each takes 24 bytes of workspace */
 } necsim_sim_params;
 
 /* One distinct speciation event = one species. 32 bytes. */
@@ -115,6 +120,11 @@ typedef struct necsim_result {
     float ms_simulate_tail;       /* of which tail epochs */
     float ms_total;               /* device time of the whole call */
     uint32_t n_kernel_launches;   /* kernels this call launched (memsets and copies not counted) */
+    /* full event stream (record_events = 1), DEVICE SoA inside the workspace, [n_stream_events], sorted by (k, f, loc, j):
+     * origin location, interval, ordinal, offset, and the parent's location (0xFFFFFFFF = the event is a speciation) */
+    const uint32_t *d_stream_loc, *d_stream_k, *d_stream_j, *d_stream_loc2;
+    const uint64_t *d_stream_f;
+    uint64_t n_stream_events;
 } necsim_result;
 
 typedef struct necsim_scenario necsim_scenario;

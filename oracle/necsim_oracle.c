@@ -476,6 +476,20 @@ static int cmp_event(const void *pa, const void *pb) {
     return 0;
 }
 
+/* Optional sink for the full event stream (paper 6.2 L813-906: Speciation and Dispersal events): every
+ * executed event is appended as (origin loc, k, j, f, parent loc or 0xFFFFFFFF for a speciation). With exact dedup each
+ * distinct event appears once; the caller sorts by (k, f, loc, j) -- the paper's stream order (event_time, L903, L966). */
+static u32 *g_sink_loc, *g_sink_k, *g_sink_j, *g_sink_loc2; static u64 *g_sink_f; static u64 g_sink_cap, *g_sink_n;
+void orc_set_event_sink(u32 *loc, u32 *k, u32 *j, u64 *f, u32 *loc2, u64 cap, u64 *n) {
+    g_sink_loc = loc; g_sink_k = k; g_sink_j = j; g_sink_f = f; g_sink_loc2 = loc2; g_sink_cap = cap; g_sink_n = n;
+    if (n) *n = 0;
+}
+static void sink_event(u32 loc, u32 k, u32 j, u64 f, u32 loc2) {
+    if (!g_sink_n) return;
+    u64 i = (*g_sink_n)++;
+    if (i < g_sink_cap) { g_sink_loc[i] = loc; g_sink_k[i] = k; g_sink_j[i] = j; g_sink_f[i] = f; g_sink_loc2[i] = loc2; }
+}
+
 /*
  * mask: n_sampleable bytes (NULL = all sampled). dedup: 0 off, 1 exact.
  * epoch_events: 0 = one epoch (horizon = never); else the horizon advances so that about that many
@@ -553,11 +567,13 @@ int orc_simulate(const orc_scenario *sc, u64 seed, double nu, const uint8_t *mas
                 if (meta_or_plain && bern(orc_draw_spec(s, j), thr_nu)) {
                     state[id] = 1; active--;
                     term[id].loc = loc[id]; term[id].k = kk[id]; term[id].j = j; term[id].f = T;
+                    sink_event(loc[id], kk[id], j, T, 0xFFFFFFFFu);
                     break;
                 }
                 u32 l2, c2;
                 r = disperse(sc, thr_m, s, j, c, &l2, &c2, &stats->resample_attempts);
                 if (r != 0) { rc = r; break; }
+                sink_event(loc[id], kk[id], j, T, l2);
                 loc[id] = l2; cell[id] = c2;
                 if (max_steps && steps[id] >= max_steps) {
                     state[id] = 3; active--; stats->n_unfinished++;

@@ -173,6 +173,26 @@ class Scenario:
         if rc != 0: raise RuntimeError("disperse rc=%d" % rc)
         return out.value
 
+    def simulate_stream(self, seed, nu, mask=None, capacity=10_000_000, **kw):
+        """simulate() with exact dedup plus the full event stream: dict gains `stream`, a structured array
+        (loc, k, j, f, loc2) of the distinct executed events sorted by (k, f, loc, j); loc2 = 0xFFFFFFFF marks a speciation."""
+        L = lib()
+        L.orc_set_event_sink.restype = None; L.orc_set_event_sink.argtypes = [C.c_void_p] * 5 + [C.c_uint64, C.c_void_p]
+        a = [np.zeros(capacity, np.uint32) for _ in range(3)]; f = np.zeros(capacity, np.uint64); l2 = np.zeros(capacity, np.uint32)
+        n = C.c_uint64()
+        L.orc_set_event_sink(_ptr(a[0]), _ptr(a[1]), _ptr(a[2]), _ptr(f), _ptr(l2), capacity, C.byref(n))
+        try:
+            out = self.simulate(seed, nu, mask, dedup=True, **kw)
+        finally:
+            L.orc_set_event_sink(None, None, None, None, None, 0, None)
+        if n.value > capacity:
+            raise RuntimeError("event stream capacity exceeded: %d" % n.value)
+        m = n.value
+        st = np.zeros(m, dtype=[("loc", "<u4"), ("k", "<u4"), ("j", "<u4"), ("f", "<u8"), ("loc2", "<u4")])
+        st["loc"], st["k"], st["j"], st["f"], st["loc2"] = a[0][:m], a[1][:m], a[2][:m], f[:m], l2[:m]
+        out["stream"] = st[np.lexsort((st["j"], st["loc"], st["f"], st["k"]))]
+        return out
+
     def simulate(self, seed, nu, mask=None, dedup=True, epoch_events=0, max_steps=0, per_lineage=False):
         """Returns dict(events, labels, richness, stats[, per_lineage, steps])."""
         n_ind = self.n_individuals

@@ -338,8 +338,8 @@ extern "C" int necsim_destroy(necsim_scenario *scn) {
 // ---------------------------------------------------------------------------------------------------
 struct ResolvedParams {
     u32 block_threads, grid_blocks, dedup_log2_slots, tail_threshold, probe_mask;
-    bool dedup;
-    u64 epoch_events, max_steps;
+    bool dedup, record;
+    u64 epoch_events, max_steps, ring_cap, stream_cap;
 };
 
 static int resolve_params(const necsim_scenario *scn, const necsim_sim_params *p, ResolvedParams &r) {
@@ -357,6 +357,10 @@ static int resolve_params(const necsim_scenario *scn, const necsim_sim_params *p
     r.max_steps = p->max_steps;
     if (r.max_steps > 0xFFFFFFFFull) return fail(NECSIM_ERR_INVALID_ARG, "max_steps must fit 32 bits");
     r.tail_threshold = p->tail_threshold;
+    r.record = p->record_events != 0;
+    r.ring_cap = r.record ? (p->event_ring_capacity ? p->event_ring_capacity : (1ull << 24)) : 0;
+    r.stream_cap = r.record ? (p->event_stream_capacity ? p->event_stream_capacity : (1ull << 26)) : 0;
+    if (r.ring_cap >= (1ull << 32)) return fail(NECSIM_ERR_INVALID_ARG, "event_ring_capacity must be < 2^32");
     if (p->dedup_probe > 4) return fail(NECSIM_ERR_INVALID_ARG, "dedup_probe must be in [0, 4]");
     r.probe_mask = p->dedup_probe ? ((1u << (p->dedup_probe - 1u)) - 1u) : 7u;   // default: every 8th event probes
     (void)scn;
@@ -365,7 +369,8 @@ static int resolve_params(const necsim_scenario *scn, const necsim_sim_params *p
 
 struct SimLayout {
     size_t off_ctr, off_qa, off_qb, off_cache, off_term_loc, off_term_k, off_term_j, off_steps, off_parent, off_ring, off_term_f,
-        off_state, off_events, off_labels, off_species, off_perm_a, off_perm_b, off_flag, off_hist, off_chunk, off_mask, total;
+        off_state, off_events, off_labels, off_species, off_perm_a, off_perm_b, off_flag, off_hist, off_chunk, off_mask,
+        off_rec_loc, off_rec_k, off_rec_j, off_rec_l2, off_rec_f, off_st_loc, off_st_k, off_st_j, off_st_l2, off_st_f, total;
     u32 n_chunks, sort_blocks;
 };
 
@@ -373,7 +378,8 @@ static void sim_layout(u64 n_individuals, u64 cap, const ResolvedParams &rp, Sim
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off = align256(off + bytes); return o; };
     L.n_chunks = (u32)((n_individuals + NS_CHUNK - 1) / NS_CHUNK);
-    L.sort_blocks = (u32)((cap + NS_SORT_TILE - 1) / NS_SORT_TILE);
+    const u64 sort_n = std::max<u64>(cap, rp.ring_cap);      // the sort scratch serves the species sort and the per-epoch stream sort
+    L.sort_blocks = (u32)((sort_n + NS_SORT_TILE - 1) / NS_SORT_TILE);
     if (L.sort_blocks == 0) L.sort_blocks = 1;
     L.off_ctr = take(sizeof(SimCounters));
     L.off_qa = take(16 * cap); L.off_qb = take(16 * cap);
@@ -381,9 +387,13 @@ static void sim_layout(u64 n_individuals, u64 cap, const ResolvedParams &rp, Sim
     L.off_term_loc = take(4 * cap); L.off_term_k = take(4 * cap); L.off_term_j = take(4 * cap); L.off_steps = take(4 * cap);
     L.off_parent = take(4 * cap); L.off_ring = take(4 * cap); L.off_term_f = take(8 * cap); L.off_state = take(cap);
     L.off_events = take(sizeof(necsim_event) * cap); L.off_labels = take(4 * cap); L.off_species = take(4 * cap);
-    L.off_perm_a = take(4 * cap); L.off_perm_b = take(4 * cap); L.off_flag = take(4 * cap);
+    L.off_perm_a = take(4 * sort_n); L.off_perm_b = take(4 * sort_n); L.off_flag = take(4 * sort_n);
     L.off_hist = take(4 * 256 * (size_t)L.sort_blocks); L.off_chunk = take(4 * ((size_t)L.n_chunks + 1));
     L.off_mask = take(n_individuals);
+    L.off_rec_loc = take(4 * rp.ring_cap); L.off_rec_k = take(4 * rp.ring_cap); L.off_rec_j = take(4 * rp.ring_cap);
+    L.off_rec_l2 = take(4 * rp.ring_cap); L.off_rec_f = take(8 * rp.ring_cap);
+    L.off_st_loc = take(4 * rp.stream_cap); L.off_st_k = take(4 * rp.stream_cap); L.off_st_j = take(4 * rp.stream_cap);
+    L.off_st_l2 = take(4 * rp.stream_cap); L.off_st_f = take(8 * rp.stream_cap);
     L.total = off;
 }
 
@@ -400,22 +410,23 @@ extern "C" int necsim_simulate_workspace_size(const necsim_scenario *scn, uint64
 }
 
 typedef void (*EpochKernel)(const ScenarioDev, const SimBuffers, const EpochArgs);
-template <int KIND, bool PERCELL, int SAMP>
-static EpochKernel pick_kernel3(bool dedup, bool tail) {
-    if (tail) return dedup ? (EpochKernel)tail_kernel<KIND, true, PERCELL, SAMP> : (EpochKernel)tail_kernel<KIND, false, PERCELL, SAMP>;
-    return dedup ? (EpochKernel)simulate_kernel<KIND, true, PERCELL, SAMP> : (EpochKernel)simulate_kernel<KIND, false, PERCELL, SAMP>;
+template <int KIND, bool PERCELL, int SAMP, bool REC>
+static EpochKernel pick_kernel4(bool dedup, bool tail) {
+    if (tail) return dedup ? (EpochKernel)tail_kernel<KIND, true, PERCELL, SAMP, REC> : (EpochKernel)tail_kernel<KIND, false, PERCELL, SAMP, REC>;
+    return dedup ? (EpochKernel)simulate_kernel<KIND, true, PERCELL, SAMP, REC> : (EpochKernel)simulate_kernel<KIND, false, PERCELL, SAMP, REC>;
 }
 template <int KIND, bool PERCELL>
-static EpochKernel pick_kernel2(int sampler, bool dedup, bool tail) {
-    return sampler ? pick_kernel3<KIND, PERCELL, 1>(dedup, tail) : pick_kernel3<KIND, PERCELL, 0>(dedup, tail);
+static EpochKernel pick_kernel2(int sampler, bool rec, bool dedup, bool tail) {
+    if (sampler) return rec ? pick_kernel4<KIND, PERCELL, 1, true>(dedup, tail) : pick_kernel4<KIND, PERCELL, 1, false>(dedup, tail);
+    return rec ? pick_kernel4<KIND, PERCELL, 0, true>(dedup, tail) : pick_kernel4<KIND, PERCELL, 0, false>(dedup, tail);
 }
 // per-cell turnover exists for the explicit kinds only
-static EpochKernel pick_kernel(int kind, bool percell, int sampler, bool dedup, bool tail) {
+static EpochKernel pick_kernel(int kind, bool percell, int sampler, bool rec, bool dedup, bool tail) {
     switch (kind) {
-    case 0: return pick_kernel2<0, false>(sampler, dedup, tail);
-    case 1: return pick_kernel2<1, false>(sampler, dedup, tail);
-    case 2: return percell ? pick_kernel2<2, true>(sampler, dedup, tail) : pick_kernel2<2, false>(sampler, dedup, tail);
-    default: return percell ? pick_kernel2<3, true>(sampler, dedup, tail) : pick_kernel2<3, false>(sampler, dedup, tail);
+    case 0: return pick_kernel2<0, false>(sampler, rec, dedup, tail);
+    case 1: return pick_kernel2<1, false>(sampler, rec, dedup, tail);
+    case 2: return percell ? pick_kernel2<2, true>(sampler, rec, dedup, tail) : pick_kernel2<2, false>(sampler, rec, dedup, tail);
+    default: return percell ? pick_kernel2<3, true>(sampler, rec, dedup, tail) : pick_kernel2<3, false>(sampler, rec, dedup, tail);
     }
 }
 static int occupancy_for(EpochKernel fn, u32 block) {
@@ -444,6 +455,11 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
     u32 *labels = (u32 *)(base + L.off_labels), *species_of = (u32 *)(base + L.off_species);
     u32 *perm_a = (u32 *)(base + L.off_perm_a), *perm_b = (u32 *)(base + L.off_perm_b), *flag = (u32 *)(base + L.off_flag);
     u32 *hist = (u32 *)(base + L.off_hist), *chunk = (u32 *)(base + L.off_chunk);
+    bf.rec_loc = (u32 *)(base + L.off_rec_loc); bf.rec_k = (u32 *)(base + L.off_rec_k); bf.rec_j = (u32 *)(base + L.off_rec_j);
+    bf.rec_loc2 = (u32 *)(base + L.off_rec_l2); bf.rec_f = (u64 *)(base + L.off_rec_f); bf.rec_cap = (u32)rp.ring_cap;
+    u32 *st_loc = (u32 *)(base + L.off_st_loc), *st_k = (u32 *)(base + L.off_st_k), *st_j = (u32 *)(base + L.off_st_j), *st_l2 = (u32 *)(base + L.off_st_l2);
+    u64 *st_f = (u64 *)(base + L.off_st_f);
+    u64 stream_n = 0;
     SimCounters *hc = scn->h_ctr;
 
     CU(cudaEventRecord(scn->ev[0], st));
@@ -479,8 +495,8 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
     ep.thr_nu = thr53(nu);
     ep.thr_m = thr53(scn->migration);
     ep.max_steps = (u32)rp.max_steps;
-    const EpochKernel fn_main = pick_kernel(sd.kind, sd.per_cell_turnover != 0, (int)sd.sampler, rp.dedup, false);
-    const EpochKernel fn_tail = pick_kernel(sd.kind, sd.per_cell_turnover != 0, (int)sd.sampler, rp.dedup, true);
+    const EpochKernel fn_main = pick_kernel(sd.kind, sd.per_cell_turnover != 0, (int)sd.sampler, rp.record, rp.dedup, false);
+    const EpochKernel fn_tail = pick_kernel(sd.kind, sd.per_cell_turnover != 0, (int)sd.sampler, rp.record, rp.dedup, true);
     const int occ = occupancy_for(fn_main, rp.block_threads);
     const int occ_tail = occupancy_for(fn_tail, rp.block_threads);
     ep.probe_mask = rp.probe_mask;
@@ -498,15 +514,20 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
     const bool params_default_epoch = !(params && params->epoch_events);
     while (active > 0) {
         u32 k_stop;
-        if (rp.epoch_events == 0) k_stop = 0xFFFFFFFFu;
+        if (rp.epoch_events == 0 && !rp.record) k_stop = 0xFFFFFFFFu;
         else {
             // (i) tail epochs are latency-bound and their warps stay roughly synchronous in simulated time: longer epochs cost
             // no dedup hits and amortise the end-of-epoch imbalance (spread of events per lineage ~ 1/sqrt(span))
             // (ii) every epoch costs each active lineage a queue round trip and a re-prime, and the kernel a ragged end: by
             // default an epoch holds at least NS_MIN_EVENTS_PER_LINEAGE events per lineage however many lineages there are
             // (measured: 2.9x on the big-deme workload, +5 % redundant events)
-            double w = (double)rp.epoch_events * ((active <= tail_threshold && params_default_epoch) ? 64.0 : 1.0);
-            if (params_default_epoch) w = std::max(w, (double)active * NS_MIN_EVENTS_PER_LINEAGE);
+            double w = rp.epoch_events ? (double)rp.epoch_events * ((active <= tail_threshold && params_default_epoch) ? 64.0 : 1.0) : 1e30;
+            if (params_default_epoch && rp.epoch_events) w = std::max(w, (double)active * NS_MIN_EVENTS_PER_LINEAGE);
+            if (rp.record) {   // (iii) the epoch's events (with the redundant ones) must fit the stream ring
+                w = std::min(w, 0.5 * (double)rp.ring_cap);
+                if ((double)active * scn->mu_max > 0.75 * (double)rp.ring_cap)
+                    return fail(NECSIM_ERR_CAPACITY, "event_ring_capacity too small for one interval of the active lineages");
+            }
             double span = w / ((double)active * scn->mu_max);
             u64 sp = span < 1.0 ? 1ull : (span > 1e9 ? 1000000000ull : (u64)span);
             u64 h = (u64)k_start + sp;
@@ -530,6 +551,7 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
         // a few thousand lineages need few slots: keep the tail's cache footprint (2 MiB) inside L2 next to the tables
         bf.cache_mask = rp.dedup ? (tail ? std::min(full_cache_mask, (1u << 17) - 1u) : full_cache_mask) : 0u;
         CU(cudaMemsetAsync(bf.ctr, 0, 8, st));   // q_head, q_out
+        if (rp.record) CU(cudaMemsetAsync(&bf.ctr->n_rec, 0, 4, st));
         CU(cudaEventRecord(scn->ev[2], st));
         (tail ? fn_tail : fn_main)<<<grid, rp.block_threads, 0, st>>>(sd, bf, ep);
         cudaError_t ce = cudaGetLastError();
@@ -544,6 +566,41 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
         if (tail) { ms_tail += ms; ++n_tail_epochs; ev_tail += hc->n_events - ev_before; }
         ev_before = hc->n_events;
         if (hc->error) return fail(NECSIM_ERR_CAPACITY, "interval index overflowed 2^32 or dispersal resampling exhausted");
+        if (rp.record && hc->n_rec > 0) {
+            // NEXT-3: this epoch's records -> sorted by (k, f, loc, j), duplicates dropped, appended to the stream. Epochs are
+            // disjoint windows of simulated time, so the concatenation is globally ordered (Water-Level, G.1 L2157-2187).
+            const u32 nr = hc->n_rec;
+            if (nr > rp.ring_cap) return fail(NECSIM_ERR_CAPACITY, "event ring overflowed: raise event_ring_capacity");
+            SimBuffers vb = bf;
+            vb.term_loc = bf.rec_loc; vb.term_k = bf.rec_k; vb.term_j = bf.rec_j; vb.term_f = bf.rec_f;
+            const u32 nb = (nr + NS_SORT_TILE - 1) / NS_SORT_TILE, g256 = (nr + 255) / 256;
+            iota_kernel<<<g256, 256, 0, st>>>(perm_a, nr);
+            u32 *src = perm_a, *dst = perm_b;
+            const u32 kmax = k_stop - 1u, lmax = (u32)(sd.n_locations - 1);
+            for (u32 b = 0; b < 18; ++b) {   // j: two bytes (ordinals stay far below 2^16 for mu <= 64), loc and k: the bytes in use
+                bool needed;
+                if (b < 4) needed = b < 2;
+                else if (b < 8) needed = (lmax >> (8 * (b - 4))) != 0;
+                else if (b < 14) needed = true;
+                else needed = (kmax >> (8 * (b - 14))) != 0;
+                if (!needed) continue;
+                radix_hist_kernel<<<nb, 256, 0, st>>>(vb, src, nr, b, hist, nb);
+                scan_exclusive_kernel<<<1, 1024, 0, st>>>(hist, 256 * nb, NULL);
+                radix_scatter_kernel<<<nb, 256, 0, st>>>(vb, src, dst, nr, b, hist, nb);
+                std::swap(src, dst);
+                n_launch += 3;
+            }
+            unique_flag_kernel<<<g256, 256, 0, st>>>(vb, src, nr, flag);
+            scan_exclusive_kernel<<<1, 1024, 0, st>>>(flag, nr, &bf.ctr->q_head);   // q_head reused: distinct events of the epoch
+            stream_write_kernel<<<g256, 256, 0, st>>>(vb, bf.rec_loc2, src, nr, flag, stream_n, rp.stream_cap, st_loc, st_k, st_j, st_f, st_l2);
+            n_launch += 4;
+            CU(cudaGetLastError());
+            u32 heads = 0;
+            CU(cudaMemcpyAsync(&heads, &bf.ctr->q_head, 4, cudaMemcpyDeviceToHost, st));
+            CU(cudaStreamSynchronize(st));
+            stream_n += heads;
+            if (stream_n > rp.stream_cap) return fail(NECSIM_ERR_CAPACITY, "event stream overflowed: raise event_stream_capacity");
+        }
         active = hc->q_out;
         std::swap(q_in, q_out);
         k_start = k_stop;
@@ -598,6 +655,10 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
     out->n_events_raw = hc->n_events; out->n_culled = hc->n_culled; out->n_speciation_raw = n_spec; out->n_epochs = n_epochs;
     out->resample_attempts = hc->resamples; out->ms_simulate = ms_sim; out->ms_simulate_tail = ms_tail; out->n_tail_epochs = n_tail_epochs; out->n_events_tail = ev_tail;
     out->ms_total = ms_total; out->n_kernel_launches = n_launch;
+    if (rp.record) {
+        out->d_stream_loc = st_loc; out->d_stream_k = st_k; out->d_stream_j = st_j; out->d_stream_loc2 = st_l2; out->d_stream_f = st_f;
+        out->n_stream_events = stream_n;
+    }
     return NECSIM_OK;
 }
 

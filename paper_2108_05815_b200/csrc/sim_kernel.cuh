@@ -169,12 +169,26 @@ __device__ __forceinline__ void poisson_stage(const ScenarioDev &sc, u64 *sP, un
     __syncthreads();
 }
 
+// Appends one executed event to the epoch's stream ring (paper 6.2 L813-847: Speciation / Dispersal events).
+// Warp-aggregated: the lanes that call this together share one atomicAdd.
+__device__ __forceinline__ void record_event(const SimBuffers &bf, u32 loc, u32 k, u32 j, u64 f, u32 loc2) {
+    const u32 mask = __activemask();
+    const u32 lane = threadIdx.x & 31u;
+    const int leader = __ffs(mask) - 1;
+    u32 base = 0;
+    if ((int)lane == leader) base = atomicAdd(&bf.ctr->n_rec, (u32)__popc(mask));
+    base = __shfl_sync(mask, base, leader);
+    const u32 idx = base + __popc(mask & lanemask_lt());
+    if (idx < bf.rec_cap) { bf.rec_loc[idx] = loc; bf.rec_k[idx] = k; bf.rec_j[idx] = j; bf.rec_f[idx] = f; bf.rec_loc2[idx] = loc2; }
+}
+
 #define NS_ST_IDLE 0u
 #define NS_ST_SEARCH 1u     // needs draws of the event-time search (re-primes first when `need_prime`)
 #define NS_ST_EVENT 2u      // event (loc, k, j) found at offset T: `att` dispersal attempts rejected so far
 
 // SAMP: 0 = exponential event-time sampler, 1 = Poisson / order statistics (2.7)
-template <int KIND, bool DEDUP, bool PERCELL, int SAMP>
+// REC: also append every executed event to the stream ring (NEXT-3)
+template <int KIND, bool DEDUP, bool PERCELL, int SAMP, bool REC>
 __global__ void __launch_bounds__(256) simulate_kernel(const ScenarioDev sc, const SimBuffers bf, const EpochArgs ep) {
     __shared__ unsigned short sQ[SAMP == 0 ? 512 : 256];      // SAMP 1: the Poisson guide
     __shared__ u64 sA[SAMP == 0 ? 512 : 256];                 // SAMP 1: the Poisson cdf thresholds
@@ -324,12 +338,14 @@ __global__ void __launch_bounds__(256) simulate_kernel(const ScenarioDev sc, con
                         bf.term_loc[id] = loc; bf.term_k[id] = k; bf.term_j[id] = j; bf.term_f[id] = T; bf.steps[id] = steps;
                         bf.spec_ring[atomicAdd(&bf.ctr->n_spec, 1u)] = id;
                         atomicMax(&bf.ctr->j_max, j);
+                        if (REC) record_event(bf, loc, k, j, T, 0xFFFFFFFFu);
                         st = NS_ST_IDLE;
                     }
                 }
             }
             if (st == NS_ST_EVENT) {
                 if (accept) {
+                    if (REC) record_event(bf, loc, k, j, T, loc2);
                     loc = loc2; cell = cell2; need_prime = true; st = NS_ST_SEARCH;
                     if (ep.max_steps && steps >= ep.max_steps) {
                         bf.state[id] = 3;

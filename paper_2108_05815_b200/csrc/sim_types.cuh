@@ -39,7 +39,7 @@ struct SimCounters {
     u32 j_max;                 // largest event ordinal seen in a speciation record
     u32 n_unfinished;
     u32 n_sampled;             // written by the init kernels
-    u32 pad;
+    u32 n_rec;                 // event-stream records written this epoch (NEXT-3)
     u64 n_events;              // events executed (raw)
     u64 n_culled;
     u64 resamples;
@@ -55,6 +55,10 @@ struct SimBuffers {
     u32 *term_loc, *term_k, *term_j, *steps, *parent, *spec_ring;
     u64 *term_f;
     uint8_t *state;            // 0 active, 1 speciated, 2 culled, 3 stopped by max_steps
+    // event-stream ring of one epoch (REC kernels): origin loc, k, j, offset f, parent loc (0xFFFFFFFF = speciation)
+    u32 *rec_loc, *rec_k, *rec_j, *rec_loc2;
+    u64 *rec_f;
+    u32 rec_cap;
     SimCounters *ctr;
 };
 

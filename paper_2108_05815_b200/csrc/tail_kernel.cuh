@@ -96,7 +96,7 @@ __device__ __forceinline__ bool tail_search_poisson(const SeedKey &key, const Sm
     return true;
 }
 
-template <int KIND, bool DEDUP, bool PERCELL, int SAMP>
+template <int KIND, bool DEDUP, bool PERCELL, int SAMP, bool REC>
 __global__ void __launch_bounds__(256) tail_kernel(const ScenarioDev sc, const SimBuffers bf, const EpochArgs ep) {
     __shared__ unsigned short sQ[SAMP == 0 ? 512 : 256];      // SAMP 1: the Poisson guide
     __shared__ u64 sA[SAMP == 0 ? 512 : 256];                 // SAMP 1: the Poisson cdf thresholds
@@ -134,7 +134,7 @@ __global__ void __launch_bounds__(256) tail_kernel(const ScenarioDev sc, const S
         // pending duplicate check: the exchange of the last probing event (lane 0 holds its result)
         bool pend = false;
         uint4 pold = make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu);
-        u32 p_loc = 0, p_k = 0, p_j = 0;
+        u32 p_loc = 0, p_k = 0, p_j = 0, p_l2 = 0;
         u64 p_T = 0;
         // consumes the pending exchange: true = this lineage is a duplicate at the pending event (culled, recorded)
         auto resolve_pending = [&]() -> bool {
@@ -151,6 +151,10 @@ __global__ void __launch_bounds__(256) tail_kernel(const ScenarioDev sc, const S
                 return true;
             }
             steps++; c_events++;                                       // the pending event was really executed
+            if (REC && lane == 0) {
+                const u32 ri = atomicAdd(&bf.ctr->n_rec, 1u);
+                if (ri < bf.rec_cap) { bf.rec_loc[ri] = p_loc; bf.rec_k[ri] = p_k; bf.rec_j[ri] = p_j; bf.rec_f[ri] = p_T; bf.rec_loc2[ri] = p_l2; }
+            }
             return false;
         };
 
@@ -276,6 +280,14 @@ __global__ void __launch_bounds__(256) tail_kernel(const ScenarioDev sc, const S
                         }
                         u = hashF(xb + att_add + (u64)(r0 + NS_TAIL_ATTEMPTS) * NS_GAMMA);   // next 29 attempts
                     }
+                }
+            }
+            if (REC) {   // the event's record: now if it did not probe, else when its exchange is consumed
+                const u32 l2 = speciates ? 0xFFFFFFFFu : loc2;
+                if (pend) p_l2 = l2;
+                else if (lane == 0) {
+                    const u32 ri = atomicAdd(&bf.ctr->n_rec, 1u);
+                    if (ri < bf.rec_cap) { bf.rec_loc[ri] = loc; bf.rec_k[ri] = k; bf.rec_j[ri] = j; bf.rec_f[ri] = Te; bf.rec_loc2[ri] = l2; }
                 }
             }
             const u32 steps_e = steps + (pend ? 1u : 0u);              // step count if this event is confirmed

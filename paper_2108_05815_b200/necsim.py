@@ -30,7 +30,8 @@ class ScenarioDesc(C.Structure):
 class SimParams(C.Structure):
     _fields_ = [("block_threads", C.c_uint32), ("grid_blocks", C.c_uint32), ("dedup", C.c_uint32),
                 ("dedup_log2_slots", C.c_uint32), ("epoch_events", C.c_uint64), ("max_steps", C.c_uint64),
-                ("tail_threshold", C.c_uint32), ("dedup_probe", C.c_uint32)]
+                ("tail_threshold", C.c_uint32), ("dedup_probe", C.c_uint32), ("record_events", C.c_uint32), ("reserved", C.c_uint32),
+                ("event_ring_capacity", C.c_uint64), ("event_stream_capacity", C.c_uint64)]
 
 
 class Result(C.Structure):
@@ -41,7 +42,9 @@ class Result(C.Structure):
                 ("n_events_raw", C.c_uint64), ("n_culled", C.c_uint64), ("n_speciation_raw", C.c_uint64),
                 ("n_epochs", C.c_uint64), ("n_tail_epochs", C.c_uint64), ("resample_attempts", C.c_uint64),
                 ("n_events_tail", C.c_uint64), ("ms_simulate", C.c_float), ("ms_simulate_tail", C.c_float),
-                ("ms_total", C.c_float), ("n_kernel_launches", C.c_uint32)]
+                ("ms_total", C.c_float), ("n_kernel_launches", C.c_uint32),
+                ("d_stream_loc", C.c_void_p), ("d_stream_k", C.c_void_p), ("d_stream_j", C.c_void_p), ("d_stream_loc2", C.c_void_p),
+                ("d_stream_f", C.c_void_p), ("n_stream_events", C.c_uint64)]
 
 
 EVENT_DTYPE = np.dtype({"names": ["loc", "k", "j", "abundance", "f", "time"],
@@ -117,12 +120,14 @@ def _dev_u32(torch, a, n=None):
 
 
 def make_params(block_threads=0, grid_blocks=0, dedup=None, dedup_log2_slots=0, epoch_events=0, max_steps=0, tail_threshold=0,
-                dedup_probe=0):
+                dedup_probe=0, record_events=False, event_ring_capacity=0, event_stream_capacity=0):
     p = SimParams()
     p.block_threads, p.grid_blocks = block_threads, grid_blocks
     p.dedup = 0 if dedup is None else (1 if dedup else 2)
     p.dedup_log2_slots, p.epoch_events, p.max_steps, p.tail_threshold = dedup_log2_slots, epoch_events, max_steps, tail_threshold
     p.dedup_probe = dedup_probe
+    p.record_events = 1 if record_events else 0
+    p.event_ring_capacity, p.event_stream_capacity = int(event_ring_capacity), int(event_stream_capacity)
     return p
 
 
@@ -220,7 +225,14 @@ class Scenario:
                    labels=_read(self._sim_ws, res.d_labels, n * 4, np.uint32),
                    stats={k: getattr(res, k) for k in ("n_lineages", "n_unfinished", "n_events_raw", "n_culled", "n_speciation_raw",
                                                        "n_epochs", "n_tail_epochs", "resample_attempts", "n_events_tail", "ms_simulate",
-                                                       "ms_simulate_tail", "ms_total", "n_kernel_launches")})
+                                                       "ms_simulate_tail", "ms_total", "n_kernel_launches", "n_stream_events")})
+        if params.record_events:
+            m = int(res.n_stream_events)
+            st = np.zeros(m, dtype=[("loc", "<u4"), ("k", "<u4"), ("j", "<u4"), ("f", "<u8"), ("loc2", "<u4")])
+            for name, ptr, dt, w in (("loc", res.d_stream_loc, np.uint32, 4), ("k", res.d_stream_k, np.uint32, 4), ("j", res.d_stream_j, np.uint32, 4),
+                                     ("f", res.d_stream_f, np.uint64, 8), ("loc2", res.d_stream_loc2, np.uint32, 4)):
+                st[name] = _read(self._sim_ws, ptr, m * w, dt)
+            out["stream"] = st
         if per_lineage:
             pl = np.zeros(n, dtype=[("loc", "<u4"), ("k", "<u4"), ("j", "<u4"), ("f", "<u8")])
             pl["loc"] = _read(self._sim_ws, res.d_term_loc, n * 4, np.uint32); pl["k"] = _read(self._sim_ws, res.d_term_k, n * 4, np.uint32)

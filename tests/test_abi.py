@@ -26,9 +26,9 @@ def test_library_exports_every_declared_symbol():
 def test_struct_sizes_match_header():
     from paper_2108_05815_b200 import necsim
     assert ctypes.sizeof(necsim.ScenarioDesc) == 96
-    assert ctypes.sizeof(necsim.SimParams) == 40
+    assert ctypes.sizeof(necsim.SimParams) == 64
     assert necsim.EVENT_DTYPE.itemsize == 32
-    assert ctypes.sizeof(necsim.Result) == 160
+    assert ctypes.sizeof(necsim.Result) == 208
 
 
 def test_error_paths_without_gpu():
