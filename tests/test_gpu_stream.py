@@ -39,3 +39,21 @@ def test_stream_capacity_errors(O):
     out = sc.simulate(cfg["seed"], cfg["nu"], cfg["mask"])        # the handle still works
     assert out["richness"] > 0
     sc.close()
+
+
+def test_full_size_stream_counts_match_the_oracle():
+    """At full size the stream holds exactly the oracle's number of distinct events (tests/golden/full_configs.json), in time
+    order, with one speciation record per species."""
+    import json, os
+    from paper_2108_05815_b200 import inputs as I, necsim as ns
+    golden = {g["name"]: g for g in json.load(open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "full_configs.json")))}
+    for cfg, ring, cap in ((I.c4_gaussian(), 2**24, 2**24), (I.c2_implicit(), 2**24, 2**26)):
+        sc = ns.Scenario(**I.scenario_kwargs(cfg))
+        got = sc.simulate(cfg["seed"], cfg["nu"], cfg["mask"], record_events=True, event_ring_capacity=ring, event_stream_capacity=cap)
+        g = golden[cfg["name"]]
+        st = got["stream"]
+        assert len(st) == g["unique_events"] and got["richness"] == g["richness"]
+        assert int((st["loc2"] == 0xFFFFFFFF).sum()) == g["richness"]
+        t = st["k"].astype(np.float64) + st["f"].astype(np.float64) / 2.0**48
+        assert np.all(np.diff(t) >= 0)
+        sc.close()
