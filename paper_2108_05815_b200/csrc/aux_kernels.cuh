@@ -63,6 +63,37 @@ __global__ void __launch_bounds__(1024) scan_exclusive_kernel(u32 *__restrict__ 
     if (threadIdx.x == 0 && total_out) *total_out = carry;
 }
 
+// exclusive scan of a long u32 array in three launches: per-block scans of 8192 elements + their totals, a scan of the totals
+// (scan_exclusive_kernel), and the add-back
+#define NS_SCAN_TILE 8192u
+__global__ void __launch_bounds__(1024) scan_tile_kernel(u32 *__restrict__ a, u32 n, u32 *__restrict__ sums) {
+    __shared__ u32 wsum[32];
+    const u32 lane = threadIdx.x & 31u, w = threadIdx.x >> 5;
+    const u32 base = blockIdx.x * NS_SCAN_TILE + threadIdx.x * 8u;
+    u32 v[8], t = 0;
+#pragma unroll
+    for (int q = 0; q < 8; ++q) { v[q] = (base + q < n) ? a[base + q] : 0u; t += v[q]; }
+    u32 x = t;
+    for (int o = 1; o < 32; o <<= 1) { u32 y = __shfl_up_sync(NS_FULL, x, o); if ((int)lane >= o) x += y; }
+    if (lane == 31) wsum[w] = x;
+    __syncthreads();
+    if (w == 0) {
+        u32 s = wsum[lane], z = s;
+        for (int o = 1; o < 32; o <<= 1) { u32 y = __shfl_up_sync(NS_FULL, z, o); if ((int)lane >= o) z += y; }
+        wsum[lane] = z - s;
+        if (lane == 31) sums[blockIdx.x] = z;
+    }
+    __syncthreads();
+    u32 run = wsum[w] + (x - t);
+#pragma unroll
+    for (int q = 0; q < 8; ++q) { if (base + q < n) a[base + q] = run; run += v[q]; }
+}
+__global__ void __launch_bounds__(1024) scan_add_kernel(u32 *__restrict__ a, u32 n, const u32 *__restrict__ sums) {
+    const u32 base = blockIdx.x * NS_SCAN_TILE + threadIdx.x * 8u, add = sums[blockIdx.x];
+#pragma unroll
+    for (int q = 0; q < 8; ++q) if (base + q < n) a[base + q] += add;
+}
+
 // S0, pass 2: ordered compaction -> queue entries {id, loc, cell, steps = 0}; id = rank in ascending loc
 __global__ void __launch_bounds__(256) mask_scatter_kernel(const ScenarioDev sc, const uint8_t *__restrict__ mask, u64 n,
                                                            const u32 *__restrict__ chunk_offset, uint4 *__restrict__ queue, u32 capacity) {

@@ -370,7 +370,7 @@ static int resolve_params(const necsim_scenario *scn, const necsim_sim_params *p
 struct SimLayout {
     size_t off_ctr, off_qa, off_qb, off_cache, off_term_loc, off_term_k, off_term_j, off_steps, off_parent, off_ring, off_term_f,
         off_state, off_events, off_labels, off_species, off_perm_a, off_perm_b, off_flag, off_hist, off_chunk, off_mask,
-        off_rec_loc, off_rec_k, off_rec_j, off_rec_l2, off_rec_f, off_st_loc, off_st_k, off_st_j, off_st_l2, off_st_f, total;
+        off_scan, off_rec_loc, off_rec_k, off_rec_j, off_rec_l2, off_rec_f, off_st_loc, off_st_k, off_st_j, off_st_l2, off_st_f, total;
     u32 n_chunks, sort_blocks;
 };
 
@@ -390,6 +390,7 @@ static void sim_layout(u64 n_individuals, u64 cap, const ResolvedParams &rp, Sim
     L.off_perm_a = take(4 * sort_n); L.off_perm_b = take(4 * sort_n); L.off_flag = take(4 * sort_n);
     L.off_hist = take(4 * 256 * (size_t)L.sort_blocks); L.off_chunk = take(4 * ((size_t)L.n_chunks + 1));
     L.off_mask = take(n_individuals);
+    L.off_scan = take(4 * ((std::max<size_t>(256 * (size_t)L.sort_blocks, sort_n) + NS_SCAN_TILE - 1) / NS_SCAN_TILE + 1));
     L.off_rec_loc = take(4 * rp.ring_cap); L.off_rec_k = take(4 * rp.ring_cap); L.off_rec_j = take(4 * rp.ring_cap);
     L.off_rec_l2 = take(4 * rp.ring_cap); L.off_rec_f = take(8 * rp.ring_cap);
     L.off_st_loc = take(4 * rp.stream_cap); L.off_st_k = take(4 * rp.stream_cap); L.off_st_j = take(4 * rp.stream_cap);
@@ -410,6 +411,16 @@ extern "C" int necsim_simulate_workspace_size(const necsim_scenario *scn, uint64
 }
 
 typedef void (*EpochKernel)(const ScenarioDev, const SimBuffers, const EpochArgs);
+// exclusive scan of n u32 on the stream; `sums` = scratch of n / NS_SCAN_TILE + 1 entries; total -> *d_total (may be NULL)
+static u32 scan_u32(u32 *a, u32 n, u32 *sums, u32 *d_total, cudaStream_t st) {   // returns the kernels launched
+    if (n <= 65536u) { scan_exclusive_kernel<<<1, 1024, 0, st>>>(a, n, d_total); return 1; }
+    const u32 nblk = (n + NS_SCAN_TILE - 1) / NS_SCAN_TILE;
+    scan_tile_kernel<<<nblk, 1024, 0, st>>>(a, n, sums);
+    scan_exclusive_kernel<<<1, 1024, 0, st>>>(sums, nblk, d_total);
+    scan_add_kernel<<<nblk, 1024, 0, st>>>(a, n, sums);
+    return 3;
+}
+
 template <int KIND, bool PERCELL, int SAMP, bool REC>
 static EpochKernel pick_kernel4(bool dedup, bool tail) {
     if (tail) return dedup ? (EpochKernel)tail_kernel<KIND, true, PERCELL, SAMP, REC> : (EpochKernel)tail_kernel<KIND, false, PERCELL, SAMP, REC>;
@@ -454,7 +465,7 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
     necsim_event *events = (necsim_event *)(base + L.off_events);
     u32 *labels = (u32 *)(base + L.off_labels), *species_of = (u32 *)(base + L.off_species);
     u32 *perm_a = (u32 *)(base + L.off_perm_a), *perm_b = (u32 *)(base + L.off_perm_b), *flag = (u32 *)(base + L.off_flag);
-    u32 *hist = (u32 *)(base + L.off_hist), *chunk = (u32 *)(base + L.off_chunk);
+    u32 *hist = (u32 *)(base + L.off_hist), *chunk = (u32 *)(base + L.off_chunk), *scan_tmp = (u32 *)(base + L.off_scan);
     bf.rec_loc = (u32 *)(base + L.off_rec_loc); bf.rec_k = (u32 *)(base + L.off_rec_k); bf.rec_j = (u32 *)(base + L.off_rec_j);
     bf.rec_loc2 = (u32 *)(base + L.off_rec_l2); bf.rec_f = (u64 *)(base + L.off_rec_f); bf.rec_cap = (u32)rp.ring_cap;
     u32 *st_loc = (u32 *)(base + L.off_st_loc), *st_k = (u32 *)(base + L.off_st_k), *st_j = (u32 *)(base + L.off_st_j), *st_l2 = (u32 *)(base + L.off_st_l2);
@@ -585,13 +596,12 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
                 else needed = (kmax >> (8 * (b - 14))) != 0;
                 if (!needed) continue;
                 radix_hist_kernel<<<nb, 256, 0, st>>>(vb, src, nr, b, hist, nb);
-                scan_exclusive_kernel<<<1, 1024, 0, st>>>(hist, 256 * nb, NULL);
+                n_launch += 2 + scan_u32(hist, 256 * nb, scan_tmp, NULL, st);
                 radix_scatter_kernel<<<nb, 256, 0, st>>>(vb, src, dst, nr, b, hist, nb);
                 std::swap(src, dst);
-                n_launch += 3;
             }
             unique_flag_kernel<<<g256, 256, 0, st>>>(vb, src, nr, flag);
-            scan_exclusive_kernel<<<1, 1024, 0, st>>>(flag, nr, &bf.ctr->q_head);   // q_head reused: distinct events of the epoch
+            n_launch += scan_u32(flag, nr, scan_tmp, &bf.ctr->q_head, st) - 1;   // q_head reused: distinct events of the epoch
             stream_write_kernel<<<g256, 256, 0, st>>>(vb, bf.rec_loc2, src, nr, flag, stream_n, rp.stream_cap, st_loc, st_k, st_j, st_f, st_l2);
             n_launch += 4;
             CU(cudaGetLastError());
@@ -626,14 +636,13 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
             else needed = (maxv[3] >> (8 * (b - 14))) != 0;
             if (!needed) continue;
             radix_hist_kernel<<<nb, 256, 0, st>>>(bf, src, n_spec, b, hist, nb);
-            scan_exclusive_kernel<<<1, 1024, 0, st>>>(hist, 256 * nb, NULL);
+            n_launch += 2 + scan_u32(hist, 256 * nb, scan_tmp, NULL, st);
             radix_scatter_kernel<<<nb, 256, 0, st>>>(bf, src, dst, n_spec, b, hist, nb);
             src = dst; std::swap(dst, other);
-            n_launch += 3;
         }
         CU(cudaGetLastError());
         unique_flag_kernel<<<g256, 256, 0, st>>>(bf, src, n_spec, flag);
-        scan_exclusive_kernel<<<1, 1024, 0, st>>>(flag, n_spec, &bf.ctr->q_head);   // q_head reused: richness
+        n_launch += scan_u32(flag, n_spec, scan_tmp, &bf.ctr->q_head, st) - 1;   // q_head reused: richness
         unique_write_kernel<<<g256, 256, 0, st>>>(bf, src, n_spec, flag, events, species_of, sd.delta_t);
         n_launch += 3;
         CU(cudaGetLastError());
