@@ -54,7 +54,7 @@ def random_scenario(I, rng):
 
 def test_random_scenarios(ns, O, I):
     rng = np.random.default_rng(2024)
-    for case in range(40):
+    for case in range(60):
         kw = random_scenario(I, rng)
         o = O.Scenario(**kw)
         n_ind = o.n_individuals
@@ -64,12 +64,22 @@ def test_random_scenarios(ns, O, I):
             mask[int(rng.integers(0, n_ind))] = 1
         nu = float(rng.choice([1.0, 0.3, 0.05, 0.01]))
         seed = int(rng.integers(0, 2**63))
+        kw["sampler"] = int(rng.integers(0, 2))                       # exponential or Poisson event-time sampler
+        record = bool(rng.integers(0, 2))                             # with or without the full event stream
         knobs = dict(tail_threshold=int(rng.choice([1, 0xFFFFFFFF, 0])), dedup_probe=int(rng.integers(0, 5)),
                      dedup_log2_slots=int(rng.choice([4, 8, 16, 0])), block_threads=int(rng.choice([32, 128, 256])),
                      epoch_events=int(rng.choice([0, 1, 50, 5000])))
-        ref = o.simulate(seed, nu, mask, dedup=True)
+        o = O.Scenario(**kw)
+        ref = o.simulate_stream(seed, nu, mask) if record else o.simulate(seed, nu, mask, dedup=True)
         sc = ns.Scenario(**kw)
-        same(sc.simulate(seed, nu, mask, **knobs), ref, (case, kw["kind"], knobs))
+        if record:
+            knobs.update(record_events=True, event_ring_capacity=int(rng.choice([1 << 16, 1 << 20])), event_stream_capacity=1 << 21)
+        got = sc.simulate(seed, nu, mask, **knobs)
+        same(got, ref, (case, kw["kind"], knobs))
+        if record:
+            assert len(got["stream"]) == len(ref["stream"]), (case, knobs)
+            for f in ("loc", "k", "j", "f", "loc2"):
+                assert np.array_equal(got["stream"][f], ref["stream"][f]), (case, knobs, f)
         sc.close()
 
 
