@@ -558,6 +558,11 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
             grid = full_grid;
             if (lanes == 1) grid = (u32)std::min<u64>(full_grid, ((u64)active + warps_per_block - 1) / warps_per_block);
         }
+        ep.rec_chunk = 1;
+        if (rp.record && tail) {   // chunked ring reservation: at most a quarter of the ring may sit in unused reservations
+            const u64 warps = std::min<u64>(active, (u64)grid * warps_per_block);
+            ep.rec_chunk = (u32)std::max<u64>(1, std::min<u64>(NS_REC_CHUNK, rp.ring_cap / (4 * std::max<u64>(warps, 1))));
+        }
         bf.q_in = q_in; bf.q_out = q_out; bf.q_in_count = active;
         // a few thousand lineages need few slots: keep the tail's cache footprint (2 MiB) inside L2 next to the tables
         bf.cache_mask = rp.dedup ? (tail ? std::min(full_cache_mask, (1u << 17) - 1u) : full_cache_mask) : 0u;
@@ -593,14 +598,14 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
                 if (b < 4) needed = b < 2;
                 else if (b < 8) needed = (lmax >> (8 * (b - 4))) != 0;
                 else if (b < 14) needed = true;
-                else needed = (kmax >> (8 * (b - 14))) != 0;
+                else needed = tail || (kmax >> (8 * (b - 14))) != 0;   // tail epochs may hold sentinels (k = 0xFFFFFFFF): they must sort last
                 if (!needed) continue;
                 radix_hist_kernel<<<nb, 256, 0, st>>>(vb, src, nr, b, hist, nb);
                 n_launch += 2 + scan_u32(hist, 256 * nb, scan_tmp, NULL, st);
                 radix_scatter_kernel<<<nb, 256, 0, st>>>(vb, src, dst, nr, b, hist, nb);
                 std::swap(src, dst);
             }
-            unique_flag_kernel<<<g256, 256, 0, st>>>(vb, src, nr, flag);
+            stream_flag_kernel<<<g256, 256, 0, st>>>(vb, src, nr, flag);
             n_launch += scan_u32(flag, nr, scan_tmp, &bf.ctr->q_head, st) - 1;   // q_head reused: distinct events of the epoch
             stream_write_kernel<<<g256, 256, 0, st>>>(vb, bf.rec_loc2, src, nr, flag, stream_n, rp.stream_cap, st_loc, st_k, st_j, st_f, st_l2);
             n_launch += 4;

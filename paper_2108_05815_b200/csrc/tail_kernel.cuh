@@ -18,6 +18,7 @@
 
 namespace necsim {
 
+#define NS_REC_CHUNK 64u           // event-stream ring slots a warp reserves at a time
 #define NS_TAIL_ATTEMPTS 29u      // dispersal attempts evaluated per pass (lanes 3..31)
 
 
@@ -119,6 +120,14 @@ __global__ void __launch_bounds__(256) tail_kernel(const ScenarioDev sc, const S
     const u32 att_lane = lane >= 3u ? lane - 3u : 0u;                  // dispersal attempt of this lane within a pass
     const u64 att_add = (u64)att_lane * NS_GAMMA;
     unsigned long long c_events = 0, c_culled = 0, c_resamples = 0;   // warp-uniform
+    // event-stream ring (REC): the warp reserves ep.rec_chunk (<= NS_REC_CHUNK) slots at a time, so that it waits for an atomic's return once per
+    // chunk and not once per event; slots left over at the end are filled with sentinels (k = 0xFFFFFFFF) the host-side pass drops
+    u32 rec_next = 0, rec_left = 0;
+    auto record = [&](u32 r_loc, u32 r_k, u32 r_j, u64 r_f, u32 r_l2) {   // lane 0 only
+        if (rec_left == 0u) { rec_next = atomicAdd(&bf.ctr->n_rec, ep.rec_chunk); rec_left = ep.rec_chunk; }
+        const u32 ri = rec_next++; --rec_left;
+        if (ri < bf.rec_cap) { bf.rec_loc[ri] = r_loc; bf.rec_k[ri] = r_k; bf.rec_j[ri] = r_j; bf.rec_f[ri] = r_f; bf.rec_loc2[ri] = r_l2; }
+    };
 
     for (;;) {
         // ---- S4: one queue entry per warp --------------------------------------------------------------
@@ -151,10 +160,7 @@ __global__ void __launch_bounds__(256) tail_kernel(const ScenarioDev sc, const S
                 return true;
             }
             steps++; c_events++;                                       // the pending event was really executed
-            if (REC && lane == 0) {
-                const u32 ri = atomicAdd(&bf.ctr->n_rec, 1u);
-                if (ri < bf.rec_cap) { bf.rec_loc[ri] = p_loc; bf.rec_k[ri] = p_k; bf.rec_j[ri] = p_j; bf.rec_f[ri] = p_T; bf.rec_loc2[ri] = p_l2; }
-            }
+            if (REC && lane == 0) record(p_loc, p_k, p_j, p_T, p_l2);
             return false;
         };
 
@@ -285,10 +291,7 @@ __global__ void __launch_bounds__(256) tail_kernel(const ScenarioDev sc, const S
             if (REC) {   // the event's record: now if it did not probe, else when its exchange is consumed
                 const u32 l2 = speciates ? 0xFFFFFFFFu : loc2;
                 if (pend) p_l2 = l2;
-                else if (lane == 0) {
-                    const u32 ri = atomicAdd(&bf.ctr->n_rec, 1u);
-                    if (ri < bf.rec_cap) { bf.rec_loc[ri] = loc; bf.rec_k[ri] = k; bf.rec_j[ri] = j; bf.rec_f[ri] = Te; bf.rec_loc2[ri] = l2; }
-                }
+                else if (lane == 0) record(loc, k, j, Te, l2);
             }
             const u32 steps_e = steps + (pend ? 1u : 0u);              // step count if this event is confirmed
             const bool capped = ep.max_steps && steps_e >= ep.max_steps;
@@ -310,6 +313,13 @@ __global__ void __launch_bounds__(256) tail_kernel(const ScenarioDev sc, const S
                 break;
             }
             f_last = (i64)Te; loc = loc2; cell = cell2; Cm = Cm2; sh = sh2;
+        }
+    }
+    if (REC) {   // sentinels into the reserved slots that stayed empty
+        const u32 nx = __shfl_sync(NS_FULL, rec_next, 0), lf = __shfl_sync(NS_FULL, rec_left, 0);
+        for (u32 q = lane; q < lf; q += 32u) {
+            const u32 ri = nx + q;
+            if (ri < bf.rec_cap) { bf.rec_loc[ri] = 0xFFFFFFFFu; bf.rec_k[ri] = 0xFFFFFFFFu; bf.rec_j[ri] = 0xFFFFFFFFu; bf.rec_f[ri] = ~0ull; bf.rec_loc2[ri] = 0xFFFFFFFFu; }
         }
     }
     if (lane == 0) {
