@@ -69,14 +69,16 @@ typedef struct necsim_scenario_desc {
  * A zero field means "library default".
  */
 typedef struct necsim_sim_params {
-    uint32_t block_threads;    /* threads per block of the simulate kernel (multiple of 32, <= 1024) */
+    uint32_t block_threads;    /* threads per block of the simulate kernels (multiple of 32, <= 256; default 256) */
     uint32_t grid_blocks;      /* persistent blocks; 0 = resident blocks per SM x number of SMs */
     uint32_t dedup;            /* 0 = default (on), 1 = on, 2 = off */
     uint32_t dedup_log2_slots; /* global duplicate-culling cache: 2^this slots of 16 bytes (default 22) */
-    uint64_t epoch_events;     /* target number of events per epoch (time-horizon step, G.1 L2157-2187) */
+    uint64_t epoch_events;     /* target number of events per epoch (time-horizon step, G.1 L2157-2187); 0 = default policy:
+                                  half the cache slots, x64 in tail epochs, and never fewer than 64 events per active lineage */
     uint64_t max_steps;        /* 0 = unlimited; else a lineage stops after this many executed events
                                   ("unfinished": label 0xFFFFFFFF) -- the MODE-T throughput workload */
-    uint32_t tail_threshold;   /* switch to the low-latency tail kernel when active lineages <= this; 0 = default */
+    uint32_t tail_threshold;   /* switch to the low-latency tail kernel (one lineage per warp) when active lineages <= this;
+                                  0 = default (two lineages per resident warp) */
     uint32_t dedup_probe;      /* 0 = default (4); else 1 + log2 of the probe period: 1 = every event, 2 = every 2nd, 3 = every 4th,
                                   4 = every 8th event (chosen by a hash of the event identity) probes the cache (PAPER.md L942-946:
                                   the paper probes every step_slice steps) */
@@ -156,9 +158,10 @@ int necsim_simulate_workspace_size(const necsim_scenario *scn, uint64_t n_sample
  *   seed : primes the hash RNG (5.2.1, L693-707).
  *   nu   : speciation probability per event in [0,1] (SPATIALLY_IMPLICIT: the metacommunity's; the
  *          local community has nu = 0, L1830). nu = 0 requires max_steps > 0.
- *   d_sample_mask : DEVICE u8[n_individuals], non-zero = sampled; NULL = everyone. n_sampled must equal
- *          the number of non-zero entries' upper bound used for the workspace (it is recounted on device;
- *          more sampled individuals than the workspace was sized for => NECSIM_ERR_WORKSPACE_TOO_SMALL).
+ *   d_sample_mask : DEVICE u8[n_individuals], non-zero = sampled; NULL = everyone.
+ *   n_sampled_capacity : the number of lineages the workspace was sized for (necsim_simulate_workspace_size); the
+ *          mask is counted on the device and more sampled individuals than that => NECSIM_ERR_WORKSPACE_TOO_SMALL.
+ *   bytes : size of d_workspace, at least what necsim_simulate_workspace_size returned for the same params.
  * Asynchronous on the stream except for one small read-back per epoch; returns after the final
  * read-back. Pointers in *out point into d_workspace and stay valid until it is reused.
  */
