@@ -128,7 +128,7 @@ __device__ __forceinline__ u32 key_byte(const SimBuffers &bf, u32 id, u32 b) {
     if (b < 4) return (bf.term_j[id] >> (8 * b)) & 255u;
     if (b < 8) return (bf.term_loc[id] >> (8 * (b - 4))) & 255u;
     if (b < 14) return (u32)(bf.term_f[id] >> (8 * (b - 8))) & 255u;
-    return (bf.term_k[id] >> (8 * (b - 14))) & 255u;
+    return ((bf.term_k[id] - bf.k_base) >> (8 * (b - 14))) & 255u;
 }
 
 #define NS_SORT_TILE 2048u
@@ -248,21 +248,21 @@ __global__ void __launch_bounds__(256) iota_kernel(u32 *perm, u32 n) {
     u32 i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i < n) perm[i] = i;
 }
-// head flags over the sorted ring; sentinel records (k = 0xFFFFFFFF: reserved but unused slots) sort last and count for nothing
-__global__ void __launch_bounds__(256) stream_flag_kernel(const SimBuffers bf, const u32 *__restrict__ perm, u32 n, u32 *__restrict__ flag) {
+// head flags over the sorted ring; sentinel records (k = the epoch's k_stop: reserved but unused slots) sort last and count for nothing
+__global__ void __launch_bounds__(256) stream_flag_kernel(const SimBuffers bf, const u32 *__restrict__ perm, u32 n, u32 k_sentinel, u32 *__restrict__ flag) {
     u32 i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const u32 id = perm[i];
-    flag[i] = (bf.term_k[id] != 0xFFFFFFFFu && (i == 0 || !same_event(bf, id, perm[i - 1]))) ? 1u : 0u;
+    flag[i] = (bf.term_k[id] != k_sentinel && (i == 0 || !same_event(bf, id, perm[i - 1]))) ? 1u : 0u;
 }
 // bf.term_* alias the ring's key arrays; duplicates of an event are adjacent after the sort: keep the first
 __global__ void __launch_bounds__(256) stream_write_kernel(const SimBuffers bf, const u32 *__restrict__ rec_loc2, const u32 *__restrict__ perm, u32 n,
-                                                           const u32 *__restrict__ uidx, u64 base, u64 cap, u32 *__restrict__ s_loc, u32 *__restrict__ s_k,
+                                                           const u32 *__restrict__ uidx, u32 k_sentinel, u64 base, u64 cap, u32 *__restrict__ s_loc, u32 *__restrict__ s_k,
                                                            u32 *__restrict__ s_j, u64 *__restrict__ s_f, u32 *__restrict__ s_loc2) {
     u32 i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const u32 id = perm[i];
-    if (bf.term_k[id] == 0xFFFFFFFFu || (i != 0 && same_event(bf, id, perm[i - 1]))) return;
+    if (bf.term_k[id] == k_sentinel || (i != 0 && same_event(bf, id, perm[i - 1]))) return;
     const u64 o = base + uidx[i];
     if (o >= cap) return;
     s_loc[o] = bf.term_loc[id]; s_k[o] = bf.term_k[id]; s_j[o] = bf.term_j[id]; s_f[o] = bf.term_f[id]; s_loc2[o] = rec_loc2[id];

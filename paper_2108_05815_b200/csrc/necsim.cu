@@ -592,22 +592,23 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
             const u32 nb = (nr + NS_SORT_TILE - 1) / NS_SORT_TILE, g256 = (nr + 255) / 256;
             iota_kernel<<<g256, 256, 0, st>>>(perm_a, nr);
             u32 *src = perm_a, *dst = perm_b;
-            const u32 kmax = k_stop - 1u, lmax = (u32)(sd.n_locations - 1);
+            vb.k_base = ep.k_start;
+            const u32 kmax = k_stop - ep.k_start, lmax = (u32)(sd.n_locations - 1);   // sentinels carry k = k_stop
             for (u32 b = 0; b < 18; ++b) {   // j: two bytes (ordinals stay far below 2^16 for mu <= 64), loc and k: the bytes in use
                 bool needed;
                 if (b < 4) needed = b < 2;
                 else if (b < 8) needed = (lmax >> (8 * (b - 4))) != 0;
                 else if (b < 14) needed = true;
-                else needed = tail || (kmax >> (8 * (b - 14))) != 0;   // tail epochs may hold sentinels (k = 0xFFFFFFFF): they must sort last
+                else needed = (kmax >> (8 * (b - 14))) != 0;
                 if (!needed) continue;
                 radix_hist_kernel<<<nb, 256, 0, st>>>(vb, src, nr, b, hist, nb);
                 n_launch += 2 + scan_u32(hist, 256 * nb, scan_tmp, NULL, st);
                 radix_scatter_kernel<<<nb, 256, 0, st>>>(vb, src, dst, nr, b, hist, nb);
                 std::swap(src, dst);
             }
-            stream_flag_kernel<<<g256, 256, 0, st>>>(vb, src, nr, flag);
+            stream_flag_kernel<<<g256, 256, 0, st>>>(vb, src, nr, k_stop, flag);
             n_launch += scan_u32(flag, nr, scan_tmp, &bf.ctr->q_head, st) - 1;   // q_head reused: distinct events of the epoch
-            stream_write_kernel<<<g256, 256, 0, st>>>(vb, bf.rec_loc2, src, nr, flag, stream_n, rp.stream_cap, st_loc, st_k, st_j, st_f, st_l2);
+            stream_write_kernel<<<g256, 256, 0, st>>>(vb, bf.rec_loc2, src, nr, flag, k_stop, stream_n, rp.stream_cap, st_loc, st_k, st_j, st_f, st_l2);
             n_launch += 4;
             CU(cudaGetLastError());
             u32 heads = 0;

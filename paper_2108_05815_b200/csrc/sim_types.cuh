@@ -59,6 +59,7 @@ struct SimBuffers {
     u32 *rec_loc, *rec_k, *rec_j, *rec_loc2;
     u64 *rec_f;
     u32 rec_cap;
+    u32 k_base;                // radix passes sort k - k_base (0 for the species table; the epoch's k_start for the stream ring)
     SimCounters *ctr;
 };
 

@@ -121,7 +121,7 @@ __global__ void __launch_bounds__(256) tail_kernel(const ScenarioDev sc, const S
     const u64 att_add = (u64)att_lane * NS_GAMMA;
     unsigned long long c_events = 0, c_culled = 0, c_resamples = 0;   // warp-uniform
     // event-stream ring (REC): the warp reserves ep.rec_chunk (<= NS_REC_CHUNK) slots at a time, so that it waits for an atomic's return once per
-    // chunk and not once per event; slots left over at the end are filled with sentinels (k = 0xFFFFFFFF) the host-side pass drops
+    // chunk and not once per event; slots left over at the end are filled with sentinels (k = k_stop, which no event of the epoch has) the host-side pass drops
     u32 rec_next = 0, rec_left = 0;
     auto record = [&](u32 r_loc, u32 r_k, u32 r_j, u64 r_f, u32 r_l2) {   // lane 0 only
         if (rec_left == 0u) { rec_next = atomicAdd(&bf.ctr->n_rec, ep.rec_chunk); rec_left = ep.rec_chunk; }
@@ -319,7 +319,7 @@ __global__ void __launch_bounds__(256) tail_kernel(const ScenarioDev sc, const S
         const u32 nx = __shfl_sync(NS_FULL, rec_next, 0), lf = __shfl_sync(NS_FULL, rec_left, 0);
         for (u32 q = lane; q < lf; q += 32u) {
             const u32 ri = nx + q;
-            if (ri < bf.rec_cap) { bf.rec_loc[ri] = 0xFFFFFFFFu; bf.rec_k[ri] = 0xFFFFFFFFu; bf.rec_j[ri] = 0xFFFFFFFFu; bf.rec_f[ri] = ~0ull; bf.rec_loc2[ri] = 0xFFFFFFFFu; }
+            if (ri < bf.rec_cap) { bf.rec_loc[ri] = 0xFFFFFFFFu; bf.rec_k[ri] = ep.k_stop; bf.rec_j[ri] = 0xFFFFFFFFu; bf.rec_f[ri] = ~0ull; bf.rec_loc2[ri] = 0xFFFFFFFFu; }
         }
     }
     if (lane == 0) {

@@ -54,7 +54,8 @@ def random_scenario(I, rng):
 
 def test_random_scenarios(ns, O, I):
     rng = np.random.default_rng(2024)
-    for case in range(60):
+    import os
+    for case in range(int(os.environ.get("NECSIM_FUZZ_CASES", "60"))):
         kw = random_scenario(I, rng)
         o = O.Scenario(**kw)
         n_ind = o.n_individuals
