@@ -183,4 +183,23 @@ __device__ __forceinline__ uint4 atomic_exch_128(uint4 *addr, uint4 v) {
     return make_uint4((u32)olo, (u32)(olo >> 32), (u32)ohi, (u32)(ohi >> 32));
 }
 
+// the same exchange under a predicate, the result landing in (olo, ohi) only where it executes: no branch around it and no
+// copy of the result after it, so that a caller which consumes the result much later does not wait for the round trip here
+__device__ __forceinline__ void atomic_exch_128_if(bool p, uint4 *addr, uint4 v, u64 &olo, u64 &ohi) {
+    const u64 lo = ((u64)v.y << 32) | v.x, hi = ((u64)v.w << 32) | v.z;
+    asm volatile(
+        "{\n\t"
+        ".reg .pred q;\n\t"
+        ".reg .b128 vin, vout;\n\t"
+        "setp.ne.u32 q, %4, 0;\n\t"
+        "mov.b128 vin, {%2, %3};\n\t"
+        "mov.b128 vout, {%0, %1};\n\t"
+        "@q atom.global.relaxed.gpu.exch.b128 vout, [%5], vin;\n\t"
+        "mov.b128 {%0, %1}, vout;\n\t"
+        "}"
+        : "+l"(olo), "+l"(ohi)
+        : "l"(lo), "l"(hi), "r"((u32)p), "l"(addr)
+        : "memory");
+}
+
 }  // namespace necsim

@@ -45,6 +45,14 @@ __device__ __forceinline__ uint2 load_rate(const ScenarioDev &sc, u32 idx) {
     return make_uint2(__ldg(&sc.thin[idx]), 0u);
 }
 
+// Gathers of one dispersal target, issued back to back (volatile: kept in this order): prefix and rate first, the habitat
+// byte last, so that the first instruction that needs the habitat byte waits for all three round trips at once.
+__device__ __forceinline__ u32 ldg_u32_ordered(const u32 *p) { u32 v; asm volatile("ld.global.nc.u32 %0, [%1];" : "=r"(v) : "l"(p)); return v; }
+__device__ __forceinline__ u32 ldg_u8_ordered(const uint8_t *p) { u32 v; asm volatile("ld.global.nc.u8 %0, [%1];" : "=r"(v) : "l"(p)); return v; }
+__device__ __forceinline__ uint2 ldg_v2_ordered(const uint2 *p) {
+    uint2 v; asm volatile("ld.global.nc.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "l"(p)); return v;
+}
+
 __device__ __forceinline__ u64 shfl_xor_u64(u64 v, int m) { return __shfl_xor_sync(NS_FULL, v, m); }
 
 // Poisson sampler, one search round of one lineage across the warp: lanes 0..15 the points 1..16 of
@@ -142,15 +150,15 @@ __global__ void __launch_bounds__(256) tail_kernel(const ScenarioDev sc, const S
         if (PERCELL) { uint2 cs = load_rate<SAMP>(sc, KIND == 3 ? xy_index(sc, cell) : cell); Cm = cs.x; sh = cs.y; }
         // pending duplicate check: the exchange of the last probing event (lane 0 holds its result)
         bool pend = false;
-        uint4 pold = make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu);
+        u64 pold_lo = ~0ull, pold_hi = ~0ull;
         u32 p_loc = 0, p_k = 0, p_j = 0, p_l2 = 0;
         u64 p_T = 0;
         // consumes the pending exchange: true = this lineage is a duplicate at the pending event (culled, recorded)
         auto resolve_pending = [&]() -> bool {
             if (!DEDUP || !pend) return false;
             pend = false;
-            const u32 ox = __shfl_sync(NS_FULL, pold.x, 0), oy = __shfl_sync(NS_FULL, pold.y, 0);
-            const u32 oz = __shfl_sync(NS_FULL, pold.z, 0), ow = __shfl_sync(NS_FULL, pold.w, 0);
+            const u32 ox = __shfl_sync(NS_FULL, (u32)pold_lo, 0), oy = __shfl_sync(NS_FULL, (u32)(pold_lo >> 32), 0);
+            const u32 oz = __shfl_sync(NS_FULL, (u32)pold_hi, 0), ow = __shfl_sync(NS_FULL, (u32)(pold_hi >> 32), 0);
             if (ox == p_loc && oy == p_k && oz == p_j && ow != id) {   // another lineage executed it first (L687, L697)
                 if (lane == 0) {
                     bf.parent[id] = ow; bf.state[id] = 2;
@@ -224,10 +232,8 @@ __global__ void __launch_bounds__(256) tail_kernel(const ScenarioDev sc, const S
             if (DEDUP) {
                 const u32 h = cache_hash(loc, k, j);
                 probes = cache_probes(h, ep.probe_mask);
-                if (probes) {
-                    if (lane == 0) pold = atomic_exch_128(&bf.cache[h & bf.cache_mask], make_uint4(loc, k, j, id));
-                    p_loc = loc; p_k = k; p_j = j; p_T = Te; pend = true;
-                }
+                atomic_exch_128_if(probes && lane == 0, &bf.cache[h & bf.cache_mask], make_uint4(loc, k, j, id), pold_lo, pold_hi);
+                if (probes) { p_loc = loc; p_k = k; p_j = j; p_T = Te; pend = true; }
             }
             if (!probes) { steps++; c_events++; }
             // S2 + S3: all draws of the event in one hash evaluation across the lanes
@@ -269,9 +275,13 @@ __global__ void __launch_bounds__(256) tail_kernel(const ScenarioDev sc, const S
                             const u32 yy = wrap_add(y0, dy, sc.height);
                             const u32 ci = yy * sc.width + xx;
                             c2 = (yy << 16) | xx;
-                            d = cell_deme(sc, ci);
-                            pf = cell_prefix(sc, ci);                       // speculative: same round trip as the habitat test
-                            if (PERCELL) cs = load_rate<SAMP>(sc, ci);
+                            pf = ldg_u32_ordered(&sc.prefix[ci]);           // speculative: same round trip as the habitat test
+                            if (PERCELL) {
+                                if (SAMP == 0) cs = ldg_v2_ordered(&sc.scale[ci]);
+                                else cs.x = ldg_u32_ordered(&sc.thin[ci]), cs.y = 0u;
+                            }
+                            d = ldg_u8_ordered(&sc.hab8[ci]);
+                            if (d == 255u) d = __ldg(&sc.deme32[ci]);
                         }
                         const u32 okm = __ballot_sync(NS_FULL, lane >= 3u && d > 0u);
                         if (okm) {

@@ -53,7 +53,7 @@ def test_product_arm_line(config, sampler):
     assert r["n_gpus"] == 1 and r["steps"] == 2 and r["warmup"] == 3 and r["scaling"] == "weak" and r["dtype"] == "int64"
     assert r["value"] > 0 and r["gpu_launches"] > 0
     e = r["e2e"]
-    assert e["value"] > 0 and e["h2d_bytes_per_step"] > 0 and e["d2h_bytes_per_step"] > 0 and e["value"] != r["value"]
+    assert e["value"] > 0 and e["h2d_bytes_per_step"] >= 0 and e["d2h_bytes_per_step"] > 0 and e["value"] != r["value"]
     rf = r["roofline"]
     assert rf["bound"] == "alu" and rf["peak"] > 0 and rf["achieved"] > 0 and abs(rf["frac"] - rf["achieved"] / rf["peak"]) < 1e-12
     assert {"sm_mhz", "sm_max_mhz", "reasons"} <= set(r["clocks"])
