@@ -74,11 +74,12 @@ typedef struct necsim_sim_params {
     uint32_t dedup;            /* 0 = default (on), 1 = on, 2 = off */
     uint32_t dedup_log2_slots; /* global duplicate-culling cache: 2^this slots of 16 bytes (default 22) */
     uint64_t epoch_events;     /* target number of events per epoch (time-horizon step, G.1 L2157-2187); 0 = default policy:
-                                  half the cache slots, x64 in tail epochs, and never fewer than 64 events per active lineage */
+                                  half the cache slots and never fewer than 64 events per active lineage; the tail kernel runs as
+                                  one launch without a horizon (with record_events: x64 per epoch, capped by the ring) */
     uint64_t max_steps;        /* 0 = unlimited; else a lineage stops after this many executed events
                                   ("unfinished": label 0xFFFFFFFF) -- the MODE-T throughput workload */
     uint32_t tail_threshold;   /* switch to the low-latency tail kernel (one lineage per warp) when active lineages <= this;
-                                  0 = default (two lineages per resident warp) */
+                                  0 = default (four lineages per resident warp) */
     uint32_t dedup_probe;      /* 0 = default (4); else 1 + log2 of the probe period: 1 = every event, 2 = every 2nd, 3 = every 4th,
                                   4 = every 8th event (chosen by a hash of the event identity) probes the cache (PAPER.md L942-946:
                                   the paper probes every step_slice steps) */

@@ -515,8 +515,8 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
     const u32 full_grid = rp.grid_blocks ? rp.grid_blocks : (u32)(occ * scn->sm_count);
     const u32 tail_grid = rp.grid_blocks ? rp.grid_blocks : (u32)(occ_tail * scn->sm_count);
     const u32 warps_per_block = rp.block_threads / 32u;
-    // one lineage per warp pays off from about two lineages per resident warp downwards (measured on C5: sweep in DESIGN.md 5)
-    const u32 tail_threshold = rp.tail_threshold ? rp.tail_threshold : 2u * tail_grid * warps_per_block;
+    // one lineage per warp pays off from about four lineages per resident warp downwards (measured on C5 / C6: sweep in DESIGN.md 5)
+    const u32 tail_threshold = rp.tail_threshold ? rp.tail_threshold : 4u * tail_grid * warps_per_block;
     const u32 full_cache_mask = rp.dedup ? ((1u << rp.dedup_log2_slots) - 1u) : 0u;
     u32 active = n_sampled, k_start = 0;
     uint4 *q_in = qa, *q_out = qb;
@@ -525,7 +525,12 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
     const bool params_default_epoch = !(params && params->epoch_events);
     while (active > 0) {
         u32 k_stop;
-        if (rp.epoch_events == 0 && !rp.record) k_stop = 0xFFFFFFFFu;
+        // The tail is ONE launch without a horizon (default policy, no event stream): it is bound by the longest lineage's chain
+        // of events, every horizon adds the spread between the slowest and the average lineage of its window, and lineages that
+        // have merged keep finding each other through the full-size cache (measured on C5: 5 tail epochs 4.80 s, one 4.24 s, with
+        // fewer redundant events).
+        const bool unbounded = params_default_epoch && !rp.record && active <= tail_threshold;
+        if ((rp.epoch_events == 0 && !rp.record) || unbounded) k_stop = 0xFFFFFFFFu;
         else {
             // (i) tail epochs are latency-bound and their warps stay roughly synchronous in simulated time: longer epochs cost
             // no dedup hits and amortise the end-of-epoch imbalance (spread of events per lineage ~ 1/sqrt(span))
@@ -564,8 +569,9 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
             ep.rec_chunk = (u32)std::max<u64>(1, std::min<u64>(NS_REC_CHUNK, rp.ring_cap / (4 * std::max<u64>(warps, 1))));
         }
         bf.q_in = q_in; bf.q_out = q_out; bf.q_in_count = active;
-        // a few thousand lineages need few slots: keep the tail's cache footprint (2 MiB) inside L2 next to the tables
-        bf.cache_mask = rp.dedup ? (tail ? std::min(full_cache_mask, (1u << 17) - 1u) : full_cache_mask) : 0u;
+        // tail epochs with a horizon: a few thousand synchronous lineages need few slots, keep the footprint (2 MiB) inside L2
+        // next to the tables. The tail without a horizon drifts apart in simulated time and needs the long memory of the full cache.
+        bf.cache_mask = rp.dedup ? ((tail && !unbounded) ? std::min(full_cache_mask, (1u << 17) - 1u) : full_cache_mask) : 0u;
         CU(cudaMemsetAsync(bf.ctr, 0, 8, st));   // q_head, q_out
         if (rp.record) CU(cudaMemsetAsync(&bf.ctr->n_rec, 0, 4, st));
         CU(cudaEventRecord(scn->ev[2], st));
