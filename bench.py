@@ -250,7 +250,7 @@ def main():
                              # dram__bytes_read.sum + dram__bytes_write.sum of one tail_kernel launch (C5, exponential sampler, 13th tail
                              # epoch, 50 ms), ncu --set full, profiles/r1_ncu_tail_kernel_c5.md; caches are flushed per ncu replay pass,
                              # so this is an upper bound
-                             "traffic": 1422595056 if (name == "c5" and dom_name == "tail_kernel" and args.sampler == "exp") else None,
+                             "traffic": 6885399296 if (name == "c5" and dom_name == "tail_kernel" and args.sampler == "exp") else None,
                              "instr_per_event": I_EVENT[name],
                              "note": "latency-bound by construction: one lineage per warp walks a serial chain of ~ln(S)/nu events (DESIGN.md 6.3)",
                              "peak_source": "derived: SMs x 4 schedulers x 32 lanes x sm_max_mhz (DESIGN.md section 6)",
