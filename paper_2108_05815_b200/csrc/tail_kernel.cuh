@@ -53,6 +53,14 @@ __device__ __forceinline__ uint2 ldg_v2_ordered(const uint2 *p) {
     uint2 v; asm volatile("ld.global.nc.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "l"(p)); return v;
 }
 
+// index of the lowest set bit of m != 0: isolate it and take its position (one FLO; __ffs costs BREV + FLO, two trips
+// through the quarter-rate unit on a chain where every cycle counts)
+__device__ __forceinline__ int first_bit(u32 m) {
+    u32 r;
+    asm("bfind.u32 %0, %1;" : "=r"(r) : "r"(m & (0u - m)));
+    return (int)r;
+}
+
 __device__ __forceinline__ u64 shfl_xor_u64(u64 v, int m) { return __shfl_xor_sync(NS_FULL, v, m); }
 
 // Poisson sampler, one search round of one lineage across the warp: lanes 0..15 the points 1..16 of
@@ -198,7 +206,7 @@ __global__ void __launch_bounds__(256) tail_kernel(const ScenarioDev sc, const S
                 const u32 evm = __ballot_sync(NS_FULL, inside && (half ? kvalid : ((i64)T > f_last)));
                 const u32 crm = __ballot_sync(NS_FULL, !inside);
                 if (evm & 0xFFFFu) {                       // next event is in interval k
-                    const int src = __ffs(evm & 0xFFFFu) - 1;
+                    const int src = first_bit(evm & 0xFFFFu);
                     j = (u32)src + 1u;
                     Te = __shfl_sync(NS_FULL, T, src); Xe = __shfl_sync(NS_FULL, X, src);
                 } else if (crm & 0xFFFFu) {                // interval k exhausted (L719, L727): first non-empty interval after it
@@ -206,7 +214,7 @@ __global__ void __launch_bounds__(256) tail_kernel(const ScenarioDev sc, const S
                     const u32 nvalid = gap < 16u ? gap : 16u;
                     const u32 hm = evm >> 16;
                     if (!hm) { k = k + 1u + nvalid; f_last = -1; continue; }   // all speculated intervals empty / beyond the horizon
-                    const int src = 16 + __ffs(hm) - 1;
+                    const int src = 16 + first_bit(hm);
                     k = k + 1u + (u32)(src - 16); j = 1u;
                     Te = __shfl_sync(NS_FULL, T, src); Xe = __shfl_sync(NS_FULL, X, src);
                 } else {
@@ -285,7 +293,7 @@ __global__ void __launch_bounds__(256) tail_kernel(const ScenarioDev sc, const S
                         }
                         const u32 okm = __ballot_sync(NS_FULL, lane >= 3u && d > 0u);
                         if (okm) {
-                            const int w = __ffs(okm) - 1;    // first accepted attempt = the sequential algorithm's choice
+                            const int w = first_bit(okm);    // first accepted attempt = the sequential algorithm's choice
                             c2 = __shfl_sync(NS_FULL, c2, w); d = __shfl_sync(NS_FULL, d, w); pf = __shfl_sync(NS_FULL, pf, w);
                             if (PERCELL) { Cm2 = __shfl_sync(NS_FULL, cs.x, w); sh2 = __shfl_sync(NS_FULL, cs.y, w); }
                             cell2 = c2;
