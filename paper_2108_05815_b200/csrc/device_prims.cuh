@@ -66,6 +66,29 @@ __host__ __device__ __forceinline__ u64 hashF(u64 x) {
     return ((u64)a << 32) | (u64)b;
 }
 
+// two / three independent evaluations of F written round by round: the compiler emits the chains as written, and a warp
+// that is alone on its scheduler then overlaps them (three in a row cost three times the latency of one)
+__device__ __forceinline__ void hashF2(u64 x0, u64 x1, u64 &y0, u64 &y1) {
+    u32 a0 = (u32)x0, b0 = (u32)(x0 >> 32), a1 = (u32)x1, b1 = (u32)(x1 >> 32);
+    feistel(a0, b0, NS_M6, NS_C6);   feistel(a1, b1, NS_M6, NS_C6);
+    feistel(a0, b0, NS_M7, NS_C7);   feistel(a1, b1, NS_M7, NS_C7);
+    feistel(a0, b0, NS_M8, NS_C8);   feistel(a1, b1, NS_M8, NS_C8);
+    feistel(a0, b0, NS_M9, NS_C9);   feistel(a1, b1, NS_M9, NS_C9);
+    feistel(a0, b0, NS_M10, NS_C10); feistel(a1, b1, NS_M10, NS_C10);
+    feistel(a0, b0, NS_M11, NS_C11); feistel(a1, b1, NS_M11, NS_C11);
+    y0 = ((u64)a0 << 32) | (u64)b0; y1 = ((u64)a1 << 32) | (u64)b1;
+}
+__device__ __forceinline__ void hashF3(u64 x0, u64 x1, u64 x2, u64 &y0, u64 &y1, u64 &y2) {
+    u32 a0 = (u32)x0, b0 = (u32)(x0 >> 32), a1 = (u32)x1, b1 = (u32)(x1 >> 32), a2 = (u32)x2, b2 = (u32)(x2 >> 32);
+    feistel(a0, b0, NS_M6, NS_C6);   feistel(a1, b1, NS_M6, NS_C6);   feistel(a2, b2, NS_M6, NS_C6);
+    feistel(a0, b0, NS_M7, NS_C7);   feistel(a1, b1, NS_M7, NS_C7);   feistel(a2, b2, NS_M7, NS_C7);
+    feistel(a0, b0, NS_M8, NS_C8);   feistel(a1, b1, NS_M8, NS_C8);   feistel(a2, b2, NS_M8, NS_C8);
+    feistel(a0, b0, NS_M9, NS_C9);   feistel(a1, b1, NS_M9, NS_C9);   feistel(a2, b2, NS_M9, NS_C9);
+    feistel(a0, b0, NS_M10, NS_C10); feistel(a1, b1, NS_M10, NS_C10); feistel(a2, b2, NS_M10, NS_C10);
+    feistel(a0, b0, NS_M11, NS_C11); feistel(a1, b1, NS_M11, NS_C11); feistel(a2, b2, NS_M11, NS_C11);
+    y0 = ((u64)a0 << 32) | (u64)b0; y1 = ((u64)a1 << 32) | (u64)b1; y2 = ((u64)a2 << 32) | (u64)b2;
+}
+
 struct SeedKey {
     u32 K[6];
 };
@@ -144,6 +167,11 @@ __device__ __forceinline__ u64 neglog(u64 x, const SmemTables &sm) {
 
 // Poisson sampler: N = #{n : c >= PC[n]}, c = F(s ^ L_COUNT). pg[b] = #{n : PC[n] < b << 56} starts a short
 // forward scan over the non-decreasing thresholds.
+__device__ __forceinline__ u32 poisson_count_of(u64 c, const SmemTables &sm) {   // c = F(s ^ L_COUNT)
+    u32 n = lds_u16(sm.pg + 2u * (u32)(c >> 56));
+    while (n < NS_POIS_N && lds_u64(sm.pc + 8u * n) <= c) ++n;
+    return n;
+}
 __device__ __forceinline__ u32 poisson_count(u64 s, const SmemTables &sm) {
     const u64 c = hashF(s ^ NS_L_COUNT);
     u32 n = lds_u16(sm.pg + 2u * (u32)(c >> 56));

@@ -75,9 +75,13 @@ __device__ __forceinline__ bool tail_search_poisson(const SeedKey &key, const Sm
     const u64 kk64 = (u64)k + seg;
     const bool kvalid = kk64 < (u64)k_stop;
     const u64 s = prime(key, loc, (u32)kk64);
-    const u32 N = poisson_count(s, smt);
     const u64 X = s + (u64)i * NS_GAMMA;
-    const u64 f = poisson_offset(X);
+    // the count, offset and thinning draws of this lane's point are independent: evaluated side by side
+    u64 hc, hf, ht = 0;
+    if (PERCELL) hashF3(s ^ NS_L_COUNT, X, X ^ NS_L_THIN, hc, hf, ht);
+    else hashF2(s ^ NS_L_COUNT, X, hc, hf);
+    const u32 N = poisson_count_of(hc, smt);
+    const u64 f = hf >> 16;
     if (__ballot_sync(NS_FULL, kvalid && N > (seg ? 8u : 16u))) {
         // more points than lanes somewhere (large mu): scan interval k one point at a time (every lane the same)
         const u64 s0 = __shfl_sync(NS_FULL, s, 0);
@@ -94,7 +98,7 @@ __device__ __forceinline__ bool tail_search_poisson(const SeedKey &key, const Sm
         return true;
     }
     bool ok = kvalid && i <= N && (seg != 0u || (i64)f > f_last);
-    if (PERCELL) ok = ok && poisson_kept(X, thin);
+    if (PERCELL) ok = ok && (thin == 0xFFFFFFFFu || (u32)ht < thin);
     u64 m = ok ? ((f << 8) | (u64)i) : ~0ull;
     m = min(m, shfl_xor_u64(m, 1)); m = min(m, shfl_xor_u64(m, 2)); m = min(m, shfl_xor_u64(m, 4));
     const u64 m16 = min(m, shfl_xor_u64(m, 8));
