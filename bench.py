@@ -142,6 +142,9 @@ def main():
     ap.add_argument("--sampler", default="exp", choices=["exp", "poisson"],
                     help="event-time sampler of the scenario (DESIGN.md 2.4 / 2.7): same law, different realisation")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--event-stream", type=int, default=0, metavar="LOG2_CAP",
+                    help="also time the path with the full event stream recorded (SURVEY NEXT-3; DESIGN.md 6.4): the stream holds up to "
+                         "2^LOG2_CAP distinct events, the per-epoch ring 2^min(LOG2_CAP, 28) records")
     args = ap.parse_args()
     name = args.config
     cfg = make_cfg(name, args.small)
@@ -259,6 +262,17 @@ def main():
                            "roofline_frac": mode_t * I_EVENT[name] / peak,
                            "ncu": "profiles/r1_ncu_simulate_kernel_c5_modeT.md (exponential sampler): issue slots 70 % active, ALU pipe 66 %, "
                                   "FMA pipe 18 % of peak, 22.1 of 32 lanes per instruction, L2 hit 98.6 %"}}
+        if args.event_stream:
+            # the same step with every executed event recorded, sorted by time and deduplicated per epoch on the device
+            pr = ns.make_params(record_events=True, event_ring_capacity=1 << min(args.event_stream, 28), event_stream_capacity=1 << args.event_stream)
+            rs, s_ms = None, 0.0
+            for i in range(1 + K):
+                flush.fill_(1)
+                torch.cuda.synchronize()
+                rs = sc.simulate_raw(seed, cfg["nu"], d_mask, n_s, pr)
+                s_ms += rs.ms_total if i else 0.0
+            line["event_stream"] = {"ms_per_step": s_ms / K, "distinct_events": int(rs.n_stream_events), "epochs": int(rs.n_epochs),
+                                    "distinct_events_per_s": int(rs.n_stream_events) * K / (s_ms * 1e-3), "launches_per_step": int(rs.n_kernel_launches)}
         if not args.no_cpu_baseline and world == 1:
             v, dt, n_ev, desc = run_oracle_sample(cfg, name)
             line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc, "seconds": dt}

@@ -132,49 +132,57 @@ __device__ __forceinline__ u32 key_byte(const SimBuffers &bf, u32 id, u32 b) {
 }
 
 #define NS_SORT_TILE 2048u
-// one LSD pass, step 1: per-block digit histogram, bin-major: hist[d * nblocks + block]
+// one LSD pass, step 1: per-block digit histogram, bin-major: hist[d * nblocks + block]. The digit of position i is kept in
+// digit[i], so that the scatter of the same pass reads it in order instead of gathering the key through perm a second time.
 __global__ void __launch_bounds__(256) radix_hist_kernel(const SimBuffers bf, const u32 *__restrict__ perm, u32 n, u32 byte,
-                                                         u32 *__restrict__ hist, u32 nblocks) {
+                                                         u32 *__restrict__ hist, u32 nblocks, uint8_t *__restrict__ digit) {
     __shared__ u32 h[256];
     h[threadIdx.x] = 0;
     __syncthreads();
     u32 start = blockIdx.x * NS_SORT_TILE;
     for (u32 r = 0; r < NS_SORT_TILE; r += 256u) {
         u32 i = start + r + threadIdx.x;
-        if (i < n) atomicAdd(&h[key_byte(bf, perm[i], byte)], 1u);
+        if (i < n) {
+            u32 d = key_byte(bf, perm[i], byte);
+            digit[i] = (uint8_t)d;
+            atomicAdd(&h[d], 1u);
+        }
     }
     __syncthreads();
     hist[threadIdx.x * nblocks + blockIdx.x] = h[threadIdx.x];
 }
-// step 3 (after an exclusive scan of hist): stable scatter
-__global__ void __launch_bounds__(256) radix_scatter_kernel(const SimBuffers bf, const u32 *__restrict__ perm_in, u32 *__restrict__ perm_out,
-                                                            u32 n, u32 byte, const u32 *__restrict__ hist, u32 nblocks) {
-    __shared__ u32 base[256];
+// step 3 (after an exclusive scan of hist): stable scatter. A warp ranks 256 consecutive positions, 32 at a time, against its own
+// digit counters (no block barrier inside the loop); the counters of the eight warps are then turned into write positions at once.
+__global__ void __launch_bounds__(256) radix_scatter_kernel(const u32 *__restrict__ perm_in, u32 *__restrict__ perm_out, u32 n,
+                                                            const u32 *__restrict__ hist, u32 nblocks, const uint8_t *__restrict__ digit) {
     __shared__ u32 wcount[8][256];
-    base[threadIdx.x] = hist[threadIdx.x * nblocks + blockIdx.x];
     const u32 lane = threadIdx.x & 31u, w = threadIdx.x >> 5;
-    u32 start = blockIdx.x * NS_SORT_TILE;
-    for (u32 r = 0; r < NS_SORT_TILE; r += 256u) {
-        for (u32 ww = 0; ww < 8; ++ww) wcount[ww][threadIdx.x] = 0;
-        __syncthreads();
-        u32 i = start + r + threadIdx.x;
+    for (u32 ww = 0; ww < 8; ++ww) wcount[ww][threadIdx.x] = 0;
+    __syncthreads();
+    const u32 start = blockIdx.x * NS_SORT_TILE + w * (NS_SORT_TILE / 8u);
+    u32 item[8], dr[8];                                 // dr = digit | rank inside the warp's 256 positions << 9
+#pragma unroll
+    for (u32 r = 0; r < 8; ++r) {
+        u32 i = start + r * 32u + lane;
         bool valid = i < n;
-        u32 item = valid ? perm_in[i] : 0u;
-        u32 d = valid ? key_byte(bf, item, byte) : 256u + lane;   // invalid lanes never match anyone
+        item[r] = valid ? perm_in[i] : 0u;
+        u32 d = valid ? (u32)digit[i] : 256u + lane;    // invalid lanes never match anyone
         u32 peers = __match_any_sync(NS_FULL, d);
-        u32 rank = __popc(peers & lanemask_lt());
-        if (valid && rank == 0) wcount[w][d] = __popc(peers);
-        __syncthreads();
-        if (valid) {
-            u32 off = base[d] + rank;
-            for (u32 ww = 0; ww < w; ++ww) off += wcount[ww][d];
-            perm_out[off] = item;
-        }
-        __syncthreads();
-        u32 add = 0;
-        for (u32 ww = 0; ww < 8; ++ww) add += wcount[ww][threadIdx.x];
-        base[threadIdx.x] += add;
-        __syncthreads();
+        u32 before = __popc(peers & lanemask_lt());
+        u32 rank = valid ? wcount[w][d] + before : 0u;
+        __syncwarp();
+        if (valid && before == 0) wcount[w][d] = rank + __popc(peers);
+        __syncwarp();
+        dr[r] = d | (rank << 9);
+    }
+    __syncthreads();
+    u32 run = hist[threadIdx.x * nblocks + blockIdx.x];   // digit threadIdx.x: the block's base, then the warps in order
+    for (u32 ww = 0; ww < 8; ++ww) { u32 c = wcount[ww][threadIdx.x]; wcount[ww][threadIdx.x] = run; run += c; }
+    __syncthreads();
+#pragma unroll
+    for (u32 r = 0; r < 8; ++r) {
+        u32 d = dr[r] & 511u;
+        if (d < 256u) perm_out[wcount[w][d] + (dr[r] >> 9)] = item[r];
     }
 }
 

@@ -465,6 +465,7 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
     necsim_event *events = (necsim_event *)(base + L.off_events);
     u32 *labels = (u32 *)(base + L.off_labels), *species_of = (u32 *)(base + L.off_species);
     u32 *perm_a = (u32 *)(base + L.off_perm_a), *perm_b = (u32 *)(base + L.off_perm_b), *flag = (u32 *)(base + L.off_flag);
+    uint8_t *digit = (uint8_t *)flag;   // the head flags are written after the sort: the same memory holds a pass's digits
     u32 *hist = (u32 *)(base + L.off_hist), *chunk = (u32 *)(base + L.off_chunk), *scan_tmp = (u32 *)(base + L.off_scan);
     bf.rec_loc = (u32 *)(base + L.off_rec_loc); bf.rec_k = (u32 *)(base + L.off_rec_k); bf.rec_j = (u32 *)(base + L.off_rec_j);
     bf.rec_loc2 = (u32 *)(base + L.off_rec_l2); bf.rec_f = (u64 *)(base + L.off_rec_f); bf.rec_cap = (u32)rp.ring_cap;
@@ -607,9 +608,9 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
                 else if (b < 14) needed = true;
                 else needed = (kmax >> (8 * (b - 14))) != 0;
                 if (!needed) continue;
-                radix_hist_kernel<<<nb, 256, 0, st>>>(vb, src, nr, b, hist, nb);
+                radix_hist_kernel<<<nb, 256, 0, st>>>(vb, src, nr, b, hist, nb, digit);
                 n_launch += 2 + scan_u32(hist, 256 * nb, scan_tmp, NULL, st);
-                radix_scatter_kernel<<<nb, 256, 0, st>>>(vb, src, dst, nr, b, hist, nb);
+                radix_scatter_kernel<<<nb, 256, 0, st>>>(src, dst, nr, hist, nb, digit);
                 std::swap(src, dst);
             }
             stream_flag_kernel<<<g256, 256, 0, st>>>(vb, src, nr, k_stop, flag);
@@ -647,9 +648,9 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
             else if (b < 14) needed = true;
             else needed = (maxv[3] >> (8 * (b - 14))) != 0;
             if (!needed) continue;
-            radix_hist_kernel<<<nb, 256, 0, st>>>(bf, src, n_spec, b, hist, nb);
+            radix_hist_kernel<<<nb, 256, 0, st>>>(bf, src, n_spec, b, hist, nb, digit);
             n_launch += 2 + scan_u32(hist, 256 * nb, scan_tmp, NULL, st);
-            radix_scatter_kernel<<<nb, 256, 0, st>>>(bf, src, dst, n_spec, b, hist, nb);
+            radix_scatter_kernel<<<nb, 256, 0, st>>>(src, dst, n_spec, hist, nb, digit);
             src = dst; std::swap(dst, other);
         }
         CU(cudaGetLastError());
@@ -757,9 +758,9 @@ extern "C" int necsim_merge_species(const necsim_event *d_in, uint64_t n64, void
     merge_unpack_kernel<<<g256, 256, 0, st>>>(d_in, n, bf, pa);
     u32 *src = pa, *dst = pb;
     for (u32 b = 0; b < 18; ++b) {   // all 18 key bytes: the tables are small (thousands of records)
-        radix_hist_kernel<<<L.nb, 256, 0, st>>>(bf, src, n, b, hist, L.nb);
+        radix_hist_kernel<<<L.nb, 256, 0, st>>>(bf, src, n, b, hist, L.nb, (uint8_t *)flag);
         scan_exclusive_kernel<<<1, 1024, 0, st>>>(hist, 256 * L.nb, NULL);
-        radix_scatter_kernel<<<L.nb, 256, 0, st>>>(bf, src, dst, n, b, hist, L.nb);
+        radix_scatter_kernel<<<L.nb, 256, 0, st>>>(src, dst, n, hist, L.nb, (const uint8_t *)flag);
         std::swap(src, dst);
     }
     unique_flag_kernel<<<g256, 256, 0, st>>>(bf, src, n, flag);
