@@ -256,6 +256,32 @@ __global__ void __launch_bounds__(256) iota_kernel(u32 *perm, u32 n) {
     u32 i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i < n) perm[i] = i;
 }
+// The ring is radix-sorted on a prefix of its key only: k and the top `fbytes` bytes of f. Records that share the prefix are
+// adjacent and few (redundant executions of one event, and distinct events whose offsets agree in the leading bits), so the
+// first thread of such a run puts it into full (f, loc, j) order by insertion. Runs of sentinels stay as they are.
+__device__ __forceinline__ bool stream_less(const SimBuffers &bf, u32 a, u32 b) {   // same k: order by (f, loc, j)
+    const u64 fa = bf.term_f[a], fb = bf.term_f[b];
+    if (fa != fb) return fa < fb;
+    const u32 la = bf.term_loc[a], lb = bf.term_loc[b];
+    if (la != lb) return la < lb;
+    return bf.term_j[a] < bf.term_j[b];
+}
+__global__ void __launch_bounds__(256) stream_ties_kernel(const SimBuffers bf, u32 *__restrict__ perm, u32 n, u32 k_sentinel, u32 fbytes) {
+    u32 i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i + 1 >= n) return;
+    const u32 sh = 48u - 8u * fbytes;
+    const u32 id = perm[i], k = bf.term_k[id];
+    if (k == k_sentinel) return;
+    const u64 fp = bf.term_f[id] >> sh;
+    if (i != 0) { const u32 pv = perm[i - 1]; if (bf.term_k[pv] == k && (bf.term_f[pv] >> sh) == fp) return; }   // not the first of its run
+    for (u32 p = i + 1; p < n; ++p) {
+        const u32 x = perm[p];
+        if (bf.term_k[x] != k || (bf.term_f[x] >> sh) != fp) break;
+        u32 q = p;
+        while (q > i && stream_less(bf, x, perm[q - 1])) { perm[q] = perm[q - 1]; --q; }
+        perm[q] = x;
+    }
+}
 // head flags over the sorted ring; sentinel records (k = the epoch's k_stop: reserved but unused slots) sort last and count for nothing
 __global__ void __launch_bounds__(256) stream_flag_kernel(const SimBuffers bf, const u32 *__restrict__ perm, u32 n, u32 k_sentinel, u32 *__restrict__ flag) {
     u32 i = blockIdx.x * blockDim.x + threadIdx.x;

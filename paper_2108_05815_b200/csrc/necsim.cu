@@ -339,6 +339,7 @@ extern "C" int necsim_destroy(necsim_scenario *scn) {
 struct ResolvedParams {
     u32 block_threads, grid_blocks, dedup_log2_slots, tail_threshold, probe_mask;
     bool dedup, record;
+    u32 stream_fbytes;
     u64 epoch_events, max_steps, ring_cap, stream_cap;
 };
 
@@ -358,6 +359,8 @@ static int resolve_params(const necsim_scenario *scn, const necsim_sim_params *p
     if (r.max_steps > 0xFFFFFFFFull) return fail(NECSIM_ERR_INVALID_ARG, "max_steps must fit 32 bits");
     r.tail_threshold = p->tail_threshold;
     r.record = p->record_events != 0;
+    if (p->stream_sort_bytes > 6) return fail(NECSIM_ERR_INVALID_ARG, "stream_sort_bytes must be in [0, 6]");
+    r.stream_fbytes = p->stream_sort_bytes ? p->stream_sort_bytes : 4u;
     r.ring_cap = r.record ? (p->event_ring_capacity ? p->event_ring_capacity : (1ull << 24)) : 0;
     r.stream_cap = r.record ? (p->event_stream_capacity ? p->event_stream_capacity : (1ull << 26)) : 0;
     if (r.ring_cap >= (1ull << 32)) return fail(NECSIM_ERR_INVALID_ARG, "event_ring_capacity must be < 2^32");
@@ -600,19 +603,18 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
             iota_kernel<<<g256, 256, 0, st>>>(perm_a, nr);
             u32 *src = perm_a, *dst = perm_b;
             vb.k_base = ep.k_start;
-            const u32 kmax = k_stop - ep.k_start, lmax = (u32)(sd.n_locations - 1);   // sentinels carry k = k_stop
-            for (u32 b = 0; b < 18; ++b) {   // j: two bytes (ordinals stay far below 2^16 for mu <= 64), loc and k: the bytes in use
-                bool needed;
-                if (b < 4) needed = b < 2;
-                else if (b < 8) needed = (lmax >> (8 * (b - 4))) != 0;
-                else if (b < 14) needed = true;
-                else needed = (kmax >> (8 * (b - 14))) != 0;
-                if (!needed) continue;
+            const u32 kmax = k_stop - ep.k_start;   // sentinels carry k = k_stop
+            // radix passes over k (the bytes in use) and the leading bytes of f only; the few records that agree there are put in
+            // (f, loc, j) order by stream_ties_kernel
+            for (u32 b = 14u - rp.stream_fbytes; b < 18; ++b) {
+                if (b >= 14 && (kmax >> (8 * (b - 14))) == 0) continue;
                 radix_hist_kernel<<<nb, 256, 0, st>>>(vb, src, nr, b, hist, nb, digit);
                 n_launch += 2 + scan_u32(hist, 256 * nb, scan_tmp, NULL, st);
                 radix_scatter_kernel<<<nb, 256, 0, st>>>(src, dst, nr, hist, nb, digit);
                 std::swap(src, dst);
             }
+            stream_ties_kernel<<<g256, 256, 0, st>>>(vb, src, nr, k_stop, rp.stream_fbytes);
+            ++n_launch;
             stream_flag_kernel<<<g256, 256, 0, st>>>(vb, src, nr, k_stop, flag);
             n_launch += scan_u32(flag, nr, scan_tmp, &bf.ctr->q_head, st) - 1;   // q_head reused: distinct events of the epoch
             stream_write_kernel<<<g256, 256, 0, st>>>(vb, bf.rec_loc2, src, nr, flag, k_stop, stream_n, rp.stream_cap, st_loc, st_k, st_j, st_f, st_l2);

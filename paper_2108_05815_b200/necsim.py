@@ -30,7 +30,7 @@ class ScenarioDesc(C.Structure):
 class SimParams(C.Structure):
     _fields_ = [("block_threads", C.c_uint32), ("grid_blocks", C.c_uint32), ("dedup", C.c_uint32),
                 ("dedup_log2_slots", C.c_uint32), ("epoch_events", C.c_uint64), ("max_steps", C.c_uint64),
-                ("tail_threshold", C.c_uint32), ("dedup_probe", C.c_uint32), ("record_events", C.c_uint32), ("reserved", C.c_uint32),
+                ("tail_threshold", C.c_uint32), ("dedup_probe", C.c_uint32), ("record_events", C.c_uint32), ("stream_sort_bytes", C.c_uint32),
                 ("event_ring_capacity", C.c_uint64), ("event_stream_capacity", C.c_uint64)]
 
 
@@ -120,13 +120,14 @@ def _dev_u32(torch, a, n=None):
 
 
 def make_params(block_threads=0, grid_blocks=0, dedup=None, dedup_log2_slots=0, epoch_events=0, max_steps=0, tail_threshold=0,
-                dedup_probe=0, record_events=False, event_ring_capacity=0, event_stream_capacity=0):
+                dedup_probe=0, record_events=False, event_ring_capacity=0, event_stream_capacity=0, stream_sort_bytes=0):
     p = SimParams()
     p.block_threads, p.grid_blocks = block_threads, grid_blocks
     p.dedup = 0 if dedup is None else (1 if dedup else 2)
     p.dedup_log2_slots, p.epoch_events, p.max_steps, p.tail_threshold = dedup_log2_slots, epoch_events, max_steps, tail_threshold
     p.dedup_probe = dedup_probe
     p.record_events = 1 if record_events else 0
+    p.stream_sort_bytes = int(stream_sort_bytes)
     p.event_ring_capacity, p.event_stream_capacity = int(event_ring_capacity), int(event_stream_capacity)
     return p
 
