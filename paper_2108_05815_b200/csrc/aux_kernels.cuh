@@ -266,39 +266,39 @@ __device__ __forceinline__ bool stream_less(const SimBuffers &bf, u32 a, u32 b) 
     if (la != lb) return la < lb;
     return bf.term_j[a] < bf.term_j[b];
 }
-__global__ void __launch_bounds__(256) stream_ties_kernel(const SimBuffers bf, u32 *__restrict__ perm, u32 n, u32 k_sentinel, u32 fbytes) {
+// Also writes the head flags of the sorted ring: 1 for the first record of every distinct event, 0 for its redundant copies
+// (adjacent after the sort) and for sentinel records (k = the epoch's k_stop: reserved but unused slots, sorted last).
+__global__ void __launch_bounds__(256) stream_ties_kernel(const SimBuffers bf, u32 *__restrict__ perm, u32 n, u32 k_sentinel, u32 fbytes,
+                                                          u32 *__restrict__ flag) {
     u32 i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i + 1 >= n) return;
+    if (i >= n) return;
     const u32 sh = 48u - 8u * fbytes;
     const u32 id = perm[i], k = bf.term_k[id];
-    if (k == k_sentinel) return;
+    if (k == k_sentinel) { flag[i] = 0u; return; }
     const u64 fp = bf.term_f[id] >> sh;
     if (i != 0) { const u32 pv = perm[i - 1]; if (bf.term_k[pv] == k && (bf.term_f[pv] >> sh) == fp) return; }   // not the first of its run
-    for (u32 p = i + 1; p < n; ++p) {
-        const u32 x = perm[p];
+    flag[i] = 1u;
+    u32 e = i + 1;
+    for (; e < n; ++e) {
+        const u32 x = perm[e];
         if (bf.term_k[x] != k || (bf.term_f[x] >> sh) != fp) break;
-        u32 q = p;
+        u32 q = e;
         while (q > i && stream_less(bf, x, perm[q - 1])) { perm[q] = perm[q - 1]; --q; }
         perm[q] = x;
     }
+    for (u32 p = i + 1; p < e; ++p) flag[p] = same_event(bf, perm[p], perm[p - 1]) ? 0u : 1u;
 }
-// head flags over the sorted ring; sentinel records (k = the epoch's k_stop: reserved but unused slots) sort last and count for nothing
-__global__ void __launch_bounds__(256) stream_flag_kernel(const SimBuffers bf, const u32 *__restrict__ perm, u32 n, u32 k_sentinel, u32 *__restrict__ flag) {
-    u32 i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    const u32 id = perm[i];
-    flag[i] = (bf.term_k[id] != k_sentinel && (i == 0 || !same_event(bf, id, perm[i - 1]))) ? 1u : 0u;
-}
-// bf.term_* alias the ring's key arrays; duplicates of an event are adjacent after the sort: keep the first
+// bf.term_* alias the ring's key arrays; uidx = the head flags scanned exclusively, *total = their sum: the heads are written
 __global__ void __launch_bounds__(256) stream_write_kernel(const SimBuffers bf, const u32 *__restrict__ rec_loc2, const u32 *__restrict__ perm, u32 n,
-                                                           const u32 *__restrict__ uidx, u32 k_sentinel, u64 base, u64 cap, u32 *__restrict__ s_loc, u32 *__restrict__ s_k,
-                                                           u32 *__restrict__ s_j, u64 *__restrict__ s_f, u32 *__restrict__ s_loc2) {
+                                                           const u32 *__restrict__ uidx, const u32 *__restrict__ total, u64 base, u64 cap, u32 *__restrict__ s_loc,
+                                                           u32 *__restrict__ s_k, u32 *__restrict__ s_j, u64 *__restrict__ s_f, u32 *__restrict__ s_loc2) {
     u32 i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    const u32 id = perm[i];
-    if (bf.term_k[id] == k_sentinel || (i != 0 && same_event(bf, id, perm[i - 1]))) return;
-    const u64 o = base + uidx[i];
+    const u32 u = uidx[i], nx = (i + 1 < n) ? uidx[i + 1] : *total;
+    if (nx == u) return;
+    const u64 o = base + u;
     if (o >= cap) return;
+    const u32 id = perm[i];
     s_loc[o] = bf.term_loc[id]; s_k[o] = bf.term_k[id]; s_j[o] = bf.term_j[id]; s_f[o] = bf.term_f[id]; s_loc2[o] = rec_loc2[id];
 }
 

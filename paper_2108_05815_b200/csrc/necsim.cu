@@ -613,11 +613,9 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
                 radix_scatter_kernel<<<nb, 256, 0, st>>>(src, dst, nr, hist, nb, digit);
                 std::swap(src, dst);
             }
-            stream_ties_kernel<<<g256, 256, 0, st>>>(vb, src, nr, k_stop, rp.stream_fbytes);
-            ++n_launch;
-            stream_flag_kernel<<<g256, 256, 0, st>>>(vb, src, nr, k_stop, flag);
+            stream_ties_kernel<<<g256, 256, 0, st>>>(vb, src, nr, k_stop, rp.stream_fbytes, flag);
             n_launch += scan_u32(flag, nr, scan_tmp, &bf.ctr->q_head, st) - 1;   // q_head reused: distinct events of the epoch
-            stream_write_kernel<<<g256, 256, 0, st>>>(vb, bf.rec_loc2, src, nr, flag, k_stop, stream_n, rp.stream_cap, st_loc, st_k, st_j, st_f, st_l2);
+            stream_write_kernel<<<g256, 256, 0, st>>>(vb, bf.rec_loc2, src, nr, flag, &bf.ctr->q_head, stream_n, rp.stream_cap, st_loc, st_k, st_j, st_f, st_l2);
             n_launch += 4;
             CU(cudaGetLastError());
             u32 heads = 0;
