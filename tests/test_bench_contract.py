@@ -59,3 +59,13 @@ def test_product_arm_line(config, sampler):
     assert {"sm_mhz", "sm_max_mhz", "reasons"} <= set(r["clocks"])
     cb = r["cpu_baseline"]
     assert cb["kind"] == "oracle" and cb["value"] > 0 and cb["cores"] == 1 and cb["sample"]
+
+
+@pytest.mark.gpu
+def test_product_arm_event_stream_leg():
+    """--event-stream adds the step timed with the full event stream recorded to the same line."""
+    lines = run_bench("--small", "--config", "c4", "--event-stream", "22", "--steps", "1", "--warmup", "3", "--no-cpu-baseline")
+    assert len(lines) == 1
+    r = json.loads(lines[0])
+    s = r["event_stream"]
+    assert s["ms_per_step"] > 0 and s["distinct_events"] >= r["richness"] > 0 and s["distinct_events_per_s"] > 0 and s["epochs"] >= 1
