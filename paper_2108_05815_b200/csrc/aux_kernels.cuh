@@ -270,13 +270,19 @@ __device__ __forceinline__ bool stream_less(const SimBuffers &bf, u32 a, u32 b) 
 // (adjacent after the sort) and for sentinel records (k = the epoch's k_stop: reserved but unused slots, sorted last).
 __global__ void __launch_bounds__(256) stream_ties_kernel(const SimBuffers bf, u32 *__restrict__ perm, u32 n, u32 k_sentinel, u32 fbytes,
                                                           u32 *__restrict__ flag) {
-    u32 i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
+    const u32 i = blockIdx.x * blockDim.x + threadIdx.x, lane = threadIdx.x & 31u;
+    const bool in = i < n;
     const u32 sh = 48u - 8u * fbytes;
-    const u32 id = perm[i], k = bf.term_k[id];
+    const u32 id = in ? perm[i] : 0u, k = in ? bf.term_k[id] : k_sentinel;
+    const u64 fp = in ? bf.term_f[id] >> sh : 0ull;
+    // the previous record's prefix comes from the neighbouring lane (a record a run's first thread is moving at this moment
+    // is still one of that run: the answer is the same)
+    u32 pk = __shfl_up_sync(NS_FULL, k, 1);
+    u64 pf = __shfl_up_sync(NS_FULL, fp, 1);
+    if (in && lane == 0 && i != 0) { const u32 pv = perm[i - 1]; pk = bf.term_k[pv]; pf = bf.term_f[pv] >> sh; }
+    if (!in) return;
     if (k == k_sentinel) { flag[i] = 0u; return; }
-    const u64 fp = bf.term_f[id] >> sh;
-    if (i != 0) { const u32 pv = perm[i - 1]; if (bf.term_k[pv] == k && (bf.term_f[pv] >> sh) == fp) return; }   // not the first of its run
+    if (i != 0 && pk == k && pf == fp) return;   // not the first of its run
     flag[i] = 1u;
     u32 e = i + 1;
     for (; e < n; ++e) {
