@@ -131,6 +131,9 @@ typedef struct necsim_result {
     const uint32_t *d_stream_loc, *d_stream_k, *d_stream_j, *d_stream_loc2;
     const uint64_t *d_stream_f;
     uint64_t n_stream_events;
+    /* tail kernel (exponential sampler): search rounds done in exact arithmetic (a fast round that was not clean is redone so,
+     * DESIGN.md section 5); compare with n_events_tail. Reported, never compared */
+    uint64_t n_tail_rounds_exact;
 } necsim_result;
 
 typedef struct necsim_scenario necsim_scenario;
@@ -225,8 +228,9 @@ int necsim_debug_next_event_poisson(const necsim_scenario *scn, uint64_t seed, c
 int necsim_debug_poisson_table(const necsim_scenario *scn, uint64_t *h_pc, uint32_t *h_thin, double *mu_max, void *cuda_stream);
 /* integer-pipe peak micro-benchmark: runs `iters` iterations of an unrolled chain of
  * independent IMAD.WIDE / LOP3 / SHF / IADD3 on every SM; kind 0 = mixed hash-like, 1 = IMAD only,
- * 2 = ALU (LOP3/SHF/IADD3) only. Returns thread-level integer instructions per second. */
-int necsim_debug_int_peak(int kind, uint32_t iters, void *cuda_stream, double *thread_instr_per_s /*HOST out*/,
+ * 2 = ALU (LOP3/SHF/IADD3) only. d_sink: DEVICE, 4 bytes of the caller (keeps the chains alive; never written in practice).
+ * Returns thread-level integer instructions per second. */
+int necsim_debug_int_peak(int kind, uint32_t iters, uint32_t *d_sink /*DEVICE*/, void *cuda_stream, double *thread_instr_per_s /*HOST out*/,
                           float *ms /*HOST out*/);
 
 #ifdef __cplusplus

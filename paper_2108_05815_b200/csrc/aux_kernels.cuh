@@ -9,14 +9,6 @@ namespace necsim {
 
 #define NS_CHUNK 4096u   // mask bytes per block in the compaction kernels (256 threads x 16 bytes)
 
-// cell of an indexed location: last cell with prefix[cell] <= loc (that cell has deme > 0)
-__device__ __forceinline__ u32 cell_of_loc(const ScenarioDev &sc, u32 loc) {
-    if (sc.kind == 0 || sc.kind == 1) return 0;      // non-spatial; implicit: only the local community is sampled
-    if (sc.uniform_deme) return loc / sc.uniform_deme;
-    u32 lo = 0, hi = sc.ncells;                      // invariant: prefix[lo] <= loc < prefix[hi]
-    while (hi - lo > 1) { u32 mid = lo + ((hi - lo) >> 1); if (sc.prefix[mid] <= loc) lo = mid; else hi = mid; }
-    return lo;
-}
 // the `cell` word of a queue entry: the cell index, or packed (y << 16 | x) for EXPLICIT_GAUSSIAN
 __device__ __forceinline__ u32 queue_cell(const ScenarioDev &sc, u32 loc) {
     const u32 c = cell_of_loc(sc, loc);

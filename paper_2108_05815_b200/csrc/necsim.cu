@@ -107,10 +107,10 @@ struct necsim_scenario {
 };
 
 struct ScenarioLayout {
-    size_t off_hab8, off_deme32, off_prefix, off_pois, off_thin, off_scale, off_alias, off_gauss, total;
-    u32 ncells, gauss_len;
+    size_t off_hab8, off_deme32, off_prefix, off_pois, off_thin, off_scale, off_alias, off_gauss, off_hab64, total;
+    u32 ncells, gauss_len, nbx, compact_deme;
     int R;
-    bool uniform_deme, need_deme32, per_cell_turnover;
+    bool uniform_deme, need_deme32, per_cell_turnover, compact;
 };
 
 static int scenario_layout(const necsim_scenario_desc *d, ScenarioLayout &L) {
@@ -157,6 +157,14 @@ static int scenario_layout(const necsim_scenario_desc *d, ScenarioLayout &L) {
         if (len > 1024u) return fail(NECSIM_ERR_UNSUPPORTED, "sigma too large: the threshold table must fit 1024 entries");
         L.gauss_len = len;
         L.off_gauss = off; off = align256(off + 4 * (size_t)len);
+        // compact habitat table: every habitat cell holds the same number of individuals
+        u32 D = 0; bool same = true;
+        if (L.uniform_deme) D = d->uniform_deme;
+        else for (u32 c = 0; c < L.ncells && same; ++c) if (d->deme[c]) { if (!D) D = d->deme[c]; else same = (d->deme[c] == D); }
+        if (same && D) {
+            L.compact = true; L.compact_deme = D; L.nbx = (d->width + 31u) / 32u;
+            L.off_hab64 = off; off = align256(off + 8 * (size_t)L.nbx * d->height);
+        }
     }
     L.total = off ? off : 256;
     return NECSIM_OK;
@@ -279,6 +287,18 @@ extern "C" int necsim_create_scenario(const necsim_scenario_desc *d, void *d_wor
             CU(cudaMemcpyAsync(base + L.off_gauss, tg.data(), 4 * (size_t)L.gauss_len, cudaMemcpyHostToDevice, st));
             CU(cudaStreamSynchronize(st));
             sd.gauss = (const u32 *)(base + L.off_gauss); sd.R = L.R; sd.gauss_len = L.gauss_len;
+            if (L.compact) {   // {habitat mask, prefix at the block's first cell} per 32-cell block of a row
+                std::vector<uint2> hb((size_t)L.nbx * d->height);
+                for (u32 y = 0; y < d->height; ++y)
+                    for (u32 b = 0; b < L.nbx; ++b) {
+                        u32 m = 0;
+                        for (u32 t = 0; t < 32u && b * 32u + t < d->width; ++t) if (hab8[(size_t)y * d->width + b * 32u + t]) m |= 1u << t;
+                        hb[(size_t)y * L.nbx + b] = make_uint2(m, prefix[(size_t)y * d->width + b * 32u]);
+                    }
+                CU(cudaMemcpyAsync(base + L.off_hab64, hb.data(), 8 * hb.size(), cudaMemcpyHostToDevice, st));
+                CU(cudaStreamSynchronize(st));
+                sd.hab64 = (const uint2 *)(base + L.off_hab64); sd.nbx = L.nbx; sd.compact_deme = L.compact_deme;
+            }
         }
     }
     sd.sampler = d->sampler;
@@ -424,23 +444,29 @@ static u32 scan_u32(u32 *a, u32 n, u32 *sums, u32 *d_total, cudaStream_t st) {  
     return 3;
 }
 
+template <int KIND, bool PERCELL, int SAMP, bool REC, bool COMPACT>
+static EpochKernel pick_kernel5(bool dedup, bool tail) {
+    if (tail) return dedup ? (EpochKernel)tail_kernel<KIND, true, PERCELL, SAMP, REC, COMPACT> : (EpochKernel)tail_kernel<KIND, false, PERCELL, SAMP, REC, COMPACT>;
+    return dedup ? (EpochKernel)simulate_kernel<KIND, true, PERCELL, SAMP, REC, COMPACT> : (EpochKernel)simulate_kernel<KIND, false, PERCELL, SAMP, REC, COMPACT>;
+}
+// the compact habitat table exists for EXPLICIT_GAUSSIAN only
 template <int KIND, bool PERCELL, int SAMP, bool REC>
-static EpochKernel pick_kernel4(bool dedup, bool tail) {
-    if (tail) return dedup ? (EpochKernel)tail_kernel<KIND, true, PERCELL, SAMP, REC> : (EpochKernel)tail_kernel<KIND, false, PERCELL, SAMP, REC>;
-    return dedup ? (EpochKernel)simulate_kernel<KIND, true, PERCELL, SAMP, REC> : (EpochKernel)simulate_kernel<KIND, false, PERCELL, SAMP, REC>;
+static EpochKernel pick_kernel4(bool dedup, bool tail, bool compact) {
+    if (KIND == 3 && compact) return pick_kernel5<KIND, PERCELL, SAMP, REC, KIND == 3>(dedup, tail);
+    return pick_kernel5<KIND, PERCELL, SAMP, REC, false>(dedup, tail);
 }
 template <int KIND, bool PERCELL>
-static EpochKernel pick_kernel2(int sampler, bool rec, bool dedup, bool tail) {
-    if (sampler) return rec ? pick_kernel4<KIND, PERCELL, 1, true>(dedup, tail) : pick_kernel4<KIND, PERCELL, 1, false>(dedup, tail);
-    return rec ? pick_kernel4<KIND, PERCELL, 0, true>(dedup, tail) : pick_kernel4<KIND, PERCELL, 0, false>(dedup, tail);
+static EpochKernel pick_kernel2(int sampler, bool rec, bool dedup, bool tail, bool compact) {
+    if (sampler) return rec ? pick_kernel4<KIND, PERCELL, 1, true>(dedup, tail, compact) : pick_kernel4<KIND, PERCELL, 1, false>(dedup, tail, compact);
+    return rec ? pick_kernel4<KIND, PERCELL, 0, true>(dedup, tail, compact) : pick_kernel4<KIND, PERCELL, 0, false>(dedup, tail, compact);
 }
 // per-cell turnover exists for the explicit kinds only
-static EpochKernel pick_kernel(int kind, bool percell, int sampler, bool rec, bool dedup, bool tail) {
+static EpochKernel pick_kernel(int kind, bool percell, int sampler, bool rec, bool dedup, bool tail, bool compact) {
     switch (kind) {
-    case 0: return pick_kernel2<0, false>(sampler, rec, dedup, tail);
-    case 1: return pick_kernel2<1, false>(sampler, rec, dedup, tail);
-    case 2: return percell ? pick_kernel2<2, true>(sampler, rec, dedup, tail) : pick_kernel2<2, false>(sampler, rec, dedup, tail);
-    default: return percell ? pick_kernel2<3, true>(sampler, rec, dedup, tail) : pick_kernel2<3, false>(sampler, rec, dedup, tail);
+    case 0: return pick_kernel2<0, false>(sampler, rec, dedup, tail, false);
+    case 1: return pick_kernel2<1, false>(sampler, rec, dedup, tail, false);
+    case 2: return percell ? pick_kernel2<2, true>(sampler, rec, dedup, tail, false) : pick_kernel2<2, false>(sampler, rec, dedup, tail, false);
+    default: return percell ? pick_kernel2<3, true>(sampler, rec, dedup, tail, compact) : pick_kernel2<3, false>(sampler, rec, dedup, tail, compact);
     }
 }
 static int occupancy_for(EpochKernel fn, u32 block) {
@@ -510,8 +536,8 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
     ep.thr_nu = thr53(nu);
     ep.thr_m = thr53(scn->migration);
     ep.max_steps = (u32)rp.max_steps;
-    const EpochKernel fn_main = pick_kernel(sd.kind, sd.per_cell_turnover != 0, (int)sd.sampler, rp.record, rp.dedup, false);
-    const EpochKernel fn_tail = pick_kernel(sd.kind, sd.per_cell_turnover != 0, (int)sd.sampler, rp.record, rp.dedup, true);
+    const EpochKernel fn_main = pick_kernel(sd.kind, sd.per_cell_turnover != 0, (int)sd.sampler, rp.record, rp.dedup, false, sd.hab64 != NULL);
+    const EpochKernel fn_tail = pick_kernel(sd.kind, sd.per_cell_turnover != 0, (int)sd.sampler, rp.record, rp.dedup, true, sd.hab64 != NULL);
     const int occ = occupancy_for(fn_main, rp.block_threads);
     const int occ_tail = occupancy_for(fn_tail, rp.block_threads);
     ep.probe_mask = rp.probe_mask;
@@ -682,6 +708,7 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
     out->n_events_raw = hc->n_events; out->n_culled = hc->n_culled; out->n_speciation_raw = n_spec; out->n_epochs = n_epochs;
     out->resample_attempts = hc->resamples; out->ms_simulate = ms_sim; out->ms_simulate_tail = ms_tail; out->n_tail_epochs = n_tail_epochs; out->n_events_tail = ev_tail;
     out->ms_total = ms_total; out->n_kernel_launches = n_launch;
+    out->n_tail_rounds_exact = hc->tail_rounds_exact;
     if (rp.record) {
         out->d_stream_loc = st_loc; out->d_stream_k = st_k; out->d_stream_j = st_j; out->d_stream_loc2 = st_l2; out->d_stream_f = st_f;
         out->n_stream_events = stream_n;
@@ -1006,13 +1033,13 @@ __global__ void __launch_bounds__(256) int_peak_kernel(u32 iters, u32 *sink) {
     if (r == 0x12345678u) sink[0] = r;   // keeps the chains alive
 }
 
-extern "C" int necsim_debug_int_peak(int kind, uint32_t iters, void *cuda_stream, double *thread_instr_per_s, float *ms_out) {
+extern "C" int necsim_debug_int_peak(int kind, uint32_t iters, uint32_t *d_sink, void *cuda_stream, double *thread_instr_per_s, float *ms_out) {
+    if (!d_sink) return fail(NECSIM_ERR_INVALID_ARG, "d_sink is NULL (a 4-byte device buffer of the caller)");
     cudaStream_t st = (cudaStream_t)cuda_stream;
     int dev_id = 0, sm = 0;
     CU(cudaGetDevice(&dev_id));
     CU(cudaDeviceGetAttribute(&sm, cudaDevAttrMultiProcessorCount, dev_id));
-    u32 *sink = NULL;
-    CU(cudaMalloc((void **)&sink, 4));   // test-only export: the one place the library allocates
+    u32 *sink = d_sink;
     cudaEvent_t e0, e1;
     CU(cudaEventCreate(&e0)); CU(cudaEventCreate(&e1));
     const u32 grid = (u32)sm * 8u, block = 256u;
@@ -1030,6 +1057,6 @@ extern "C" int necsim_debug_int_peak(int kind, uint32_t iters, void *cuda_stream
     CU(cudaEventElapsedTime(&ms, e0, e1));
     if (ms_out) *ms_out = ms;
     if (thread_instr_per_s) *thread_instr_per_s = per_step * 8.0 * (double)iters * (double)grid * (double)block / ((double)ms * 1e-3);
-    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(sink);
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
     return NECSIM_OK;
 }

@@ -81,6 +81,14 @@ __device__ __forceinline__ u32 cell_deme(const ScenarioDev &sc, u32 cell) {
 }
 __device__ __forceinline__ u32 cell_prefix(const ScenarioDev &sc, u32 cell) { return __ldg(&sc.prefix[cell]); }
 
+// cell of an indexed location: last cell with prefix[cell] <= loc (that cell has deme > 0)
+__device__ __forceinline__ u32 cell_of_loc(const ScenarioDev &sc, u32 loc) {
+    if (sc.kind == 0 || sc.kind == 1) return 0;      // non-spatial; implicit: only the local community is sampled
+    if (sc.uniform_deme) return loc / sc.uniform_deme;
+    u32 lo = 0, hi = sc.ncells;                      // invariant: prefix[lo] <= loc < prefix[hi]
+    while (hi - lo > 1) { u32 mid = lo + ((hi - lo) >> 1); if (sc.prefix[mid] <= loc) lo = mid; else hi = mid; }
+    return lo;
+}
 // EXPLICIT_GAUSSIAN lineages carry their cell as packed coordinates (y << 16 | x): no division on the hot path.
 __device__ __forceinline__ u32 pack_xy(const ScenarioDev &sc, u32 cell) {
     u32 y = cell / sc.width;
@@ -140,16 +148,10 @@ __device__ __forceinline__ bool disperse(const ScenarioDev &sc, u64 thr_m, u64 X
     }
 }
 
-__device__ __forceinline__ u32 cache_hash(u32 loc, u32 k, u32 j) {
-    // the hash only chooses a bucket (low bits) and whether the event probes at all (top 3 bits);
-    // a hit always compares the full key
-    u32 h = loc * 0x9E3779B1u;
-    h ^= (k + j * 0x7FEB352Du) * 0x85EBCA6Bu;
-    h ^= h >> 15;
-    h *= 0x2C1B3C6Du;
-    h ^= h >> 13;
-    return h;
-}
+// The event's stream position X = prime(loc, k) + j * GAMMA is already a well-mixed function of the event identity (six keyed
+// Feistel rounds): folded to 32 bits it chooses the bucket (low bits) and whether the event probes at all (top 3 bits).
+// A hit always compares the full key. Every kernel uses this function: entries live across launches.
+__device__ __forceinline__ u32 cache_hash(u64 X) { return (u32)X ^ (u32)(X >> 32); }
 __device__ __forceinline__ bool cache_probes(u32 h, u32 probe_mask) { return ((h >> 29) & probe_mask) == 0u; }
 
 // -ln tables in global memory (filled once per process from neglog_tables.inc), staged to smem per block
@@ -188,7 +190,7 @@ __device__ __forceinline__ void record_event(const SimBuffers &bf, u32 loc, u32 
 
 // SAMP: 0 = exponential event-time sampler, 1 = Poisson / order statistics (2.7)
 // REC: also append every executed event to the stream ring (NEXT-3)
-template <int KIND, bool DEDUP, bool PERCELL, int SAMP, bool REC>
+template <int KIND, bool DEDUP, bool PERCELL, int SAMP, bool REC, bool COMPACT>
 __global__ void __launch_bounds__(256) simulate_kernel(const ScenarioDev sc, const SimBuffers bf, const EpochArgs ep) {
     __shared__ unsigned short sQ[SAMP == 0 ? 512 : 256];      // SAMP 1: the Poisson guide
     __shared__ u64 sA[SAMP == 0 ? 512 : 256];                 // SAMP 1: the Poisson cdf thresholds
@@ -300,7 +302,7 @@ __global__ void __launch_bounds__(256) simulate_kernel(const ScenarioDev sc, con
                 // S5: duplicate-culling cache keyed on the full event identity; the 128-bit exchange is issued first
                 // and consumed after the (side-effect free) speciation and dispersal draws of this pass
                 if (DEDUP) {
-                    const u32 h = cache_hash(loc, k, j);
+                    const u32 h = cache_hash(X);
                     if (cache_probes(h, ep.probe_mask)) old = atomic_exch_128(&bf.cache[h & bf.cache_mask], make_uint4(loc, k, j, id));
                 }
                 // S2: speciation test on the event's SPEC lane (local community of the implicit model: nu = 0, L1830)
@@ -316,12 +318,20 @@ __global__ void __launch_bounds__(256) simulate_kernel(const ScenarioDev sc, con
                 const u64 x = draw_disp(X, att);
                 const u32 xx = wrap_add(cell & 0xFFFFu, gauss_disp(gl, (u32)(x >> 32)), sc.width);
                 const u32 yy = wrap_add(cell >> 16, gauss_disp(gl, (u32)x), sc.height);
-                const u32 c2 = yy * sc.width + xx;
-                const u32 d = cell_deme(sc, c2);
+                u32 d, pfx = 0;
+                if (COMPACT) {   // deme and prefix of the target from one 8-byte read of the compact habitat table
+                    const uint2 hb = __ldg(&sc.hab64[yy * sc.nbx + (xx >> 5)]);
+                    const u32 bit = 1u << (xx & 31u);
+                    d = (hb.x & bit) ? sc.compact_deme : 0u;
+                    pfx = hb.y + sc.compact_deme * (u32)__popc(hb.x & (bit - 1u));
+                } else {
+                    d = cell_deme(sc, yy * sc.width + xx);
+                }
                 accept = d > 0u;
                 if (accept) {
                     cell2 = (yy << 16) | xx;
-                    loc2 = cell_prefix(sc, c2) + ((d == 1u) ? 0u : mulhi64_u32(draw_index(X), d));
+                    if (!COMPACT) pfx = cell_prefix(sc, yy * sc.width + xx);
+                    loc2 = pfx + ((d == 1u) ? 0u : mulhi64_u32(draw_index(X), d));
                 }
             }
             if (att == 0) {

@@ -19,6 +19,13 @@ struct ScenarioDev {
     const uint8_t *hab8;       // [ncells] min(deme, 255)
     const u32 *deme32;         // [ncells] full deme (read only where hab8 == 255)
     const u32 *prefix;         // [ncells+1] exclusive prefix sum of deme
+    // compact habitat table (EXPLICIT_GAUSSIAN whose habitat cells all hold `compact_deme` individuals; NULL otherwise): per
+    // 32-cell block of a row {habitat bit mask, prefix sum at the block's first cell}. deme and prefix of a cell come out of
+    // ONE 8-byte read: deme = bit ? compact_deme : 0, prefix = base + compact_deme * popc(mask below the bit). 128x smaller
+    // than hab8 + prefix (C5: 4 MB instead of 84 MB), so a lineage's neighbourhood stays in L1 and the table in L2.
+    const uint2 *hab64;        // [height * nbx]
+    u32 nbx;                   // 32-cell blocks per row = ceil(width / 32)
+    u32 compact_deme;
     const uint2 *scale;        // [ncells] (Cm, sh) when per_cell_turnover
     const uint2 *alias;        // [ncells*ncells] (thresh, alias) for EXPLICIT_MATRIX
     const u64 *pois;           // [256] Poisson cdf thresholds of mu_max (sampler 1)
@@ -43,6 +50,7 @@ struct SimCounters {
     u64 n_events;              // events executed (raw)
     u64 n_culled;
     u64 resamples;
+    u64 tail_rounds_exact;     // tail kernel, exponential sampler: search rounds done in exact arithmetic (the fast round's fall-back count)
 };
 
 // Per-lineage SoA outputs + queues + dedup cache (all inside the simulate workspace).

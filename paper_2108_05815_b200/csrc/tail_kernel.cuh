@@ -5,38 +5,37 @@
 // throughput. Every draw is a pure function of its key (seed, loc, k, j, lane) -- PAPER.md 5.2.1, L693-707 --
 // so the 32 lanes of a warp may evaluate candidate draws of ONE lineage speculatively and in parallel; the
 // result is identical by construction (tests/test_gpu_invariance.py runs both kernels on the same inputs):
-//   - candidates: lanes 0..15 hold the points j = 1..16 of interval k (a segmented prefix sum gives the partial
-//     sums T_j), lanes 16..31 the FIRST point of intervals k+1..k+16 (the event if interval k is exhausted: a
-//     fresh interval's first point is its next event, L719-729);
-//   - once the winning candidate is known, ONE hash evaluation across the lanes yields all the event's draws: lane 0
+//   - candidates: the points j = 1.. of interval k (a prefix sum over the lanes gives the partial sums T_j) and the FIRST
+//     point of the following intervals (the event if interval k is exhausted: a fresh interval's first point is its next
+//     event, L719-729);
+//   - general path, once the winning candidate is known: ONE hash evaluation across the lanes yields all the event's draws: lane 0
 //     the speciation draw, lane 1 the index draw, lane 2 the migration draw, lanes 3..31 the dispersal attempts
 //     r = 0..28 (R16), each with its habitat / prefix / turnover-scale gathers; a ballot picks the first accepted;
 //   - the duplicate-culling exchange of an event is issued when the event is selected and consumed one event
 //     later (never after another cache insertion: an unconfirmed lineage must not publish entries).
+//
+// Exponential sampler, fast path ("speculative round"): the search for the next event and the evaluation of the events it
+// may find run SIDE BY SIDE, not one after the other. The draws of a candidate event are a pure function of (seed, loc, k, j)
+// and do not depend on its time, so each round the warp evaluates, with two interleaved hash evaluations per lane,
+//   8 candidates (lane >> 2): the points j = 1..5 of interval k and the first point of the intervals k+1, k+2, k+3
+//                             (99.6 % of the events at mu = 2, measured by simulation; the rest takes the general path)
+//   x 4 lanes (lane & 3):     slot A = dispersal attempt r = lane & 3 with its rounded-normal lookups and table gathers,
+//                             slot B = the time draw / speciation draw / index draw / migration draw of the candidate.
+// While the gathers are in flight the warp computes the logarithms and the partial sums; two ballots pick the event, a third
+// the first accepted attempt among the winner's four lanes. The critical path of an event is prime -> hash -> max(gather,
+// logarithm + scan) -> select instead of prime -> hash -> logarithm -> scan -> select -> hash -> gather -> select.
+// A candidate outside the set, or four rejected attempts, falls back to the general code below (identical results).
 #pragma once
 #include "sim_kernel.cuh"
 
 namespace necsim {
 
+#define NS_SPEC_NJ 5u              // speculative round: candidates 0..4 = points 1..5 of interval k
+#define NS_SPEC_ND 3u              //                    candidates 5..7 = first point of intervals k+1..k+3
+
 #define NS_REC_CHUNK 64u           // event-stream ring slots a warp reserves at a time
 #define NS_TAIL_ATTEMPTS 29u      // dispersal attempts evaluated per pass (lanes 3..31)
 
-
-// one level of the inclusive prefix sum over 16-lane segments: T += T of the lane `o` below, where that lane is in the
-// same segment (the shuffle's own predicate says so): 2 SHFL + 2 predicated adds
-__device__ __forceinline__ void seg16_scan_step(u32 &lo, u32 &hi, u32 o) {
-    asm volatile(
-        "{\n\t"
-        ".reg .pred p;\n\t"
-        ".reg .b32 tl, th;\n\t"
-        "shfl.sync.up.b32 tl|p, %0, %2, 0x1000, 0xffffffff;\n\t"
-        "shfl.sync.up.b32 th, %1, %2, 0x1000, 0xffffffff;\n\t"
-        "@p add.cc.u32 %0, %0, tl;\n\t"
-        "@p addc.u32 %1, %1, th;\n\t"
-        "}"
-        : "+r"(lo), "+r"(hi)
-        : "r"(o));
-}
 
 // per-cell rate data: exponential sampler -> (Cm, sh) of 1/(lambda dt); Poisson sampler -> (thinning threshold, unused)
 template <int SAMP>
@@ -117,8 +116,140 @@ __device__ __forceinline__ bool tail_search_poisson(const SeedKey &key, const Sm
     return true;
 }
 
-template <int KIND, bool DEDUP, bool PERCELL, int SAMP, bool REC>
-__global__ void __launch_bounds__(256) tail_kernel(const ScenarioDev sc, const SimBuffers bf, const EpochArgs ep) {
+// dispersal target of one attempt of EXPLICIT_GAUSSIAN from (x0, y0) with the draw u: packed cell, deme (0 = not habitat: rejected),
+// prefix of the cell, rate data of the cell. The gathers are issued back to back before anything consumes them.
+// FAST: no exact rescan of crowded guide buckets (far tails, probability ~ 2^-10): `bad` says that the target is unknown.
+template <bool PERCELL, int SAMP, bool COMPACT, bool FAST>
+__device__ __forceinline__ void gauss_target(const ScenarioDev &sc, const GaussLut &gl, u32 x0, u32 y0, u64 u, u32 &c2, u32 &d, u32 &pf, uint2 &cs, bool &bad) {
+    bool e1, e2;
+    int dx = gauss_disp_fast(gl, (u32)(u >> 32), e1), dy = gauss_disp_fast(gl, (u32)u, e2);
+    bad = !(e1 && e2);
+    if (!FAST && bad) { dx = gauss_disp(gl, (u32)(u >> 32)); dy = gauss_disp(gl, (u32)u); }   // rare: crowded tail buckets
+    const u32 xx = wrap_add(x0, dx, sc.width);
+    const u32 yy = wrap_add(y0, dy, sc.height);
+    c2 = (yy << 16) | xx;
+    if (COMPACT) {
+        const uint2 hb = ldg_v2_ordered(&sc.hab64[yy * sc.nbx + (xx >> 5)]);
+        if (PERCELL) {
+            const u32 ci = yy * sc.width + xx;
+            if (SAMP == 0) cs = ldg_v2_ordered(&sc.scale[ci]);
+            else cs.x = ldg_u32_ordered(&sc.thin[ci]), cs.y = 0u;
+        }
+        const u32 bit = 1u << (xx & 31u);
+        d = (hb.x & bit) ? sc.compact_deme : 0u;
+        pf = hb.y + sc.compact_deme * (u32)__popc(hb.x & (bit - 1u));
+    } else {
+        const u32 ci = yy * sc.width + xx;
+        pf = ldg_u32_ordered(&sc.prefix[ci]);           // speculative: same round trip as the habitat test
+        if (PERCELL) {
+            if (SAMP == 0) cs = ldg_v2_ordered(&sc.scale[ci]);
+            else cs.x = ldg_u32_ordered(&sc.thin[ci]), cs.y = 0u;
+        }
+        d = ldg_u8_ordered(&sc.hab8[ci]);
+        if (d == 255u) d = __ldg(&sc.deme32[ci]);
+    }
+}
+
+// ---- approximate event times for the fast round (exponential sampler) ----------------------------------------------------
+// The decisions of the event-time search ("T >= 2^48" and "T > f_last") are comparisons of partial sums of
+// -ln(U_i)/mu. The fast round evaluates them in binary32 from the top 32 bits of each draw: A = (32 - lg2(hi)) * ln2 / mu.
+// |A_j - T_j| is bounded ("filter"): a comparison further than the margin from equality has the same outcome as
+// the fixed-point comparison of 2.4, anything closer (or a draw with hi < 2^20) is "ambiguous" and the round is redone with
+// the exact arithmetic. Exact offsets are needed for records only and are recomputed from the event identity (loc, k, j):
+// T(loc, k, j) is a pure function of it (exact_offset).
+#define NS_LN2F 0.69314718f
+#define NS_MARGIN 6.1035156e-05f                     // 2^-14, times (1 + 1/mu)
+__device__ __forceinline__ float lg2_approx(float x) { float y; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+// 1/mu = Cm * 2^-(24 + sh) as binary32 (T = (E * Cm) >> (32 + sh) with E in Q8.56, T in Q16.48)
+__device__ __forceinline__ float rate_to_float(u32 Cm, u32 sh) { return __uint2float_rz(Cm) * __uint_as_float((103u - sh) << 23); }
+__device__ __forceinline__ float approx_exp_time(u64 draw, float ln2_over_mu) {
+    return (32.0f - lg2_approx(__uint2float_rz((u32)(draw >> 32)))) * ln2_over_mu;
+}
+
+// (Cm, sh) of the cell that holds indexed location loc
+template <bool PERCELL>
+__device__ __forceinline__ uint2 rate_of_loc(const ScenarioDev &sc, u32 loc) {
+    if (!PERCELL) return make_uint2(sc.Cm_u, sc.sh_u);
+    return __ldg(&sc.scale[cell_of_loc(sc, loc)]);
+}
+// exact offset T of the event (loc, k, j): the sum of the first j scaled draws of the stream primed on (loc, k)
+template <bool PERCELL>
+__device__ __forceinline__ u64 exact_offset(const ScenarioDev &sc, const SeedKey &key, const SmemTables &smt, u32 loc, u32 k, u32 j) {
+    const uint2 cs = rate_of_loc<PERCELL>(sc, loc);
+    u64 X = prime(key, loc, k), T = 0;
+    for (u32 i = 0; i < j; ++i) { X += NS_GAMMA; T += scale_exp(neglog(draw_time(X), smt), cs.x, cs.y); }
+    return T;
+}
+
+__device__ __forceinline__ uint2 lds_v2_ordered(u32 addr) { uint2 v; asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(addr)); return v; }
+// (x * d) >> 64 for a 32-bit d (see mulhi64_u32), with the two halves of x given
+__device__ __forceinline__ u32 mulhi64_u32_parts(u32 xlo, u32 xhi, u32 d) {
+    const u64 hi = (u64)xhi * (u64)d + (u64)__umulhi(xlo, d);
+    return (u32)(hi >> 32);
+}
+
+// Fast round, slot A of one lane (DESIGN.md 2.5 step 2): the dispersal target this lane's draw `ua` leads to, as the complete new
+// location: loc2 = prefix[cell'] + index, cell' (packed for EXPLICIT_GAUSSIAN), rate of cell'. acc = the target is habitat (this
+// attempt is accepted); bad = the target could not be determined here (crowded guide bucket): the round falls back.
+// xi = the index draw of the lane's candidate. Loads are issued before anything consumes them.
+template <int KIND, bool PERCELL, bool COMPACT>
+__device__ __forceinline__ void fast_slot_a(const ScenarioDev &sc, const GaussLut &gl, u32 sp_q, u32 lane, u32 bm, u32 cell, u64 ua, u32 xi_lo, u32 xi_hi,
+                                            u32 &loc2, u32 &c2, uint2 &cs, bool &acc, bool &bad) {
+    bad = false;
+    if (KIND == 0) {
+        loc2 = mulhi64_u32(ua, (u32)sc.n_locations); c2 = 0u; acc = sp_q == 0u;
+    } else if (KIND == 1) {
+        const bool to_meta = (cell != 0) || ((bm >> ((lane & 28u) + 3u)) & 1u);
+        loc2 = to_meta ? sc.J_local + mulhi64_u32(ua, sc.J_meta) : mulhi64_u32(ua, sc.J_local);
+        c2 = to_meta ? 1u : 0u; acc = sp_q == 0u;
+    } else if (KIND == 2) {
+        u32 d = 0, pf = 0;
+        c2 = 0;
+        if (sp_q == 0u) {
+            const u32 n = sc.ncells, col = __umulhi((u32)(ua >> 32), n);
+            const uint2 e = __ldg(&sc.alias[(size_t)cell * n + col]);
+            c2 = ((u32)ua < e.x) ? col : e.y;
+            pf = ldg_u32_ordered(&sc.prefix[c2]);
+            if (PERCELL) cs = ldg_v2_ordered(&sc.scale[c2]);
+            d = ldg_u8_ordered(&sc.hab8[c2]);
+            if (d == 255u) d = __ldg(&sc.deme32[c2]);
+        }
+        acc = d > 0u;
+        loc2 = pf + ((d == 1u) ? 0u : mulhi64_u32_parts(xi_lo, xi_hi, d));
+    } else {
+        // rounded-normal displacement of both axes: the two guide reads back to back, then pos = pos0 + (u >= threshold)
+        const u32 ux = (u32)(ua >> 32), uy = (u32)ua;
+        const uint2 ex = lds_v2_ordered(gl.g2 + 8u * (ux >> (32 - NS_G2_BITS)));
+        const uint2 ey = lds_v2_ordered(gl.g2 + 8u * (uy >> (32 - NS_G2_BITS)));
+        bad = ((ex.x | ey.x) >> 16) != 0u;
+        // torus (R17): t = coordinate + displacement + size lies in (0, 3 * size); two unsigned minima with t - size bring it into [0, size)
+        u32 xx = (ex.x & 0xFFFFu) + ((ex.y <= ux) ? 1u : 0u) + ((cell & 0xFFFFu) + sc.width - (u32)gl.R);
+        u32 yy = (ey.x & 0xFFFFu) + ((ey.y <= uy) ? 1u : 0u) + ((cell >> 16) + sc.height - (u32)gl.R);
+        xx = min(xx, xx - sc.width); xx = min(xx, xx - sc.width);
+        yy = min(yy, yy - sc.height); yy = min(yy, yy - sc.height);
+        c2 = (yy << 16) | xx;
+        if (COMPACT) {
+            const uint2 hb = ldg_v2_ordered(&sc.hab64[yy * sc.nbx + (xx >> 5)]);
+            if (PERCELL) cs = ldg_v2_ordered(&sc.scale[yy * sc.width + xx]);
+            const u32 D = sc.compact_deme;
+            const u32 idx = (D == 1u) ? 0u : mulhi64_u32_parts(xi_lo, xi_hi, D);     // in flight with the gather
+            const u32 bit = 1u << (xx & 31u);
+            acc = (hb.x & bit) != 0u;
+            loc2 = hb.y + D * (u32)__popc(hb.x & (bit - 1u)) + idx;
+        } else {
+            const u32 ci = yy * sc.width + xx;
+            const u32 pf = ldg_u32_ordered(&sc.prefix[ci]);
+            if (PERCELL) cs = ldg_v2_ordered(&sc.scale[ci]);
+            u32 d = ldg_u8_ordered(&sc.hab8[ci]);
+            if (d == 255u) d = __ldg(&sc.deme32[ci]);
+            acc = d > 0u;
+            loc2 = pf + ((d == 1u) ? 0u : mulhi64_u32_parts(xi_lo, xi_hi, d));
+        }
+    }
+}
+
+template <int KIND, bool DEDUP, bool PERCELL, int SAMP, bool REC, bool COMPACT>
+__global__ void __launch_bounds__(256, 2) tail_kernel(const ScenarioDev sc, const SimBuffers bf, const EpochArgs ep) {
     __shared__ unsigned short sQ[SAMP == 0 ? 512 : 256];      // SAMP 1: the Poisson guide
     __shared__ u64 sA[SAMP == 0 ? 512 : 256];                 // SAMP 1: the Poisson cdf thresholds
     __shared__ u32 sG[KIND == 3 ? 1024 : 1];
@@ -129,17 +260,26 @@ __global__ void __launch_bounds__(256) tail_kernel(const ScenarioDev sc, const S
     __syncthreads();
     GaussLut gl; gl.tg = smem_addr(sG); gl.g2 = smem_addr(sG2); gl.R = sc.R;
     SmemTables smt; smt.q = smem_addr(sQ); smt.a = smem_addr(sA); smt.tg = gl.tg; smt.g2 = gl.g2; smt.pc = smt.a; smt.pg = smt.q;
+    constexpr bool FAST = (SAMP == 0) && !REC;                // the fast round: exponential sampler, no event stream
 
     u32 lane;
     asm volatile("mov.u32 %0, %%laneid;" : "=r"(lane));                // opaque: kept in a register, not re-read per use
-    const u32 half = lane >> 4, sub = lane & 15u;
-    const u32 jj = half ? 1u : sub + 1u;                               // ordinal of this lane's candidate point
-    const u64 cand_add = (u64)jj * NS_GAMMA;                           // stream position of the candidate: s + jj * GAMMA
-    // event draws, one per lane: draw = F((X ^ lane_xor) + lane_add)
+    // general path: event draws, one per lane: draw = F((X ^ lane_xor) + lane_add)
     const u64 lane_xor = lane == 0 ? NS_L_SPEC : lane == 1 ? NS_L_INDEX : lane == 2 ? NS_L_MIGR : NS_L_DISP;
     const u32 att_lane = lane >= 3u ? lane - 3u : 0u;                  // dispersal attempt of this lane within a pass
     const u64 att_add = (u64)att_lane * NS_GAMMA;
-    unsigned long long c_events = 0, c_culled = 0, c_resamples = 0;   // warp-uniform
+    // speculative round (SAMP 0): candidate and slot of this lane
+    const u32 sp_c = lane >> 2, sp_q = lane & 3u;
+    const u32 sp_dk = sp_c < NS_SPEC_NJ ? 0u : sp_c - NS_SPEC_NJ + 1u;
+    const u64 sp_cand_add = (u64)(sp_c < NS_SPEC_NJ ? sp_c + 1u : 1u) * NS_GAMMA;
+    const u64 sp_a_add = (KIND == 3 ? (u64)sp_q : 0ull) * NS_GAMMA;                       // slot A: attempt sp_q
+    const u64 sp_b_xor = sp_q == 0 ? 0ull : sp_q == 1 ? NS_L_SPEC : sp_q == 2 ? NS_L_INDEX : NS_L_MIGR;   // slot B
+    const bool sp_in_k = lane < 4u * NS_SPEC_NJ;
+    const bool sp_add4 = sp_in_k && lane >= 4u, sp_add8 = sp_in_k && lane >= 8u, sp_add16 = sp_in_k && lane >= 16u;
+    const u32 kmask = (1u << (4u * NS_SPEC_NJ)) - 1u;
+    const u32 qb = lane & ~3u;
+    unsigned long long c_events = 0, c_culled = 0, c_resamples = 0, c_exact = 0;   // warp-uniform
+    u32 w_resamples = 0;                                                        // fast rounds: flushed into c_resamples per lineage
     // event-stream ring (REC): the warp reserves ep.rec_chunk (<= NS_REC_CHUNK) slots at a time, so that it waits for an atomic's return once per
     // chunk and not once per event; slots left over at the end are filled with sentinels (k = k_stop, which no event of the epoch has) the host-side pass drops
     u32 rec_next = 0, rec_left = 0;
@@ -158,10 +298,18 @@ __global__ void __launch_bounds__(256) tail_kernel(const ScenarioDev sc, const S
         const uint4 qe = bf.q_in[qi];
         const u32 id = qe.x;
         u32 loc = qe.y, cell = qe.z, steps = qe.w, k = ep.k_start, Cm = sc.Cm_u, sh = sc.sh_u;
-        i64 f_last = -1;
         if (PERCELL) { uint2 cs = load_rate<SAMP>(sc, KIND == 3 ? xy_index(sc, cell) : cell); Cm = cs.x; sh = cs.y; }
+        // lower bound of the search inside interval k: exact (f_last; -1 = fresh, none) for the general path, binary32 (fa_last)
+        // for the fast round. After a fast round only fa_last is current (f_exact = false); the exact value is then the offset
+        // of the last executed event (e_loc, k, e_j), recomputed when the general path needs it.
+        i64 f_last = -1;
+        bool f_exact = true;
+        float fa_last = -1.0f, fm_last = 0.0f, ln2_over_mu = 0.0f, margin = 0.0f;   // fm_last: error margin of fa_last
+        u32 e_loc = 0, e_j = 0;
+        if (FAST) { const float finv = rate_to_float(Cm, sh); ln2_over_mu = NS_LN2F * finv; margin = NS_MARGIN * (1.0f + finv); }
+        const u32 cap_at = ep.max_steps ? ep.max_steps : 0xFFFFFFFFu;
         // pending duplicate check: the exchange of the last probing event (lane 0 holds its result)
-        bool pend = false;
+        bool pend = false, p_T_known = true;
         u64 pold_lo = ~0ull, pold_hi = ~0ull;
         u32 p_loc = 0, p_k = 0, p_j = 0, p_l2 = 0;
         u64 p_T = 0;
@@ -172,6 +320,7 @@ __global__ void __launch_bounds__(256) tail_kernel(const ScenarioDev sc, const S
             const u32 ox = __shfl_sync(NS_FULL, (u32)pold_lo, 0), oy = __shfl_sync(NS_FULL, (u32)(pold_lo >> 32), 0);
             const u32 oz = __shfl_sync(NS_FULL, (u32)pold_hi, 0), ow = __shfl_sync(NS_FULL, (u32)(pold_hi >> 32), 0);
             if (ox == p_loc && oy == p_k && oz == p_j && ow != id) {   // another lineage executed it first (L687, L697)
+                if (FAST && !p_T_known) p_T = exact_offset<PERCELL>(sc, ep.key, smt, p_loc, p_k, p_j);
                 if (lane == 0) {
                     bf.parent[id] = ow; bf.state[id] = 2;
                     bf.term_loc[id] = p_loc; bf.term_k[id] = p_k; bf.term_j[id] = p_j; bf.term_f[id] = p_T; bf.steps[id] = steps;
@@ -179,7 +328,7 @@ __global__ void __launch_bounds__(256) tail_kernel(const ScenarioDev sc, const S
                 c_culled++;
                 return true;
             }
-            steps++; c_events++;                                       // the pending event was really executed
+            steps++;                                       // the pending event was really executed
             if (REC && lane == 0) record(p_loc, p_k, p_j, p_T, p_l2);
             return false;
         };
@@ -190,41 +339,170 @@ __global__ void __launch_bounds__(256) tail_kernel(const ScenarioDev sc, const S
                 if (lane == 0) bf.q_out[atomicAdd(&bf.ctr->q_out, 1u)] = make_uint4(id, loc, cell, steps);
                 break;
             }
+            if (FAST) {
+                // ---- fast rounds: the search in binary32 with a margin (see approx_exp_time), every candidate's outcome from its own four
+                // lanes. The loop commits clean events (99 %: candidate in the set, unambiguous comparisons, an attempt accepted, no
+                // speciation, no duplicate, no step cap) and leaves at the first round that is not, which the general code below redoes.
+                for (;;) {
+                    const u64 X = prime(ep.key, loc, k + sp_dk) + sp_cand_add;
+                    u64 ua, ub;
+                    hashF2((X ^ NS_L_DISP) + sp_a_add, X ^ sp_b_xor, ua, ub);
+                    const u32 ubh = (u32)(ub >> 32);
+                    const u32 bm = __ballot_sync(NS_FULL, bern(ub, sp_q == 3u ? ep.thr_m : ep.thr_nu));   // bit 4c+1: speciation, 4c+3: migration
+                    const u32 xi_lo = __shfl_sync(NS_FULL, (u32)ub, (int)(qb + 2u)), xi_hi = __shfl_sync(NS_FULL, ubh, (int)(qb + 2u));
+                    u32 loc2o, c2o; uint2 cso = make_uint2(Cm, sh); bool acc, bad;
+                    fast_slot_a<KIND, PERCELL, COMPACT>(sc, gl, sp_q, lane, bm, cell, ua, xi_lo, xi_hi, loc2o, c2o, cso, acc, bad);
+                    // slot B of the lanes with sp_q == 0: approximate offsets of the candidates (partial sums over the points of interval k)
+                    float a = sp_q == 0u ? approx_exp_time(ub, ln2_over_mu) : 0.0f;
+                    { const float y = __shfl_up_sync(NS_FULL, a, 4); if (sp_add4) a += y; }
+                    { const float y = __shfl_up_sync(NS_FULL, a, 8); if (sp_add8) a += y; }
+                    { const float y = __shfl_up_sync(NS_FULL, a, 16); if (sp_add16) a += y; }
+                    const float mc = margin + fm_last;
+                    const bool ins = a < 1.0f - margin, outs = a > 1.0f + margin;
+                    const bool aft = a > fa_last + mc, bef = a < fa_last - mc;
+                    const bool kvalid = (ep.k_stop - k) > sp_dk;              // never look at or past the horizon (k < k_stop here)
+                    const bool amb = (ubh < (1u << 20)) || !(ins || outs) || (sp_in_k && !(aft || bef));
+                    const u32 evm = __ballot_sync(NS_FULL, sp_q == 0u && ins && (sp_in_k ? aft : kvalid));
+                    const u32 crm = __ballot_sync(NS_FULL, sp_q == 0u && outs);
+                    const u32 okm = __ballot_sync(NS_FULL, acc);
+                    // trouble: an ambiguous comparison anywhere, or an undetermined target
+                    // trouble: an ambiguous comparison anywhere, an undetermined target, or (lane 0, which holds the result of the pending
+                    // exchange) a match there: another lineage executed the pending event first and this one is a duplicate
+                    bool culled = false;
+                    if (DEDUP) culled = lane == 0 && pend && (u32)pold_lo == p_loc && (u32)(pold_lo >> 32) == p_k && (u32)pold_hi == p_j && (u32)(pold_hi >> 32) != id;
+                    const u32 trm = __ballot_sync(NS_FULL, (sp_q == 0u && amb) || bad || culled);
+                    // every candidate's outcome: the first accepted attempt of its four lanes (the sequential algorithm's choice, R16)
+                    const int qsrc = (int)(qb + ((u32)first_bit(((okm >> qb) & 15u) | 16u) & 3u));
+                    const u32 loc2q = __shfl_sync(NS_FULL, loc2o, qsrc), cq = __shfl_sync(NS_FULL, c2o, qsrc);
+                    u32 Cmq = Cm, shq = sh;
+                    if (PERCELL) { Cmq = __shfl_sync(NS_FULL, cso.x, qsrc); shq = __shfl_sync(NS_FULL, cso.y, qsrc); }
+                    // the winner: first point of interval k after fa_last, else (interval exhausted, L719, L727) the first non-empty later interval
+                    const u32 m0 = evm & kmask;
+                    const u32 m1 = (crm & kmask) ? (evm & ~kmask) : 0u;
+                    const u32 wm = m0 ? m0 : m1;
+                    const u32 wl = (u32)first_bit(wm | 0x80000000u);
+                    const u32 q4 = 15u << wl;
+                    const u32 spec_w = (KIND == 1 && cell == 0) ? 0u : ((bm >> wl) & 2u);
+                    const u32 steps_e = steps + (pend ? 2u : 1u);       // step count after this event
+                    // clean: a winner, no trouble at the time lanes or in the winner's lanes, an attempt accepted, no speciation, no step cap
+                    const bool clean = wm != 0u && ((trm & (0x11111111u | q4)) | spec_w) == 0u && (okm & q4) != 0u && steps_e < cap_at;
+                    if (!__all_sync(NS_FULL, clean)) break;
+                    // commit: event (loc, k2, j2) executed, the lineage moves to the winner's target
+                    const u32 wc = wl >> 2;
+                    const u32 k2 = k + (wc < NS_SPEC_NJ ? 0u : wc - NS_SPEC_NJ + 1u);
+                    const u32 j2 = wc < NS_SPEC_NJ ? wc + 1u : 1u;
+                    const u32 loc2 = __shfl_sync(NS_FULL, loc2q, (int)wl), cell2 = __shfl_sync(NS_FULL, cq, (int)wl);
+                    const float a_w = __shfl_sync(NS_FULL, a, (int)wl);
+                    if (KIND == 3) w_resamples += (u32)first_bit((okm >> wl) & 15u);
+                    if (DEDUP) {
+                        if (pend) { steps++; pend = false; }                      // the pending event was really executed
+                        const u64 Xw = __shfl_sync(NS_FULL, X, (int)wl);
+                        const u32 h = cache_hash(Xw);
+                        const bool probes = cache_probes(h, ep.probe_mask);
+                        atomic_exch_128_if(probes && lane == 0, &bf.cache[h & bf.cache_mask], make_uint4(loc, k2, j2, id), pold_lo, pold_hi);
+                        if (probes) { p_loc = loc; p_k = k2; p_j = j2; p_T_known = false; pend = true; }
+                        else steps++;
+                    } else steps++;
+                    e_loc = loc; e_j = j2; f_exact = false; fa_last = a_w; fm_last = margin;
+                    if (PERCELL) {
+                        Cm = __shfl_sync(NS_FULL, Cmq, (int)wl); sh = __shfl_sync(NS_FULL, shq, (int)wl);
+                        const float finv = rate_to_float(Cm, sh);
+                        ln2_over_mu = NS_LN2F * finv; margin = NS_MARGIN * (1.0f + finv);
+                    }
+                    k = k2; loc = loc2; cell = cell2;
+                }
+                // the round that was not clean is done below in exact arithmetic, from the exact lower bound
+                if (!f_exact) { f_last = (i64)exact_offset<PERCELL>(sc, ep.key, smt, e_loc, k, e_j); f_exact = true; }
+                c_exact++;
+            }
             u32 j;
             u64 Te, Xe;
+            // outcome of the event when the speculative round evaluated it already
+            bool have = false, h_spec = false;
+            u32 h_loc2 = 0, h_cell2 = 0, h_Cm2 = Cm, h_sh2 = sh;
             if (SAMP == 1) {
                 // S1 (Poisson sampler, Cm = thinning threshold of the cell)
                 if (!tail_search_poisson<PERCELL>(ep.key, smt, lane, loc, k, f_last, ep.k_stop, Cm, j, Te, Xe)) continue;
             } else {
-                // ---- S1: candidate points of the event-time search ---------------------------------------------------
-                const u64 kk64 = (u64)k + (half ? (u64)(1u + sub) : 0ull);
-                const bool kvalid = kk64 < (u64)ep.k_stop;                // never look at or past the horizon
-                u64 X = prime(ep.key, loc, (u32)kk64) + cand_add;
-                const u64 T1 = scale_exp(neglog(draw_time(X), smt), Cm, sh);
-                // partial sums over each 16-lane half (half 1 keeps its single draws: first points of fresh intervals)
-                u32 t_lo = (u32)T1, t_hi = (u32)(T1 >> 32);
-                seg16_scan_step(t_lo, t_hi, 1); seg16_scan_step(t_lo, t_hi, 2);
-                seg16_scan_step(t_lo, t_hi, 4); seg16_scan_step(t_lo, t_hi, 8);
-                const u64 T = half ? T1 : (((u64)t_hi << 32) | t_lo);
-                const bool inside = T < NS_TWO48;
-                const u32 evm = __ballot_sync(NS_FULL, inside && (half ? kvalid : ((i64)T > f_last)));
-                const u32 crm = __ballot_sync(NS_FULL, !inside);
-                if (evm & 0xFFFFu) {                       // next event is in interval k
-                    const int src = first_bit(evm & 0xFFFFu);
-                    j = (u32)src + 1u;
-                    Te = __shfl_sync(NS_FULL, T, src); Xe = __shfl_sync(NS_FULL, X, src);
-                } else if (crm & 0xFFFFu) {                // interval k exhausted (L719, L727): first non-empty interval after it
-                    const u32 gap = ep.k_stop - 1u - k;    // k < k_stop here
-                    const u32 nvalid = gap < 16u ? gap : 16u;
-                    const u32 hm = evm >> 16;
-                    if (!hm) { k = k + 1u + nvalid; f_last = -1; continue; }   // all speculated intervals empty / beyond the horizon
-                    const int src = 16 + first_bit(hm);
-                    k = k + 1u + (u32)(src - 16); j = 1u;
-                    Te = __shfl_sync(NS_FULL, T, src); Xe = __shfl_sync(NS_FULL, X, src);
+                // ---- S1 + S2 + S3 side by side: 8 candidate events x (4 attempts | time, speciation, index, migration) -----------
+                const bool kvalid = (ep.k_stop - k) > sp_dk;              // never look at or past the horizon (k < k_stop here)
+                const u64 X = prime(ep.key, loc, k + sp_dk) + sp_cand_add;
+                u64 ua, ub;
+                hashF2((X ^ NS_L_DISP) + sp_a_add, X ^ sp_b_xor, ua, ub);
+                const u32 bm = __ballot_sync(NS_FULL, bern(ub, sp_q == 3u ? ep.thr_m : ep.thr_nu));   // bit 4c+1: speciation, 4c+3: migration
+                // slot A: dispersal target (gathers in flight during the arithmetic below)
+                u32 c2 = 0, d = 0, pf = 0;
+                uint2 cs = make_uint2(Cm, sh);
+                bool bad = false;
+                if (KIND == 0) {
+                    if (sp_q == 0u) { pf = mulhi64_u32(ua, (u32)sc.n_locations); d = 1u; }
+                } else if (KIND == 1) {
+                    if (sp_q == 0u) {
+                        const bool to_meta = (cell != 0) || ((bm >> (lane + 3u)) & 1u);
+                        if (to_meta) { pf = sc.J_local + mulhi64_u32(ua, sc.J_meta); c2 = 1u; }
+                        else pf = mulhi64_u32(ua, sc.J_local);
+                        d = 1u;
+                    }
+                } else if (KIND == 2) {
+                    if (sp_q == 0u) {
+                        const u32 n = sc.ncells, col = __umulhi((u32)(ua >> 32), n);
+                        const uint2 e = __ldg(&sc.alias[(size_t)cell * n + col]);
+                        c2 = ((u32)ua < e.x) ? col : e.y;
+                        pf = ldg_u32_ordered(&sc.prefix[c2]);
+                        if (PERCELL) cs = ldg_v2_ordered(&sc.scale[c2]);
+                        d = ldg_u8_ordered(&sc.hab8[c2]);
+                        if (d == 255u) d = __ldg(&sc.deme32[c2]);
+                    }
                 } else {
-                    // more than 16 points of interval k at or before f_last (large mu): continue the scan one draw at a time
-                    u64 Tc = __shfl_sync(NS_FULL, T, 15), Xc = __shfl_sync(NS_FULL, X, 15);
-                    u32 jc = 16u;
+                    gauss_target<PERCELL, SAMP, COMPACT, true>(sc, gl, cell & 0xFFFFu, cell >> 16, ua, c2, d, pf, cs, bad);
+                }
+                // the outcome of EVERY candidate from its own four lanes, before the search says which one it is: first accepted
+                // attempt (= the sequential algorithm's choice, R16), its cell and prefix, the index draw of the candidate
+                const u32 okm = __ballot_sync(NS_FULL, d > 0u);
+                const u32 badm = KIND == 3 ? __ballot_sync(NS_FULL, bad) : 0u;
+                const int qsrc = (int)(qb + ((u32)first_bit(((okm >> qb) & 15u) | 16u) & 3u));
+                const u32 dq = __shfl_sync(NS_FULL, d, qsrc), pq = __shfl_sync(NS_FULL, pf, qsrc), cq = __shfl_sync(NS_FULL, c2, qsrc);
+                u32 Cmq = Cm, shq = sh;
+                if (PERCELL) { Cmq = __shfl_sync(NS_FULL, cs.x, qsrc); shq = __shfl_sync(NS_FULL, cs.y, qsrc); }
+                const u64 xiq = __shfl_sync(NS_FULL, ub, (int)(qb + 2u));
+                const u32 loc2q = pq + ((dq == 1u) ? 0u : mulhi64_u32(xiq, dq));
+
+                // slot B of the lanes with sp_q == 0: the time draw of the candidate (every lane runs the arithmetic)
+                const u64 T1 = scale_exp(neglog(ub, smt), Cm, sh);
+                // partial sums T_j over the points of interval k: lanes 0, 4, .., 16 (offsets of 1, 2, 4 candidates)
+                u64 T = sp_q == 0u ? T1 : 0ull;
+                { const u64 y = __shfl_up_sync(NS_FULL, T, 4); if (sp_add4) T += y; }
+                { const u64 y = __shfl_up_sync(NS_FULL, T, 8); if (sp_add8) T += y; }
+                { const u64 y = __shfl_up_sync(NS_FULL, T, 16); if (sp_add16) T += y; }
+                const bool inside = T < NS_TWO48;
+                const u32 evm = __ballot_sync(NS_FULL, sp_q == 0u && inside && (sp_in_k ? ((i64)T > f_last) : kvalid));
+                const u32 crm = __ballot_sync(NS_FULL, sp_q == 0u && !inside);
+                const u32 m0 = evm & kmask;                    // next event is in interval k
+                const u32 m1 = (crm & kmask) ? (evm & ~kmask) : 0u;   // interval k exhausted (L719, L727): first non-empty interval after it
+                const u32 wm = m0 ? m0 : m1;
+                if (wm) {
+                    const int wl = first_bit(wm);              // lane of the winning candidate's slot-A attempt 0 / time draw
+                    const u32 wc = (u32)wl >> 2;
+                    k += wc < NS_SPEC_NJ ? 0u : wc - NS_SPEC_NJ + 1u;
+                    j = wc < NS_SPEC_NJ ? wc + 1u : 1u;
+                    Te = __shfl_sync(NS_FULL, T, wl); Xe = __shfl_sync(NS_FULL, X, wl);
+                    h_spec = !(KIND == 1 && cell == 0) && ((bm >> ((u32)wl + 1u)) & 1u);
+                    const u32 acc = (okm >> (u32)wl) & 15u;
+                    if (h_spec) have = true;
+                    else if (acc && !((badm >> (u32)wl) & 15u)) {
+                        h_loc2 = __shfl_sync(NS_FULL, loc2q, wl); h_cell2 = __shfl_sync(NS_FULL, cq, wl);
+                        if (PERCELL) { h_Cm2 = __shfl_sync(NS_FULL, Cmq, wl); h_sh2 = __shfl_sync(NS_FULL, shq, wl); }
+                        if (KIND == 3) c_resamples += (u32)first_bit(acc);
+                        have = true;
+                    }
+                } else if (crm & kmask) {                      // all speculated intervals empty / beyond the horizon
+                    const u32 gap = ep.k_stop - 1u - k;
+                    k = k + 1u + (gap < NS_SPEC_ND ? gap : NS_SPEC_ND); f_last = -1; fa_last = -1.0f; fm_last = 0.0f;
+                    continue;
+                } else {
+                    // more than NS_SPEC_NJ points of interval k at or before f_last: continue the scan one draw at a time
+                    u64 Tc = __shfl_sync(NS_FULL, T, 4 * (NS_SPEC_NJ - 1u)), Xc = __shfl_sync(NS_FULL, X, 4 * (NS_SPEC_NJ - 1u));
+                    u32 jc = NS_SPEC_NJ;
                     bool found = false;
                     for (;;) {
                         jc += 1u; Xc += NS_GAMMA;
@@ -232,7 +510,7 @@ __global__ void __launch_bounds__(256) tail_kernel(const ScenarioDev sc, const S
                         if (Tc >= NS_TWO48) break;
                         if ((i64)Tc > f_last) { found = true; break; }
                     }
-                    if (!found) { k += 1u; f_last = -1; continue; }
+                    if (!found) { k += 1u; f_last = -1; fa_last = -1.0f; fm_last = 0.0f; continue; }
                     j = jc; Te = Tc; Xe = Xc;
                 }
             }
@@ -242,71 +520,61 @@ __global__ void __launch_bounds__(256) tail_kernel(const ScenarioDev sc, const S
             if (resolve_pending()) break;
             bool probes = false;
             if (DEDUP) {
-                const u32 h = cache_hash(loc, k, j);
+                const u32 h = cache_hash(Xe);
                 probes = cache_probes(h, ep.probe_mask);
                 atomic_exch_128_if(probes && lane == 0, &bf.cache[h & bf.cache_mask], make_uint4(loc, k, j, id), pold_lo, pold_hi);
-                if (probes) { p_loc = loc; p_k = k; p_j = j; p_T = Te; pend = true; }
+                if (probes) { p_loc = loc; p_k = k; p_j = j; p_T = Te; p_T_known = true; pend = true; }
             }
-            if (!probes) { steps++; c_events++; }
-            // S2 + S3: all draws of the event in one hash evaluation across the lanes
-            const u64 xb = Xe ^ lane_xor;
-            u64 u = hashF(xb + att_add);
-            const bool can_speciate = !(KIND == 1 && cell == 0);      // local community of the implicit model: nu = 0 (L1830)
-            const u32 bm = __ballot_sync(NS_FULL, bern(u, lane == 2 ? ep.thr_m : ep.thr_nu));
-            const bool speciates = can_speciate && (bm & 1u);
-            u32 loc2 = loc, cell2 = cell, Cm2 = Cm, sh2 = sh;
+            if (!probes) steps++;
+            bool speciates = h_spec;
+            u32 loc2 = h_loc2, cell2 = h_cell2, Cm2 = h_Cm2, sh2 = h_sh2;
             bool ok = true;
-            if (!speciates) {
-                if (KIND == 0) {
-                    loc2 = mulhi64_u32(__shfl_sync(NS_FULL, u, 3), (u32)sc.n_locations); cell2 = 0;
-                } else if (KIND == 1) {
-                    const u64 x = __shfl_sync(NS_FULL, u, 3);
-                    const bool to_meta = (cell != 0) || (bm & 4u);
-                    if (to_meta) { loc2 = sc.J_local + mulhi64_u32(x, sc.J_meta); cell2 = 1; }
-                    else { loc2 = mulhi64_u32(x, sc.J_local); cell2 = 0; }
-                } else if (KIND == 2) {
-                    const u64 x = __shfl_sync(NS_FULL, u, 3), xi = __shfl_sync(NS_FULL, u, 1);
-                    const u32 n = sc.ncells, col = __umulhi((u32)(x >> 32), n);
-                    const uint2 e = __ldg(&sc.alias[(size_t)cell * n + col]);
-                    cell2 = ((u32)x < e.x) ? col : e.y;
-                    const u32 d = cell_deme(sc, cell2);
-                    loc2 = cell_prefix(sc, cell2) + ((d == 1u) ? 0u : mulhi64_u32(xi, d));
-                    if (PERCELL) { const uint2 cs = load_rate<SAMP>(sc, cell2); Cm2 = cs.x; sh2 = cs.y; }
-                } else {
-                    const u64 xi = __shfl_sync(NS_FULL, u, 1);
-                    const u32 x0 = cell & 0xFFFFu, y0 = cell >> 16;
-                    ok = false;
-                    for (u32 r0 = 0; r0 < NS_MAX_RESAMPLE; r0 += NS_TAIL_ATTEMPTS) {
-                        u32 c2 = 0, d = 0, pf = 0;
-                        uint2 cs = make_uint2(Cm, sh);
-                        if (lane >= 3u) {   // attempt r0 + lane - 3 (R16: redraw the whole (dx, dy) pair)
-                            bool e1, e2;
-                            int dx = gauss_disp_fast(gl, (u32)(u >> 32), e1), dy = gauss_disp_fast(gl, (u32)u, e2);
-                            if (!(e1 && e2)) { dx = gauss_disp(gl, (u32)(u >> 32)); dy = gauss_disp(gl, (u32)u); }   // rare: crowded tail buckets
-                            const u32 xx = wrap_add(x0, dx, sc.width);
-                            const u32 yy = wrap_add(y0, dy, sc.height);
-                            const u32 ci = yy * sc.width + xx;
-                            c2 = (yy << 16) | xx;
-                            pf = ldg_u32_ordered(&sc.prefix[ci]);           // speculative: same round trip as the habitat test
-                            if (PERCELL) {
-                                if (SAMP == 0) cs = ldg_v2_ordered(&sc.scale[ci]);
-                                else cs.x = ldg_u32_ordered(&sc.thin[ci]), cs.y = 0u;
+            if (!have) {
+                // S2 + S3, general path: all draws of the event in one hash evaluation across the lanes
+                const u64 xb = Xe ^ lane_xor;
+                u64 u = hashF(xb + att_add);
+                const bool can_speciate = !(KIND == 1 && cell == 0);      // local community of the implicit model: nu = 0 (L1830)
+                const u32 bm = __ballot_sync(NS_FULL, bern(u, lane == 2 ? ep.thr_m : ep.thr_nu));
+                speciates = can_speciate && (bm & 1u);
+                loc2 = loc; cell2 = cell; Cm2 = Cm; sh2 = sh;
+                if (!speciates) {
+                    if (KIND == 0) {
+                        loc2 = mulhi64_u32(__shfl_sync(NS_FULL, u, 3), (u32)sc.n_locations); cell2 = 0;
+                    } else if (KIND == 1) {
+                        const u64 x = __shfl_sync(NS_FULL, u, 3);
+                        const bool to_meta = (cell != 0) || (bm & 4u);
+                        if (to_meta) { loc2 = sc.J_local + mulhi64_u32(x, sc.J_meta); cell2 = 1; }
+                        else { loc2 = mulhi64_u32(x, sc.J_local); cell2 = 0; }
+                    } else if (KIND == 2) {
+                        const u64 x = __shfl_sync(NS_FULL, u, 3), xi = __shfl_sync(NS_FULL, u, 1);
+                        const u32 n = sc.ncells, col = __umulhi((u32)(x >> 32), n);
+                        const uint2 e = __ldg(&sc.alias[(size_t)cell * n + col]);
+                        cell2 = ((u32)x < e.x) ? col : e.y;
+                        const u32 d = cell_deme(sc, cell2);
+                        loc2 = cell_prefix(sc, cell2) + ((d == 1u) ? 0u : mulhi64_u32(xi, d));
+                        if (PERCELL) { const uint2 cs = load_rate<SAMP>(sc, cell2); Cm2 = cs.x; sh2 = cs.y; }
+                    } else {
+                        const u64 xi = __shfl_sync(NS_FULL, u, 1);
+                        const u32 x0 = cell & 0xFFFFu, y0 = cell >> 16;
+                        ok = false;
+                        for (u32 r0 = 0; r0 < NS_MAX_RESAMPLE; r0 += NS_TAIL_ATTEMPTS) {
+                            u32 c2 = 0, d = 0, pf = 0;
+                            uint2 cs = make_uint2(Cm, sh);
+                            bool bad_;
+                            if (lane >= 3u) gauss_target<PERCELL, SAMP, COMPACT, false>(sc, gl, x0, y0, u, c2, d, pf, cs, bad_);   // attempt r0 + lane - 3 (R16: redraw the whole (dx, dy) pair)
+                            const u32 okm = __ballot_sync(NS_FULL, lane >= 3u && d > 0u);
+                            if (okm) {
+                                const int w = first_bit(okm);    // first accepted attempt = the sequential algorithm's choice
+                                c2 = __shfl_sync(NS_FULL, c2, w); d = __shfl_sync(NS_FULL, d, w); pf = __shfl_sync(NS_FULL, pf, w);
+                                if (PERCELL) { Cm2 = __shfl_sync(NS_FULL, cs.x, w); sh2 = __shfl_sync(NS_FULL, cs.y, w); }
+                                cell2 = c2;
+                                loc2 = pf + ((d == 1u) ? 0u : mulhi64_u32(xi, d));
+                                c_resamples += r0 + (u32)w - 3u;
+                                ok = true;
+                                break;
                             }
-                            d = ldg_u8_ordered(&sc.hab8[ci]);
-                            if (d == 255u) d = __ldg(&sc.deme32[ci]);
+                            u = hashF(xb + att_add + (u64)(r0 + NS_TAIL_ATTEMPTS) * NS_GAMMA);   // next 29 attempts
                         }
-                        const u32 okm = __ballot_sync(NS_FULL, lane >= 3u && d > 0u);
-                        if (okm) {
-                            const int w = first_bit(okm);    // first accepted attempt = the sequential algorithm's choice
-                            c2 = __shfl_sync(NS_FULL, c2, w); d = __shfl_sync(NS_FULL, d, w); pf = __shfl_sync(NS_FULL, pf, w);
-                            if (PERCELL) { Cm2 = __shfl_sync(NS_FULL, cs.x, w); sh2 = __shfl_sync(NS_FULL, cs.y, w); }
-                            cell2 = c2;
-                            loc2 = pf + ((d == 1u) ? 0u : mulhi64_u32(xi, d));
-                            c_resamples += r0 + (u32)w - 3u;
-                            ok = true;
-                            break;
-                        }
-                        u = hashF(xb + att_add + (u64)(r0 + NS_TAIL_ATTEMPTS) * NS_GAMMA);   // next 29 attempts
                     }
                 }
             }
@@ -335,7 +603,13 @@ __global__ void __launch_bounds__(256) tail_kernel(const ScenarioDev sc, const S
                 break;
             }
             f_last = (i64)Te; loc = loc2; cell = cell2; Cm = Cm2; sh = sh2;
+            if (FAST) {
+                f_exact = true; fa_last = (float)Te * 0x1p-48f; fm_last = 2.4e-07f;   // binary32 rounding of an offset < 1
+                if (PERCELL) { const float finv = rate_to_float(Cm, sh); ln2_over_mu = NS_LN2F * finv; margin = NS_MARGIN * (1.0f + finv); }
+            }
         }
+        c_events += steps - qe.w;                  // events this lineage executed in this launch
+        c_resamples += w_resamples; w_resamples = 0;
     }
     if (REC) {   // sentinels into the reserved slots that stayed empty
         const u32 nx = __shfl_sync(NS_FULL, rec_next, 0), lf = __shfl_sync(NS_FULL, rec_left, 0);
@@ -348,6 +622,7 @@ __global__ void __launch_bounds__(256) tail_kernel(const ScenarioDev sc, const S
         if (c_events) atomicAdd((unsigned long long *)&bf.ctr->n_events, c_events);
         if (c_culled) atomicAdd((unsigned long long *)&bf.ctr->n_culled, c_culled);
         if (c_resamples) atomicAdd((unsigned long long *)&bf.ctr->resamples, c_resamples);
+        if (c_exact) atomicAdd((unsigned long long *)&bf.ctr->tail_rounds_exact, c_exact);
     }
 }
 

@@ -56,11 +56,22 @@ def gather_tables(local, record_bytes=32):
     return cat, offsets
 
 
+def translate_labels(labels, dmap, offset):
+    """Labels of one partition -> ranks in the merged table: dmap[offset + label]. An unfinished lineage (stopped by
+    max_steps: label 0xFFFFFFFF, i.e. -1 once widened from the int32 storage) stays -1 instead of indexing a neighbour's record."""
+    labels = labels.to(torch.int64)
+    unf = (labels < 0) | (labels >= 0xFFFFFFFF)
+    if dmap.numel() == 0:
+        return torch.full_like(labels, -1)
+    out = dmap[offset + torch.where(unf, torch.zeros_like(labels), labels)]
+    return torch.where(unf, torch.full_like(out, -1), out)
+
+
 def simulate_partitioned(scenario, seed, nu, mask=None, rank=0, world=1, params=None):
     """Isolated partitions + merge: this rank simulates its share of the sample with no
     communication, then ONE all-gather of the species tables and a device-side merge (necsim_merge_species) give the table
     of the whole sample. Returns dict(events: CUDA uint8 [S * 32] merged table, labels: CUDA int64 [local lineages] indices
-    into it, richness, local: the rank's Result)."""
+    into it (-1 = unfinished, stopped by max_steps), richness, local: the rank's Result, ms_merge: device time of gather + merge)."""
     from . import necsim as ns
     m = shard_mask(mask, scenario.n_individuals, rank, world)
     if int(m.sum()) == 0:
@@ -69,9 +80,16 @@ def simulate_partitioned(scenario, seed, nu, mask=None, rank=0, world=1, params=
         res = scenario.simulate_raw(seed, nu, torch.from_numpy(m).cuda(), int(m.sum()), params)
         tab, lab = scenario.result_tensors(res)
         local_tab, labels = tab.clone(), lab.to(torch.int64)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
     cat, offsets = gather_tables(local_tab)
-    merged, dmap = ns.merge_species(cat)
-    return dict(events=merged, labels=dmap[offsets[rank if len(offsets) > 1 else 0] + labels], richness=merged.numel() // 32, local=res)
+    if cat.numel() == 0:      # no rank reached a speciation (every lineage unfinished): nothing to merge
+        merged, dmap = cat, torch.empty(0, dtype=torch.int64, device=cat.device)
+    else:
+        merged, dmap = ns.merge_species(cat)
+    out_labels = translate_labels(labels, dmap, offsets[rank if len(offsets) > 1 else 0])
+    e1.record(); e1.synchronize()
+    return dict(events=merged, labels=out_labels, richness=merged.numel() // 32, local=res, ms_merge=e0.elapsed_time(e1))
 
 
 def throughput(units_total, time_ms_max):

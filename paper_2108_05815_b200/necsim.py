@@ -44,7 +44,7 @@ class Result(C.Structure):
                 ("n_events_tail", C.c_uint64), ("ms_simulate", C.c_float), ("ms_simulate_tail", C.c_float),
                 ("ms_total", C.c_float), ("n_kernel_launches", C.c_uint32),
                 ("d_stream_loc", C.c_void_p), ("d_stream_k", C.c_void_p), ("d_stream_j", C.c_void_p), ("d_stream_loc2", C.c_void_p),
-                ("d_stream_f", C.c_void_p), ("n_stream_events", C.c_uint64)]
+                ("d_stream_f", C.c_void_p), ("n_stream_events", C.c_uint64), ("n_tail_rounds_exact", C.c_uint64)]
 
 
 EVENT_DTYPE = np.dtype({"names": ["loc", "k", "j", "abundance", "f", "time"],
@@ -84,7 +84,7 @@ def lib():
         L.necsim_debug_next_event.argtypes = [u64] + [vp] * 9 + [u64, vp]
         L.necsim_debug_disperse.argtypes = [vp, u64, vp, vp, vp, vp, u64, vp]
         L.necsim_debug_tables.argtypes = [vp] * 8
-        L.necsim_debug_int_peak.argtypes = [C.c_int, u32, vp, vp, vp]
+        L.necsim_debug_int_peak.argtypes = [C.c_int, u32, vp, vp, vp, vp]
         L.necsim_debug_next_event_poisson.argtypes = [vp, u64] + [vp] * 8 + [u64, vp]
         L.necsim_debug_poisson_table.argtypes = [vp] * 5
         L.necsim_merge_workspace_size.argtypes = [u64, vp]
@@ -226,7 +226,7 @@ class Scenario:
                    labels=_read(self._sim_ws, res.d_labels, n * 4, np.uint32),
                    stats={k: getattr(res, k) for k in ("n_lineages", "n_unfinished", "n_events_raw", "n_culled", "n_speciation_raw",
                                                        "n_epochs", "n_tail_epochs", "resample_attempts", "n_events_tail", "ms_simulate",
-                                                       "ms_simulate_tail", "ms_total", "n_kernel_launches", "n_stream_events")})
+                                                       "ms_simulate_tail", "ms_total", "n_kernel_launches", "n_stream_events", "n_tail_rounds_exact")})
         if params.record_events:
             m = int(res.n_stream_events)
             st = np.zeros(m, dtype=[("loc", "<u4"), ("k", "<u4"), ("j", "<u4"), ("f", "<u8"), ("loc2", "<u4")])
@@ -351,5 +351,6 @@ def int_peak(kind, iters=4096):
     """Integer-pipe micro-benchmark: returns (thread-level integer instructions per second, ms)."""
     torch = _torch()
     v, ms = C.c_double(), C.c_float()
-    _check(lib().necsim_debug_int_peak(int(kind), int(iters), _stream_ptr(torch), C.byref(v), C.byref(ms)))
+    sink = torch.zeros(1, dtype=torch.int32, device="cuda")
+    _check(lib().necsim_debug_int_peak(int(kind), int(iters), C.c_void_p(sink.data_ptr()), _stream_ptr(torch), C.byref(v), C.byref(ms)))
     return v.value, ms.value

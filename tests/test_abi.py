@@ -28,7 +28,7 @@ def test_struct_sizes_match_header():
     assert ctypes.sizeof(necsim.ScenarioDesc) == 96
     assert ctypes.sizeof(necsim.SimParams) == 64
     assert necsim.EVENT_DTYPE.itemsize == 32
-    assert ctypes.sizeof(necsim.Result) == 208
+    assert ctypes.sizeof(necsim.Result) == 216
 
 
 def test_error_paths_without_gpu():

@@ -57,3 +57,14 @@ def test_single_process_is_identity():
     from paper_2108_05815_b200 import dist as D
     assert D.aggregate([1.5], [2.0]) == ([1.5], [2.0])
     assert D.replica_seed(2**64 - 1, 1) == 0
+
+
+def test_translate_labels_keeps_unfinished_and_handles_empty_tables():
+    """a lineage stopped by max_steps (label 0xFFFFFFFF -> -1 in int64) must not index a neighbour's record."""
+    from paper_2108_05815_b200 import dist as D
+    dmap = torch.tensor([5, 6, 7, 8, 9], dtype=torch.int64)
+    lab = torch.tensor([0, -1, 1, 0xFFFFFFFF], dtype=torch.int64)
+    assert D.translate_labels(lab, dmap, 2).tolist() == [7, -1, 8, -1]
+    assert D.translate_labels(lab, dmap, 0).tolist() == [5, -1, 6, -1]          # rank 0: no negative wrap to the last record
+    assert D.translate_labels(torch.tensor([-1, -1]), torch.empty(0, dtype=torch.int64), 0).tolist() == [-1, -1]
+    assert D.translate_labels(torch.empty(0, dtype=torch.int64), dmap, 3).numel() == 0

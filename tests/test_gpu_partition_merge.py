@@ -38,3 +38,24 @@ def test_partition_merge_equals_whole(O, idx, world):
     out = D.simulate_partitioned(sc, cfg["seed"], cfg["nu"], cfg["mask"])
     assert out["richness"] == ref["richness"] and np.array_equal(out["labels"].cpu().numpy(), ref["labels"].astype(np.int64))
     sc.close()
+
+
+def test_partitioned_with_step_cap_marks_unfinished(O):
+    """with max_steps some lineages end unfinished (label 0xFFFFFFFF); the translated labels keep them at -1, the others
+    agree with the oracle's run under the same cap (dedup off on both sides: per-lineage results are then scheduling-independent)."""
+    import torch
+    from paper_2108_05815_b200 import inputs as I, necsim as ns, dist as D
+    cfg = I.small_configs()[0]
+    kw = I.scenario_kwargs(cfg)
+    ref = O.Scenario(**kw).simulate(cfg["seed"], cfg["nu"], cfg["mask"], dedup=False, max_steps=300)
+    assert 0 < ref["stats"]["n_unfinished"] < ref["stats"]["n_lineages"]
+    sc = ns.Scenario(**kw)
+    out = D.simulate_partitioned(sc, cfg["seed"], cfg["nu"], cfg["mask"], params=ns.make_params(dedup=False, max_steps=300))
+    lab = out["labels"].cpu().numpy()
+    want = ref["labels"].astype(np.int64); want[ref["labels"] == 0xFFFFFFFF] = -1
+    assert np.array_equal(lab, want) and out["richness"] == ref["richness"]
+    # every lineage unfinished: empty tables, no merge call, all labels -1
+    out = D.simulate_partitioned(sc, cfg["seed"], cfg["nu"], cfg["mask"], params=ns.make_params(dedup=False, max_steps=1))
+    if out["richness"] == 0:
+        assert (out["labels"].cpu().numpy() == -1).all()
+    sc.close()
