@@ -541,12 +541,13 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
     const int occ = occupancy_for(fn_main, rp.block_threads);
     const int occ_tail = occupancy_for(fn_tail, rp.block_threads);
     ep.probe_mask = rp.probe_mask;
+    ep.zero = 0;
     if (occ <= 0 || occ_tail <= 0) return fail(NECSIM_ERR_CUDA, "simulate kernel cannot be resident (occupancy 0)");
     const u32 full_grid = rp.grid_blocks ? rp.grid_blocks : (u32)(occ * scn->sm_count);
     const u32 tail_grid = rp.grid_blocks ? rp.grid_blocks : (u32)(occ_tail * scn->sm_count);
     const u32 warps_per_block = rp.block_threads / 32u;
     // one lineage per warp pays off from about four lineages per resident warp downwards (measured on C5 / C6: sweep in DESIGN.md 5)
-    const u32 tail_threshold = rp.tail_threshold ? rp.tail_threshold : 4u * tail_grid * warps_per_block;
+    const u32 tail_threshold = rp.tail_threshold ? rp.tail_threshold : 128u * (u32)scn->sm_count;
     const u32 full_cache_mask = rp.dedup ? ((1u << rp.dedup_log2_slots) - 1u) : 0u;
     u32 active = n_sampled, k_start = 0;
     uint4 *q_in = qa, *q_out = qb;

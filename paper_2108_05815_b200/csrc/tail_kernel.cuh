@@ -159,11 +159,12 @@ __device__ __forceinline__ void gauss_target(const ScenarioDev &sc, const GaussL
 // T(loc, k, j) is a pure function of it (exact_offset).
 #define NS_LN2F 0.69314718f
 #define NS_MARGIN 6.1035156e-05f                     // 2^-14, times (1 + 1/mu)
-__device__ __forceinline__ float lg2_approx(float x) { float y; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+// volatile: stays after the table gathers of slot A in issue order (the gathers have the longest latency and go first)
+__device__ __forceinline__ float lg2_approx(float x) { float y; asm volatile("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 // 1/mu = Cm * 2^-(24 + sh) as binary32 (T = (E * Cm) >> (32 + sh) with E in Q8.56, T in Q16.48)
 __device__ __forceinline__ float rate_to_float(u32 Cm, u32 sh) { return __uint2float_rz(Cm) * __uint_as_float((103u - sh) << 23); }
-__device__ __forceinline__ float approx_exp_time(u64 draw, float ln2_over_mu) {
-    return (32.0f - lg2_approx(__uint2float_rz((u32)(draw >> 32)))) * ln2_over_mu;
+__device__ __forceinline__ float approx_exp_time(u32 draw_hi, float ln2_over_mu) {
+    return (32.0f - lg2_approx(__uint2float_rz(draw_hi))) * ln2_over_mu;
 }
 
 // (Cm, sh) of the cell that holds indexed location loc
@@ -173,11 +174,9 @@ __device__ __forceinline__ uint2 rate_of_loc(const ScenarioDev &sc, u32 loc) {
     return __ldg(&sc.scale[cell_of_loc(sc, loc)]);
 }
 // exact offset T of the event (loc, k, j): the sum of the first j scaled draws of the stream primed on (loc, k)
-template <bool PERCELL>
-__device__ __forceinline__ u64 exact_offset(const ScenarioDev &sc, const SeedKey &key, const SmemTables &smt, u32 loc, u32 k, u32 j) {
-    const uint2 cs = rate_of_loc<PERCELL>(sc, loc);
+__device__ __forceinline__ u64 exact_offset(const SeedKey &key, const SmemTables &smt, u32 loc, u32 k, u32 j, u32 Cm, u32 sh) {
     u64 X = prime(key, loc, k), T = 0;
-    for (u32 i = 0; i < j; ++i) { X += NS_GAMMA; T += scale_exp(neglog(draw_time(X), smt), cs.x, cs.y); }
+    for (u32 i = 0; i < j; ++i) { X += NS_GAMMA; T += scale_exp(neglog(draw_time(X), smt), Cm, sh); }
     return T;
 }
 
@@ -305,7 +304,7 @@ __global__ void __launch_bounds__(256, 2) tail_kernel(const ScenarioDev sc, cons
         i64 f_last = -1;
         bool f_exact = true;
         float fa_last = -1.0f, fm_last = 0.0f, ln2_over_mu = 0.0f, margin = 0.0f;   // fm_last: error margin of fa_last
-        u32 e_loc = 0, e_j = 0;
+        u32 e_loc = 0xFFFFFFFFu, e_j = 0, e_Cm = Cm, e_sh = sh;   // last executed event (origin, ordinal, rate of the origin's cell)
         if (FAST) { const float finv = rate_to_float(Cm, sh); ln2_over_mu = NS_LN2F * finv; margin = NS_MARGIN * (1.0f + finv); }
         const u32 cap_at = ep.max_steps ? ep.max_steps : 0xFFFFFFFFu;
         // pending duplicate check: the exchange of the last probing event (lane 0 holds its result)
@@ -320,7 +319,7 @@ __global__ void __launch_bounds__(256, 2) tail_kernel(const ScenarioDev sc, cons
             const u32 ox = __shfl_sync(NS_FULL, (u32)pold_lo, 0), oy = __shfl_sync(NS_FULL, (u32)(pold_lo >> 32), 0);
             const u32 oz = __shfl_sync(NS_FULL, (u32)pold_hi, 0), ow = __shfl_sync(NS_FULL, (u32)(pold_hi >> 32), 0);
             if (ox == p_loc && oy == p_k && oz == p_j && ow != id) {   // another lineage executed it first (L687, L697)
-                if (FAST && !p_T_known) p_T = exact_offset<PERCELL>(sc, ep.key, smt, p_loc, p_k, p_j);
+                if (FAST && !p_T_known) { const uint2 pr = rate_of_loc<PERCELL>(sc, p_loc); p_T = exact_offset(ep.key, smt, p_loc, p_k, p_j, pr.x, pr.y); }
                 if (lane == 0) {
                     bf.parent[id] = ow; bf.state[id] = 2;
                     bf.term_loc[id] = p_loc; bf.term_k[id] = p_k; bf.term_j[id] = p_j; bf.term_f[id] = p_T; bf.steps[id] = steps;
@@ -353,24 +352,31 @@ __global__ void __launch_bounds__(256, 2) tail_kernel(const ScenarioDev sc, cons
                     u32 loc2o, c2o; uint2 cso = make_uint2(Cm, sh); bool acc, bad;
                     fast_slot_a<KIND, PERCELL, COMPACT>(sc, gl, sp_q, lane, bm, cell, ua, xi_lo, xi_hi, loc2o, c2o, cso, acc, bad);
                     // slot B of the lanes with sp_q == 0: approximate offsets of the candidates (partial sums over the points of interval k)
-                    float a = sp_q == 0u ? approx_exp_time(ub, ln2_over_mu) : 0.0f;
+                    // (the draw is tied to the target cell of slot A by an OR with zero: the table gathers, which have the longest latency,
+                    // are then issued before this chain starts)
+                    float a = sp_q == 0u ? approx_exp_time(ubh | (c2o & ep.zero), ln2_over_mu) : 0.0f;
                     { const float y = __shfl_up_sync(NS_FULL, a, 4); if (sp_add4) a += y; }
                     { const float y = __shfl_up_sync(NS_FULL, a, 8); if (sp_add8) a += y; }
                     { const float y = __shfl_up_sync(NS_FULL, a, 16); if (sp_add16) a += y; }
                     const float mc = margin + fm_last;
                     const bool ins = a < 1.0f - margin, outs = a > 1.0f + margin;
-                    const bool aft = a > fa_last + mc, bef = a < fa_last - mc;
+                    bool aft = a > fa_last + mc, bef = a < fa_last - mc;
+                    // a lineage that stayed where it was (self-dispersal) sees the points of the same stream again: after the last event
+                    // means a larger ordinal, exactly (the partial sums are the same numbers as in the round before)
+                    if (loc == e_loc && fa_last >= 0.0f) { aft = sp_c + 1u > e_j; bef = !aft; }
                     const bool kvalid = (ep.k_stop - k) > sp_dk;              // never look at or past the horizon (k < k_stop here)
-                    const bool amb = (ubh < (1u << 20)) || !(ins || outs) || (sp_in_k && !(aft || bef));
+                    // draws with hi < 2^20 (coarse logarithm) or hi >= 2^32 - 2^8 (an increment that may round to zero) are not decided here
+                    const bool amb = (ubh - (1u << 20) >= 0xFFEFFF00u) || !(ins || outs) || (sp_in_k && !(aft || bef));
                     const u32 evm = __ballot_sync(NS_FULL, sp_q == 0u && ins && (sp_in_k ? aft : kvalid));
                     const u32 crm = __ballot_sync(NS_FULL, sp_q == 0u && outs);
                     const u32 okm = __ballot_sync(NS_FULL, acc);
                     // trouble: an ambiguous comparison anywhere, or an undetermined target
-                    // trouble: an ambiguous comparison anywhere, an undetermined target, or (lane 0, which holds the result of the pending
+                    // trouble: an ambiguous comparison anywhere, or (lane 0, which holds the result of the pending
                     // exchange) a match there: another lineage executed the pending event first and this one is a duplicate
                     bool culled = false;
                     if (DEDUP) culled = lane == 0 && pend && (u32)pold_lo == p_loc && (u32)(pold_lo >> 32) == p_k && (u32)pold_hi == p_j && (u32)(pold_hi >> 32) != id;
-                    const u32 trm = __ballot_sync(NS_FULL, (sp_q == 0u && amb) || bad || culled);
+                    const u32 trm = __ballot_sync(NS_FULL, (sp_q == 0u && amb) || culled);
+                    const u32 badm = KIND == 3 ? __ballot_sync(NS_FULL, bad) : 0u;
                     // every candidate's outcome: the first accepted attempt of its four lanes (the sequential algorithm's choice, R16)
                     const int qsrc = (int)(qb + ((u32)first_bit(((okm >> qb) & 15u) | 16u) & 3u));
                     const u32 loc2q = __shfl_sync(NS_FULL, loc2o, qsrc), cq = __shfl_sync(NS_FULL, c2o, qsrc);
@@ -385,7 +391,7 @@ __global__ void __launch_bounds__(256, 2) tail_kernel(const ScenarioDev sc, cons
                     const u32 spec_w = (KIND == 1 && cell == 0) ? 0u : ((bm >> wl) & 2u);
                     const u32 steps_e = steps + (pend ? 2u : 1u);       // step count after this event
                     // clean: a winner, no trouble at the time lanes or in the winner's lanes, an attempt accepted, no speciation, no step cap
-                    const bool clean = wm != 0u && ((trm & (0x11111111u | q4)) | spec_w) == 0u && (okm & q4) != 0u && steps_e < cap_at;
+                    const bool clean = wm != 0u && ((trm & 0x11111111u) | (badm & q4) | spec_w) == 0u && (okm & q4) != 0u && steps_e < cap_at;
                     if (!__all_sync(NS_FULL, clean)) break;
                     // commit: event (loc, k2, j2) executed, the lineage moves to the winner's target
                     const u32 wc = wl >> 2;
@@ -403,7 +409,7 @@ __global__ void __launch_bounds__(256, 2) tail_kernel(const ScenarioDev sc, cons
                         if (probes) { p_loc = loc; p_k = k2; p_j = j2; p_T_known = false; pend = true; }
                         else steps++;
                     } else steps++;
-                    e_loc = loc; e_j = j2; f_exact = false; fa_last = a_w; fm_last = margin;
+                    e_loc = loc; e_j = j2; e_Cm = Cm; e_sh = sh; f_exact = false; fa_last = a_w; fm_last = margin;
                     if (PERCELL) {
                         Cm = __shfl_sync(NS_FULL, Cmq, (int)wl); sh = __shfl_sync(NS_FULL, shq, (int)wl);
                         const float finv = rate_to_float(Cm, sh);
@@ -412,7 +418,7 @@ __global__ void __launch_bounds__(256, 2) tail_kernel(const ScenarioDev sc, cons
                     k = k2; loc = loc2; cell = cell2;
                 }
                 // the round that was not clean is done below in exact arithmetic, from the exact lower bound
-                if (!f_exact) { f_last = (i64)exact_offset<PERCELL>(sc, ep.key, smt, e_loc, k, e_j); f_exact = true; }
+                if (!f_exact) { f_last = (i64)exact_offset(ep.key, smt, e_loc, k, e_j, e_Cm, e_sh); f_exact = true; }
                 c_exact++;
             }
             u32 j;
@@ -602,6 +608,7 @@ __global__ void __launch_bounds__(256, 2) tail_kernel(const ScenarioDev sc, cons
                 }
                 break;
             }
+            if (FAST) { e_loc = loc; e_j = j; e_Cm = Cm; e_sh = sh; }
             f_last = (i64)Te; loc = loc2; cell = cell2; Cm = Cm2; sh = sh2;
             if (FAST) {
                 f_exact = true; fa_last = (float)Te * 0x1p-48f; fm_last = 2.4e-07f;   // binary32 rounding of an offset < 1
