@@ -209,6 +209,12 @@ int necsim_debug_draw(uint64_t seed, int lane, const uint32_t *d_loc, const uint
                       uint64_t *d_out, uint64_t n, void *cuda_stream);
 /* fixed-point -ln, DESIGN.md 2.3 (PAPER.md Eq. C.3) */
 int necsim_debug_neglog(const uint64_t *d_x, uint64_t *d_out, uint64_t n, void *cuda_stream);
+/* The tail kernel's fast round decides the comparisons of the event-time search in binary32 where the outcome is
+ * certain and redoes the round in fixed point otherwise. For every draw d_x[i] and the turnover scale (Cm, sh):
+ * d_approx[i] = the binary32 offset of the draw, d_exact[i] = the Q16.48 offset of 2.4; *d_margin = the margin the kernel uses for
+ * this scale. tests/test_gpu_primitives.py checks |approx - exact| against it. All pointers DEVICE. */
+int necsim_debug_approx_time(const uint64_t *d_x, uint32_t Cm, uint32_t sh, float *d_approx, uint64_t *d_exact, float *d_margin, uint64_t n,
+                             void *cuda_stream);
 /* event-time search, DESIGN.md 2.4. rc[i]: 0 found, -3 k overflow */
 int necsim_debug_next_event(uint64_t seed, const uint32_t *d_loc, const uint32_t *d_k, const int64_t *d_f_last, const uint32_t *d_Cm,
                             const uint32_t *d_sh, uint32_t *d_k_out, uint32_t *d_j_out, uint64_t *d_T_out, int32_t *d_rc, uint64_t n,

@@ -906,6 +906,21 @@ __global__ void debug_next_event_poisson_kernel(const ScenarioDev sc, SeedKey ke
     }
 }
 
+// the fast round's binary32 offset of one draw beside the exact one, for the error-bound test of the filter
+__global__ void debug_approx_time_kernel(const u64 *x, u32 Cm, u32 sh, float *approx, u64 *exact, float *margin, u64 n) {
+    __shared__ unsigned short sQ[512];
+    __shared__ u64 sA[512];
+    for (u32 i = threadIdx.x; i < 512; i += blockDim.x) { sQ[i] = NEGLOG_Q_DEV[i]; sA[i] = NEGLOG_A_DEV[i]; }
+    __syncthreads();
+    SmemTables smt; smt.q = smem_addr(sQ); smt.a = smem_addr(sA); smt.tg = smt.g2 = 0;
+    u64 i = (u64)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const float finv = rate_to_float(Cm, sh);
+    approx[i] = approx_exp_time((u32)(x[i] >> 32), NS_LN2F * finv);
+    exact[i] = scale_exp(neglog(x[i], smt), Cm, sh);
+    if (i == 0) *margin = NS_MARGIN * (1.0f + finv);
+}
+
 static inline u32 grid_for(u64 n, u32 block) { return (u32)((n + block - 1) / block); }
 
 extern "C" int necsim_debug_draw(uint64_t seed, int lane, const uint32_t *d_loc, const uint32_t *d_k, const uint32_t *d_j, const uint32_t *d_r,
@@ -920,6 +935,15 @@ extern "C" int necsim_debug_neglog(const uint64_t *d_x, uint64_t *d_out, uint64_
     int rc = upload_neglog_tables((cudaStream_t)cuda_stream);
     if (rc) return rc;
     debug_neglog_kernel<<<grid_for(n, 256), 256, 0, (cudaStream_t)cuda_stream>>>(d_x, d_out, n);
+    CU(cudaGetLastError());
+    return NECSIM_OK;
+}
+extern "C" int necsim_debug_approx_time(const uint64_t *d_x, uint32_t Cm, uint32_t sh, float *d_approx, uint64_t *d_exact, float *d_margin, uint64_t n,
+                                        void *cuda_stream) {
+    if (n == 0) return NECSIM_OK;
+    int rc = upload_neglog_tables((cudaStream_t)cuda_stream);
+    if (rc) return rc;
+    debug_approx_time_kernel<<<grid_for(n, 256), 256, 0, (cudaStream_t)cuda_stream>>>(d_x, Cm, sh, d_approx, d_exact, d_margin, n);
     CU(cudaGetLastError());
     return NECSIM_OK;
 }

@@ -17,7 +17,7 @@ EXPORTS = ["necsim_scenario_workspace_size", "necsim_create_scenario", "necsim_s
            "necsim_simulate_workspace_size", "necsim_simulate", "necsim_simulate_host", "necsim_destroy", "necsim_last_error",
            "necsim_debug_draw", "necsim_debug_neglog", "necsim_debug_next_event", "necsim_debug_disperse", "necsim_debug_tables",
            "necsim_debug_int_peak", "necsim_debug_next_event_poisson", "necsim_debug_poisson_table",
-           "necsim_merge_workspace_size", "necsim_merge_species"]
+           "necsim_merge_workspace_size", "necsim_merge_species", "necsim_debug_approx_time"]
 
 
 class ScenarioDesc(C.Structure):
@@ -87,6 +87,7 @@ def lib():
         L.necsim_debug_int_peak.argtypes = [C.c_int, u32, vp, vp, vp, vp]
         L.necsim_debug_next_event_poisson.argtypes = [vp, u64] + [vp] * 8 + [u64, vp]
         L.necsim_debug_poisson_table.argtypes = [vp] * 5
+        L.necsim_debug_approx_time.argtypes = [vp, u32, u32, vp, vp, vp, u64, vp]
         L.necsim_merge_workspace_size.argtypes = [u64, vp]
         L.necsim_merge_species.argtypes = [vp, u64, vp, C.c_size_t, vp, vp, vp, vp]
         _lib = L
@@ -333,6 +334,16 @@ def debug_neglog(x):
     out = torch.empty_like(dx)
     _check(lib().necsim_debug_neglog(dx.data_ptr(), out.data_ptr(), len(x), _stream_ptr(torch)))
     return out.cpu().numpy().view(np.uint64)
+
+
+def debug_approx_time(x, Cm, sh):
+    """(binary32 offsets of the fast round, exact Q16.48 offsets, the kernel's margin) for an array of 64-bit draws."""
+    torch = _torch()
+    x = np.ascontiguousarray(x, dtype=np.uint64)
+    dx = torch.from_numpy(x.view(np.int64)).cuda()
+    ap = torch.empty(len(x), dtype=torch.float32, device="cuda"); ex = torch.empty_like(dx); mg = torch.zeros(1, dtype=torch.float32, device="cuda")
+    _check(lib().necsim_debug_approx_time(dx.data_ptr(), int(Cm), int(sh), ap.data_ptr(), ex.data_ptr(), mg.data_ptr(), len(x), _stream_ptr(torch)))
+    return ap.cpu().numpy(), ex.cpu().numpy().view(np.uint64), float(mg.item())
 
 
 def debug_next_event(seed, loc, k, f_last, Cm, sh):

@@ -82,3 +82,33 @@ def test_tables_and_dispersal_bit_exact(ns, O, I):
         k = rng.integers(0, 1000, n).astype(np.uint32); j = rng.integers(1, 9, n).astype(np.uint32)
         assert np.array_equal(g.debug_disperse(cfg["seed"], loc, k, j), O.batch_disperse(o, cfg["seed"], loc, k, j)), cfg["name"]
         g.close()
+
+
+def test_fast_round_filter_error_bound(ns, O):
+    """The tail kernel's fast round compares binary32 offsets (top 32 bits of a draw, lg2.approx) and only trusts a comparison
+    further than `margin` from equality. Pin of that filter: over the draws it accepts (2^20 <= hi < 2^32 - 2^8)
+    the binary32 offset is within margin / 8 of the exact Q16.48 offset of DESIGN.md 2.4 (taken from the ORACLE), for turnover
+    scales over the whole admissible range of mu; partial sums of up to five terms then stay within margin / 1.6."""
+    rng = np.random.default_rng(11)
+    n = 2_000_003
+    x = rng.integers(0, 1 << 64, n, dtype=np.uint64)
+    x[: n // 4] |= np.uint64(0xFFF0_0000_0000_0000)                      # many draws near U = 1 (tiny offsets)
+    q = n // 4
+    x[q: 2 * q] >>= rng.integers(0, 12, q).astype(np.uint64)             # small U (large offsets), down to hi = 2^20
+    hi = x >> np.uint64(32)
+    ok = (hi >= (1 << 20)) & (hi < (1 << 32) - (1 << 8))
+    x = x[ok]
+    E = O.batch_neglog(x)
+    for lam_dt in (1.0 / 200, 0.1, 0.5, 1.0, 2.0, 3.0, 17.0, 64.0):
+        Cm, sh = O.turnover_scale(lam_dt, 1.0)
+        ap, ex, margin = ns.debug_approx_time(x, Cm, sh)
+        ref = np.array([O.scale(int(e), Cm, sh) for e in E[:2000]], dtype=np.uint64)
+        assert np.array_equal(ex[:2000], ref)                            # the exact side of the export is the oracle's arithmetic
+        t = ex.astype(np.float64) * 2.0 ** -48
+        rel = t < 2.0                                                    # offsets that can take part in a decision (sums near <= 1)
+        err = np.abs(ap.astype(np.float64) - t)[rel]
+        assert err.size > 1000 and err.max() <= margin / 8.0, (lam_dt, err.max(), margin)
+    # zero increments cannot hide behind an accepted draw: hi < 2^32 - 2^8 means an exact offset > 0
+    Cm, sh = O.turnover_scale(64.0, 1.0)
+    _, ex, _ = ns.debug_approx_time(x, Cm, sh)
+    assert (ex > 0).all()
