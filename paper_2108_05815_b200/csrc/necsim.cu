@@ -6,6 +6,7 @@
 #include <math.h>
 #include <stdio.h>
 #include <string.h>
+#include <stdlib.h>
 #include <string>
 #include <vector>
 #include <algorithm>
@@ -202,7 +203,7 @@ extern "C" int necsim_create_scenario(const necsim_scenario_desc *d, void *d_wor
     memset(&sd, 0, sizeof(sd));
     sd.kind = d->kind; sd.delta_t = d->delta_t; sd.width_shift = 0xFFFFFFFFu;
     uint8_t *base = (uint8_t *)d_workspace;
-    double mu_max = 0.0;
+    double mu_max = 0.0, mu_min = 1e300;
     const u32 n = L.ncells;
 
     if (d->kind == NECSIM_SPATIALLY_IMPLICIT) {
@@ -210,7 +211,7 @@ extern "C" int necsim_create_scenario(const necsim_scenario_desc *d, void *d_wor
         sd.J_local = (u32)d->local_size; sd.J_meta = (u32)d->meta_size;
         sd.n_locations = d->local_size + d->meta_size; sd.n_sampleable = d->local_size;
         if (!turnover_scale(d->uniform_turnover, d->delta_t, sd.Cm_u, sd.sh_u)) return fail(NECSIM_ERR_INVALID_ARG, "turnover*delta_t out of range");
-        mu_max = d->uniform_turnover * d->delta_t;
+        mu_max = mu_min = d->uniform_turnover * d->delta_t;
     } else {
         sd.width = d->width; sd.height = d->height; sd.ncells = n;
         if ((d->width & (d->width - 1)) == 0) { u32 s = 0; while ((1u << s) < d->width) ++s; sd.width_shift = s; }
@@ -242,13 +243,13 @@ extern "C" int necsim_create_scenario(const necsim_scenario_desc *d, void *d_wor
                 u32 dm = L.uniform_deme ? sd.uniform_deme : d->deme[c];
                 if (dm > 0) {
                     if (!turnover_scale(d->turnover[c], d->delta_t, scale[c].x, scale[c].y)) return fail(NECSIM_ERR_INVALID_ARG, "turnover*delta_t out of range");
-                    mu_max = std::max(mu_max, d->turnover[c] * d->delta_t);
+                    mu_max = std::max(mu_max, d->turnover[c] * d->delta_t); mu_min = std::min(mu_min, d->turnover[c] * d->delta_t);
                 } else scale[c] = make_uint2(0, 0);
             }
             sd.per_cell_turnover = 1;
         } else {
             if (!turnover_scale(d->uniform_turnover, d->delta_t, sd.Cm_u, sd.sh_u)) return fail(NECSIM_ERR_INVALID_ARG, "turnover*delta_t out of range");
-            mu_max = d->uniform_turnover * d->delta_t;
+            mu_max = mu_min = d->uniform_turnover * d->delta_t;
         }
         if (tables) {
             CU(cudaMemcpyAsync(base + L.off_hab8, hab8.data(), n, cudaMemcpyHostToDevice, st));
@@ -302,6 +303,7 @@ extern "C" int necsim_create_scenario(const necsim_scenario_desc *d, void *d_wor
         }
     }
     sd.sampler = d->sampler;
+    sd.margin = (float)(6.1035156e-05 * (1.0 + 1.0 / mu_min));   // NS_MARGIN * (1 + 1/mu_min)
     if (d->sampler) {   // Poisson sampler tables: cdf thresholds of mu_max; per-cell thinning thresholds
         std::vector<u64> pc(NS_POIS_N);
         double p = exp(-mu_max), cdf = 0.0;
@@ -587,12 +589,17 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
             ep.lanes_per_warp = 32;
             grid = (u32)std::min<u64>(tail_grid, ((u64)active + warps_per_block - 1) / warps_per_block);
         } else {
+            // Fewer lineages than lanes: fill warps, not the machine. A warp's pass costs the same whether 4 or 32 of its lanes hold
+            // lineages, and with more than about four warps per scheduler the warps wait for issue slots instead of for their own
+            // dependent instructions: 20 000 lineages of C5 spread over all 5 920 resident warps ran at 5.3 us per sequential event,
+            // packed into 16 warps per SM at 1.8 us. So: 16 warps per SM (four per scheduler) as full as the lineages make them,
+            // more warps only when those are full.
             const u64 total_warps = (u64)full_grid * warps_per_block;
-            u32 lanes = 32;
-            if ((u64)active < total_warps * 32ull) lanes = (u32)std::max<u64>(1, ((u64)active + total_warps - 1) / total_warps);
+            const u64 few_warps = std::min<u64>(total_warps, 16ull * (u64)scn->sm_count);
+            u64 warps = std::min<u64>(total_warps, std::max<u64>(few_warps, ((u64)active + 31) / 32));
+            u32 lanes = (u32)std::min<u64>(32, std::max<u64>(1, ((u64)active + warps - 1) / warps));
             ep.lanes_per_warp = lanes;
-            grid = full_grid;
-            if (lanes == 1) grid = (u32)std::min<u64>(full_grid, ((u64)active + warps_per_block - 1) / warps_per_block);
+            grid = (u32)std::min<u64>(full_grid, (warps + warps_per_block - 1) / warps_per_block);
         }
         ep.rec_chunk = 1;
         if (rp.record && tail) {   // chunked ring reservation: at most a quarter of the ring may sit in unused reservations
@@ -616,6 +623,9 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
         CU(cudaEventElapsedTime(&ms, scn->ev[2], scn->ev[3]));
         ms_sim += ms;
         ++n_epochs; ++n_launch;
+        if (getenv("NECSIM_TRACE"))   // per-epoch trace for diagnosis (stderr)
+            fprintf(stderr, "[necsim] epoch %llu %s k=[%u,%u) active=%u grid=%u lanes=%u events=%llu culled=%llu ms=%.3f\n", (unsigned long long)n_epochs, tail ? "tail" : "lane",
+                    ep.k_start, k_stop, active, grid, ep.lanes_per_warp, (unsigned long long)(hc->n_events - ev_before), (unsigned long long)hc->n_culled, ms);
         if (tail) { ms_tail += ms; ++n_tail_epochs; ev_tail += hc->n_events - ev_before; }
         ev_before = hc->n_events;
         if (hc->error) return fail(NECSIM_ERR_CAPACITY, "interval index overflowed 2^32 or dispersal resampling exhausted");

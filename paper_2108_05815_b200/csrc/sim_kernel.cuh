@@ -184,6 +184,57 @@ __device__ __forceinline__ void record_event(const SimBuffers &bf, u32 loc, u32 
     if (idx < bf.rec_cap) { bf.rec_loc[idx] = loc; bf.rec_k[idx] = k; bf.rec_j[idx] = j; bf.rec_f[idx] = f; bf.rec_loc2[idx] = loc2; }
 }
 
+// ---- approximate event times: the search filter of both simulate kernels (exponential sampler) ----------------------------------------------------
+// The decisions of the event-time search ("T >= 2^48" and "T > f_last") are comparisons of partial sums of
+// -ln(U_i)/mu. The kernels evaluate them in binary32 from the top 32 bits of each draw: A = (32 - lg2(hi)) * ln2 / mu.
+// |A_j - T_j| is bounded ("filter"): a comparison further than the margin from equality has the same outcome as
+// the fixed-point comparison of 2.4, anything closer (or a draw with hi < 2^20) is "ambiguous" and the round is redone with
+// the exact arithmetic. Exact offsets are needed for records only and are recomputed from the event identity (loc, k, j):
+// T(loc, k, j) is a pure function of it (exact_offset).
+#define NS_LN2F 0.69314718f
+#define NS_MARGIN 6.1035156e-05f                     // 2^-14, times (1 + 1/mu)
+// volatile: stays after the table gathers of slot A in issue order (the gathers have the longest latency and go first)
+__device__ __forceinline__ float lg2_approx(float x) { float y; asm volatile("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+// 1/mu = Cm * 2^-(24 + sh) as binary32 (T = (E * Cm) >> (32 + sh) with E in Q8.56, T in Q16.48)
+__device__ __forceinline__ float rate_to_float(u32 Cm, u32 sh) { return __uint2float_rz(Cm) * __uint_as_float((103u - sh) << 23); }
+__device__ __forceinline__ float approx_exp_time(u32 draw_hi, float ln2_over_mu) {
+    return (32.0f - lg2_approx(__uint2float_rz(draw_hi))) * ln2_over_mu;
+}
+
+// (Cm, sh) of the cell that holds indexed location loc
+template <bool PERCELL>
+__device__ __forceinline__ uint2 rate_of_loc(const ScenarioDev &sc, u32 loc) {
+    if (!PERCELL) return make_uint2(sc.Cm_u, sc.sh_u);
+    return __ldg(&sc.scale[cell_of_loc(sc, loc)]);
+}
+// exact offset T of the event (loc, k, j): the sum of the first j scaled draws of the stream primed on (loc, k)
+__device__ __forceinline__ u64 exact_offset(const SeedKey &key, const SmemTables &smt, u32 loc, u32 k, u32 j, u32 Cm, u32 sh) {
+    u64 X = prime(key, loc, k), T = 0;
+    for (u32 i = 0; i < j; ++i) { X += NS_GAMMA; T += scale_exp(neglog(draw_time(X), smt), Cm, sh); }
+    return T;
+}
+// out-of-line variants for the per-lane kernel, where these rare paths must not cost registers
+__device__ __noinline__ u64 exact_offset_nl(SeedKey key, u32 q_addr, u32 a_addr, u32 loc, u32 k, u32 j, u32 Cm, u32 sh) {
+    SmemTables smt; smt.q = q_addr; smt.a = a_addr; smt.tg = smt.g2 = smt.pc = smt.pg = 0;
+    return exact_offset(key, smt, loc, k, j, Cm, sh);
+}
+// exact offset of the event (loc, k, j) with the rate of the cell that holds loc (explicit kinds with per-cell turnover)
+__device__ __noinline__ u64 exact_offset_of_loc_nl(SeedKey key, u32 q_addr, u32 a_addr, const u32 *prefix, const uint2 *scale, u32 ncells, u32 uniform_deme,
+                                                   u32 loc, u32 k, u32 j) {
+    u32 c;
+    if (uniform_deme) c = loc / uniform_deme;
+    else { u32 lo = 0, hi = ncells; while (hi - lo > 1) { u32 mid = lo + ((hi - lo) >> 1); if (prefix[mid] <= loc) lo = mid; else hi = mid; } c = lo; }
+    const uint2 cs = __ldg(&scale[c]);
+    SmemTables smt; smt.q = q_addr; smt.a = a_addr; smt.tg = smt.g2 = smt.pc = smt.pg = 0;
+    return exact_offset(key, smt, loc, k, j, cs.x, cs.y);
+}
+
+// phase choice of a pass: SEARCH while n_event * WE <= n_search * WS. Measured on C5 MODE-T: 1:1 (the majority phase) 2.92e10
+// events/s, 1:2 (weighted by the cost of a pass: an event pass is about twice a search pass) 2.83e10
+#ifndef NS_PHASE_WE
+#define NS_PHASE_WE 1u
+#define NS_PHASE_WS 1u
+#endif
 #define NS_ST_IDLE 0u
 #define NS_ST_SEARCH 1u     // needs draws of the event-time search (re-primes first when `need_prime`)
 #define NS_ST_EVENT 2u      // event (loc, k, j) found at offset T: `att` dispersal attempts rejected so far
@@ -212,6 +263,13 @@ __global__ void __launch_bounds__(256) simulate_kernel(const ScenarioDev sc, con
     u32 id = 0, loc = 0, cell = 0, k = 0, steps = 0, j = 0, Cm = sc.Cm_u, sh = sc.sh_u;
     i64 f_last = -1;
     u64 X = 0, T = 0;
+    // search filter (FILT: exponential sampler without the event stream): the partial sum `a` and the lower bound `fa_last` are
+    // binary32 (see approx_exp_time); exact offsets are recomputed from the event identity where a record or an ambiguous comparison
+    // needs them. (e_loc, k, e_j) = the last executed event, whose offset is the exact lower bound while fa_last >= 0.
+    constexpr bool FILT = (SAMP == 0) && !REC;
+    float a = 0.0f, fa_last = -1.0f, lnmu = NS_LN2F * rate_to_float(sc.Cm_u, sc.sh_u);
+    u32 e_loc = 0xFFFFFFFFu, e_j = 0;
+    const float margin = sc.margin;
     u32 c_events = 0, c_culled = 0, c_resamples = 0;   // per-thread counters, reduced at the end
 
     for (;;) {
@@ -228,7 +286,7 @@ __global__ void __launch_bounds__(256) simulate_kernel(const ScenarioDev sc, con
                 if (idx < bf.q_in_count) {
                     uint4 e = bf.q_in[idx];
                     id = e.x; loc = e.y; cell = e.z; steps = e.w;
-                    k = ep.k_start; f_last = -1; need_prime = true; st = NS_ST_SEARCH;
+                    k = ep.k_start; f_last = -1; fa_last = -1.0f; need_prime = true; st = NS_ST_SEARCH;
                 }
             }
             exhausted = (base + cnt >= bf.q_in_count);
@@ -237,7 +295,7 @@ __global__ void __launch_bounds__(256) simulate_kernel(const ScenarioDev sc, con
         const u32 n_search = __popc(bs), n_event = __popc(be);
         if ((n_search | n_event) == 0u) break;
 
-        if (n_event <= n_search) {
+        if (n_event * NS_PHASE_WE <= n_search * NS_PHASE_WS) {
             // ======== SEARCH phase ======================================================================
             // S1a: (re-)prime on (loc, k); pause at the epoch horizon
             bool pause = false;
@@ -246,9 +304,12 @@ __global__ void __launch_bounds__(256) simulate_kernel(const ScenarioDev sc, con
                     pause = true;
                 } else {
                     X = prime(ep.key, loc, k);
-                    T = 0; j = 0; need_prime = false;
+                    T = 0; a = 0.0f; j = 0; need_prime = false;
                     if (SAMP == 0) {
-                        if (PERCELL) { uint2 cs = __ldg(&sc.scale[KIND == 3 ? xy_index(sc, cell) : cell]); Cm = cs.x; sh = cs.y; }
+                        if (PERCELL) {
+                            uint2 cs = __ldg(&sc.scale[KIND == 3 ? xy_index(sc, cell) : cell]); Cm = cs.x; sh = cs.y;
+                            if (FILT) lnmu = NS_LN2F * rate_to_float(Cm, sh);
+                        }
                     } else {   // sh = number of points of this interval, Cm = thinning threshold of the cell, att = best point so far
                         sh = poisson_count(X, smt); att = 0;
                         if (PERCELL) Cm = __ldg(&sc.thin[KIND == 3 ? xy_index(sc, cell) : cell]);
@@ -283,7 +344,7 @@ __global__ void __launch_bounds__(256) simulate_kernel(const ScenarioDev sc, con
                     else { k += 1; f_last = -1; need_prime = true; }
                 }
             }
-            if (SAMP == 0 && st == NS_ST_SEARCH) {
+            if (SAMP == 0 && !FILT && st == NS_ST_SEARCH) {
                 // S1b: one exponential draw of the event-time search
                 j += 1; X += NS_GAMMA;
                 T += scale_exp(neglog(draw_time(X), smt), Cm, sh);
@@ -291,6 +352,33 @@ __global__ void __launch_bounds__(256) simulate_kernel(const ScenarioDev sc, con
                     if (k == 0xFFFFFFFFu) { atomicMax(&bf.ctr->error, 3u); st = NS_ST_IDLE; }
                     else { k += 1; f_last = -1; need_prime = true; }
                 } else if ((i64)T > f_last) {              // strictly later than the last event (L729): the next event
+                    st = NS_ST_EVENT; att = 0;
+                }
+            }
+            if (FILT && st == NS_ST_SEARCH) {
+                // S1b: one exponential draw of the event-time search, decided in binary32 where the outcome is certain
+                j += 1; X += NS_GAMMA;
+                const u32 hh = (u32)(draw_time(X) >> 32);
+                a += approx_exp_time(hh, lnmu);
+                bool outs = a > 1.0f + margin;                                           // T >= 2^48: interval exhausted
+                const bool ins = a < 1.0f - margin;
+                bool aft = a > fa_last + 2.0f * margin, bef = a < fa_last - 2.0f * margin;   // T > f_last (strictly later, L729)
+                if (loc == e_loc && fa_last >= 0.0f) { aft = j > e_j; bef = !aft; }      // same stream as the last event: by ordinal
+                // not decided here: coarse logarithm (hi < 2^20), an increment that may round to zero (hi >= 2^32 - 2^8), a partial
+                // sum of many terms, a comparison inside the margin
+                if ((hh - (1u << 20) >= 0xFFEFFF00u) || j > 32u || !(ins || outs) || (ins && !(aft || bef))) {
+                    const u64 Tx = exact_offset_nl(ep.key, smt.q, smt.a, loc, k, j, Cm, sh);
+                    i64 fl = -1;
+                    if (fa_last >= 0.0f)
+                        fl = PERCELL ? (i64)exact_offset_of_loc_nl(ep.key, smt.q, smt.a, sc.prefix, sc.scale, sc.ncells, sc.uniform_deme, e_loc, k, e_j)
+                                     : (i64)exact_offset_nl(ep.key, smt.q, smt.a, e_loc, k, e_j, Cm, sh);
+                    outs = Tx >= NS_TWO48; aft = (i64)Tx > fl;
+                    a = (float)Tx * 0x1p-48f;
+                }
+                if (outs) {                                // interval exhausted: cross and re-prime (L719, L727)
+                    if (k == 0xFFFFFFFFu) { atomicMax(&bf.ctr->error, 3u); st = NS_ST_IDLE; }
+                    else { k += 1; fa_last = -1.0f; need_prime = true; }
+                } else if (aft) {                          // the next event
                     st = NS_ST_EVENT; att = 0;
                 }
             }
@@ -336,6 +424,7 @@ __global__ void __launch_bounds__(256) simulate_kernel(const ScenarioDev sc, con
             }
             if (att == 0) {
                 if (DEDUP) culled = old.x == loc && old.y == k && old.z == j && old.w != id;
+                if (FILT && (culled || speciates)) T = exact_offset_nl(ep.key, smt.q, smt.a, loc, k, j, Cm, sh);   // the record's exact offset
                 if (culled) {
                     // another lineage executed this event: identical future (L687, L697) -> cull, link to it
                     bf.parent[id] = old.w; bf.state[id] = 2;
@@ -343,6 +432,7 @@ __global__ void __launch_bounds__(256) simulate_kernel(const ScenarioDev sc, con
                     c_culled++; st = NS_ST_IDLE;
                 } else {
                     f_last = (i64)T; steps++; c_events++;
+                    if (FILT) { fa_last = a; e_loc = loc; e_j = j; }
                     if (speciates) {
                         bf.state[id] = 1;
                         bf.term_loc[id] = loc; bf.term_k[id] = k; bf.term_j[id] = j; bf.term_f[id] = T; bf.steps[id] = steps;
@@ -358,6 +448,7 @@ __global__ void __launch_bounds__(256) simulate_kernel(const ScenarioDev sc, con
                     if (REC) record_event(bf, loc, k, j, T, loc2);
                     loc = loc2; cell = cell2; need_prime = true; st = NS_ST_SEARCH;
                     if (ep.max_steps && steps >= ep.max_steps) {
+                        if (FILT) T = exact_offset_nl(ep.key, smt.q, smt.a, e_loc, k, j, Cm, sh);   // (Cm, sh) are still the origin's
                         bf.state[id] = 3;
                         bf.term_loc[id] = loc; bf.term_k[id] = k; bf.term_j[id] = j; bf.term_f[id] = T; bf.steps[id] = steps;
                         st = NS_ST_IDLE;

@@ -35,6 +35,7 @@ struct ScenarioDev {
     int R;                     // displacement range: dx in [-R, R]
     u32 gauss_len;             // power of two >= 2R
     double delta_t;
+    float margin;              // search filter (exponential sampler): NS_MARGIN * (1 + 1/mu_min), mu_min over the habitat cells
 };
 
 // Device counters of one simulate call (zeroed at its start). 64-bit where they can exceed 2^32.

@@ -150,36 +150,6 @@ __device__ __forceinline__ void gauss_target(const ScenarioDev &sc, const GaussL
     }
 }
 
-// ---- approximate event times for the fast round (exponential sampler) ----------------------------------------------------
-// The decisions of the event-time search ("T >= 2^48" and "T > f_last") are comparisons of partial sums of
-// -ln(U_i)/mu. The fast round evaluates them in binary32 from the top 32 bits of each draw: A = (32 - lg2(hi)) * ln2 / mu.
-// |A_j - T_j| is bounded ("filter"): a comparison further than the margin from equality has the same outcome as
-// the fixed-point comparison of 2.4, anything closer (or a draw with hi < 2^20) is "ambiguous" and the round is redone with
-// the exact arithmetic. Exact offsets are needed for records only and are recomputed from the event identity (loc, k, j):
-// T(loc, k, j) is a pure function of it (exact_offset).
-#define NS_LN2F 0.69314718f
-#define NS_MARGIN 6.1035156e-05f                     // 2^-14, times (1 + 1/mu)
-// volatile: stays after the table gathers of slot A in issue order (the gathers have the longest latency and go first)
-__device__ __forceinline__ float lg2_approx(float x) { float y; asm volatile("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
-// 1/mu = Cm * 2^-(24 + sh) as binary32 (T = (E * Cm) >> (32 + sh) with E in Q8.56, T in Q16.48)
-__device__ __forceinline__ float rate_to_float(u32 Cm, u32 sh) { return __uint2float_rz(Cm) * __uint_as_float((103u - sh) << 23); }
-__device__ __forceinline__ float approx_exp_time(u32 draw_hi, float ln2_over_mu) {
-    return (32.0f - lg2_approx(__uint2float_rz(draw_hi))) * ln2_over_mu;
-}
-
-// (Cm, sh) of the cell that holds indexed location loc
-template <bool PERCELL>
-__device__ __forceinline__ uint2 rate_of_loc(const ScenarioDev &sc, u32 loc) {
-    if (!PERCELL) return make_uint2(sc.Cm_u, sc.sh_u);
-    return __ldg(&sc.scale[cell_of_loc(sc, loc)]);
-}
-// exact offset T of the event (loc, k, j): the sum of the first j scaled draws of the stream primed on (loc, k)
-__device__ __forceinline__ u64 exact_offset(const SeedKey &key, const SmemTables &smt, u32 loc, u32 k, u32 j, u32 Cm, u32 sh) {
-    u64 X = prime(key, loc, k), T = 0;
-    for (u32 i = 0; i < j; ++i) { X += NS_GAMMA; T += scale_exp(neglog(draw_time(X), smt), Cm, sh); }
-    return T;
-}
-
 __device__ __forceinline__ uint2 lds_v2_ordered(u32 addr) { uint2 v; asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(addr)); return v; }
 // (x * d) >> 64 for a 32-bit d (see mulhi64_u32), with the two halves of x given
 __device__ __forceinline__ u32 mulhi64_u32_parts(u32 xlo, u32 xhi, u32 d) {
