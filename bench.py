@@ -6,7 +6,9 @@
 A "step" is one pass of the whole hot path S0-S6 (necsim_simulate: sample mask -> lineage queue, epochs of
 the simulate kernel with duplicate culling, sort/unique -> species) over the synthetic config. Default workload:
 C5 (BASELINE.json configs[4], the largest; the one north_star quotes the roofline target on).
-`value` = raw lineage events executed per second, whole job, inputs resident in HBM (device time, CUDA events).
+`value` = DISTINCT lineage events (loc, k, j) per second of the whole job (the oracle's count of the workload, scheduling
+          independent), inputs resident in HBM (device time, CUDA events); raw executed events per second ride along as
+          `raw_events_per_s` (redundancy = raw / distinct). Without a stored count (reduced configs) value = raw, `value_kind` says which.
 `e2e`   = the same through necsim_simulate_host: pinned host mask in, events + labels back to the host each step.
 `--impl reference` times the CPU oracle (as it stands, one core) on a bounded sample of the same workload.
 """
@@ -32,9 +34,26 @@ SMALL = dict(zip(("c1", "c2", "c3", "c4", "c5"), range(5)))
 # Algorithmic integer instructions per executed event (minimal 32-bit instruction sequence of
 # each primitive, weighted by the expected number of draws per event at mu = 2 and the measured attempts per event).
 I_EVENT = dict(c1=230, c2=232, c3=252, c4=263, c5=272, c6=259)   # c6: one attempt + 5 % resampling, index draw, deme32 gather
+# The same count when the event-time search is decided by the binary32 filter (a time draw is then hash 12 +
+# advance 2 + lg2 / scale 4 + accumulate and compare 5 = 23 instead of 68): what the kernels must issue at the least.
+I_EVENT_FILTERED = dict(c1=118, c2=120, c3=140, c4=151, c5=160, c6=147)
 # issue-slot peak: 148 SMs x 4 schedulers x 32 lanes x 1 instr/clk x sm_max_mhz (B300_MICROARCH "Pipe rates")
 def alu_peak(sm_count, sm_mhz):
     return sm_count * 4 * 32 * sm_mhz * 1e6
+
+
+def profile_traffic(kernel, name, sampler):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel, read from the committed ncu summary
+    (profiles/r2_ncu_<kernel>_<config>.md, line `traffic_bytes_per_launch=N`); None when there is no capture for this case."""
+    if sampler != "exp":
+        return None, None
+    f = os.path.join(ROOT, "profiles", "r2_ncu_%s_%s.md" % (kernel, name))
+    if not os.path.exists(f):
+        return None, None
+    for line in open(f):
+        if line.startswith("traffic_bytes_per_launch="):
+            return int(line.split("=")[1].split()[0]), os.path.relpath(f, ROOT)
+    return None, None
 
 
 def make_cfg(name, small):
@@ -219,49 +238,62 @@ def main():
     (ms, e2e_ms, sim_ms), (ev_all, e2e_ev_all) = D.aggregate([ms, e2e_s * 1e3, sim_ms], [float(ev), float(e2e_ev)], device="cuda")
     if rank == 0:
         K = args.steps
-        value = D.throughput(ev_all, ms)
+        raw_value = D.throughput(ev_all, ms)
+        uniq = unique_events(cfg, args) if world == 1 else None      # the stored count belongs to the config's own seed (rank 0)
+        value, value_kind = (uniq * K / (ms * 1e-3), "distinct events (oracle's count of the workload) / device time") if uniq else \
+                            (raw_value, "raw executed events / device time (no stored count of distinct events for this case)")
         prop = torch.cuda.get_device_properties(local)
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))) if os.path.exists(os.path.join(ROOT, "MEASURED_PEAKS.json")) else {}
         sm_max = float(peaks.get("sm_max_mhz", clocks.get("sm_max_mhz") or 1965.0))
         peak = alu_peak(prop.multi_processor_count, sm_max)
-        # dominant kernel of a step = tail_kernel (95.7 % of the step in the ncu launch list, profiles/r1_launches_c5.md):
-        # algorithmic instructions of its launches / their summed device time (CUDA events around every launch)
+        # dominant kernel of a step = the one with the larger summed device time (CUDA events around every launch; the ncu launch
+        # list profiles/r2_launches_c5.md agrees on its share): algorithmic instructions of its launches / that time
         dom_ms, dom_ev, dom_name = (tail_ms, ev_tail, "tail_kernel") if tail_ms >= sim_ms - tail_ms else (sim_ms - tail_ms, ev - ev_tail, "simulate_kernel")
         achieved = dom_ev * I_EVENT[name] / max(dom_ms * 1e-3, 1e-12)
         int_meas = {k: ns.int_peak(i, 2048)[0] for i, k in enumerate(("hash_round_mix", "imad_only", "alu_only"))}
+        # the measured peak that binds for this instruction mix: the hash round (IMAD.WIDE on the FMA pipe + LOP3 on the ALU pipe,
+        # about 40 % of the path's instructions are multiplies) -- below the issue-slot peak because IMAD.WIDE is not full rate
+        peak_meas = int_meas["hash_round_mix"]
+        traffic, traffic_src = profile_traffic(dom_name, name, args.sampler)
         # MODE-T: the saturated workload (dedup off, every lineage advanced 200 events): where the ALU roofline is meaningful
         rt = sc.simulate_raw(seed, cfg["nu"], d_mask, n_s, ns.make_params(dedup=False, max_steps=200))
         mode_t = rt.n_events_raw / (rt.ms_simulate * 1e-3)
+        sat_evs = (ev - ev_tail) / max((sim_ms - tail_ms) * 1e-3, 1e-9)
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": args.warmup, "ms_per_step": ms / K,
                 "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int64", "data": "synthetic",
+                "value_kind": value_kind, "raw_events_per_s": raw_value,
                 "config": {"workload": cfg["name"], "event_time_sampler": args.sampler, "n_lineages": int(res.n_lineages), "nu": cfg["nu"], "mode": "MODE-S (dedup on, to completion)",
                            "l2": "256 MiB flush write between steps", "parallelism": "replicas x%d" % world},
                 "clocks": clocks,
-                "e2e": {"value": e2e_ev_all / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms / K,
+                "e2e": {"value": (uniq * K if uniq else e2e_ev_all) / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms / K,
                         "h2d_bytes_per_step": int(0 if h_mask is None else h_mask.nbytes),
                         "d2h_bytes_per_step": int(res_h.richness * 32 + res_h.n_lineages * 4)},
                 "gpu_launches": int(launches),
                 "individuals_per_s": world * res.n_lineages / (ms / K * 1e-3),
                 "richness": int(res.richness), "epochs_per_step": epochs / K, "raw_events_per_step": ev / K,
-                "unique_events": unique_events(cfg, args), "redundancy": (ev / K) / unique_events(cfg, args) if unique_events(cfg, args) else None,
-                "phases": {"saturated": {"events_per_s": (ev - ev_tail) / max((sim_ms - tail_ms) * 1e-3, 1e-9), "ms_per_step": (sim_ms - tail_ms) / K,
-                                         "events_per_step": (ev - ev_tail) / K, "kernel": "simulate_kernel (one lineage per lane)"},
+                "unique_events": uniq, "redundancy": (ev / K) / uniq if uniq else None,
+                "phases": {"saturated": {"events_per_s": sat_evs, "ms_per_step": (sim_ms - tail_ms) / K,
+                                         "events_per_step": (ev - ev_tail) / K, "kernel": "simulate_kernel (one lineage per lane)",
+                                         "roofline_frac": sat_evs * I_EVENT[name] / peak},
                            "tail": {"events_per_s": ev_tail / max(tail_ms * 1e-3, 1e-9), "ms_per_step": tail_ms / K, "events_per_step": ev_tail / K,
+                                    "exact_rounds_per_event": int(res.n_tail_rounds_exact) / max(int(res.n_events_tail), 1),
                                     "kernel": "tail_kernel (one lineage per warp; bound by event latency x chain length, DESIGN.md 6.3)"}},
                 "roofline": {"bound": "alu", "kernel": dom_name + " (all its launches of the timed steps)", "achieved": achieved / 1e12, "peak": peak / 1e12,
                              "unit": "Tinstr/s", "frac": achieved / peak,
-                             # dram__bytes_read.sum + dram__bytes_write.sum of one tail_kernel launch (C5, exponential sampler, 13th tail
-                             # epoch, 50 ms), ncu --set full, profiles/r1_ncu_tail_kernel_c5.md; caches are flushed per ncu replay pass,
-                             # so this is an upper bound
-                             "traffic": 6885399296 if (name == "c5" and dom_name == "tail_kernel" and args.sampler == "exp") else None,
-                             "instr_per_event": I_EVENT[name],
+                             "peak_measured": peak_meas / 1e12, "frac_measured": achieved / peak_meas,
+                             "binding_pipe": "FMA pipe for the multiplies (IMAD.WIDE.U32, not full rate) with the ALU pipe beside it: the measured "
+                                             "hash-round mix is the ceiling of this instruction mix; `peak` is the issue-slot bound above it",
+                             "traffic": traffic, "traffic_source": traffic_src,
+                             "instr_per_event": I_EVENT[name], "instr_per_event_filtered": I_EVENT_FILTERED[name],
+                             "frac_filtered_count": dom_ev * I_EVENT_FILTERED[name] / max(dom_ms * 1e-3, 1e-12) / peak,
+                             "instr_per_event_check": "profiles/r2_sass_mix_simulate_kernel_c5.md (executed instructions per event by pipe, ncu source counters)",
                              "note": "latency-bound by construction: one lineage per warp walks a serial chain of ~ln(S)/nu events (DESIGN.md 6.3)",
-                             "peak_source": "derived: SMs x 4 schedulers x 32 lanes x sm_max_mhz (DESIGN.md section 6)",
+                             "peak_source": "derived: SMs x 4 schedulers x 32 lanes x sm_max_mhz (DESIGN.md section 6); peak_measured: necsim_debug_int_peak in this run",
                              "measured_int_peaks_Tinstr_s": {k: v / 1e12 for k, v in int_meas.items()}},
                 "mode_t": {"value": mode_t, "unit": UNIT, "what": "dedup off, 200 events per lineage, saturated machine",
-                           "roofline_frac": mode_t * I_EVENT[name] / peak,
-                           "ncu": "profiles/r1_ncu_simulate_kernel_c5_modeT.md (exponential sampler): issue slots 70 % active, ALU pipe 66 %, "
-                                  "FMA pipe 18 % of peak, 22.1 of 32 lanes per instruction, L2 hit 98.6 %"}}
+                           "roofline_frac": mode_t * I_EVENT[name] / peak, "frac_measured": mode_t * I_EVENT[name] / peak_meas,
+                           "frac_filtered_count": mode_t * I_EVENT_FILTERED[name] / peak,
+                           "ncu": "profiles/r2_ncu_simulate_kernel_c5_modeT.md"}}
         if args.event_stream:
             # the same step with every executed event recorded, sorted by time and deduplicated per epoch on the device
             pr = ns.make_params(record_events=True, event_ring_capacity=1 << min(args.event_stream, 28), event_stream_capacity=1 << args.event_stream)

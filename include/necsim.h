@@ -171,6 +171,8 @@ int necsim_simulate_workspace_size(const necsim_scenario *scn, uint64_t n_sample
  *   bytes : size of d_workspace, at least what necsim_simulate_workspace_size returned for the same params.
  * Asynchronous on the stream except for one small read-back per epoch; returns after the final
  * read-back. Pointers in *out point into d_workspace and stay valid until it is reused.
+ * One call at a time per scenario handle: the handle owns the pinned read-back block and the timing events of a call
+ * (concurrent simulations need one handle each; the scenario workspace may be shared, it is read-only after creation).
  */
 int necsim_simulate(necsim_scenario *scn, uint64_t seed, double nu, const uint8_t *d_sample_mask /*DEVICE or NULL*/,
                     uint64_t n_sampled_capacity, const necsim_sim_params *params /*HOST or NULL*/, void *d_workspace /*DEVICE*/,

@@ -274,6 +274,9 @@ typedef struct orc_scenario {
     double delta_t;
     int sampler;         /* 0 exponential (2.4), 1 Poisson / order statistics (2.7) */
     u64 *PC; u32 *thin;  /* Poisson: cdf thresholds of mu_max; per-cell thinning threshold */
+    /* temporally varying habitat: era e holds for interval indices k in [era_start[e], era_start[e+1]); era 0 = the
+     * present. With eras, `deme` / `prefix` are those of the OLDEST (largest) map: indexed locations are canonical on it. */
+    u32 n_eras; u32 *era_deme; u32 *era_start; u32 *prefix0; u32 *deme0;
     double mu_max; double *lam; /* lambda per cell (as given) */
 } orc_scenario;
 
@@ -282,6 +285,7 @@ static void set_err(char *err, int errlen, const char *msg) { if (err && errlen 
 void orc_scenario_destroy(orc_scenario *sc) {
     if (!sc) return;
     free(sc->deme); free(sc->prefix); free(sc->Cm); free(sc->sh); free(sc->thresh); free(sc->alias); free(sc->TG); free(sc->PC); free(sc->thin); free(sc->lam);
+    free(sc->era_deme); free(sc->era_start); free(sc->prefix0); free(sc->deme0);
     free(sc);
 }
 
@@ -345,6 +349,49 @@ orc_scenario *orc_scenario_create(int kind, u32 width, u32 height, const u32 *de
 }
 
 u64 orc_scenario_num_individuals(const orc_scenario *sc) { return sc->n_sampleable; }
+
+/* Temporally varying habitat (paper 9.3 L1498: "temporally varying landscapes, which enables simulating gradual habitat loss";
+ * DESIGN.md 2.8, reading R24). The scenario's deme map is the present (era 0); past_deme[e-1] is the map of era e >= 1, which holds
+ * for interval indices k >= past_start_k[e-1] (strictly increasing, > 0). Habitat is only lost towards the present: every era's map
+ * contains the younger one cell by cell (an individual of a younger era has a place in every older one). Indexed locations become
+ * canonical on the oldest map; the sample mask stays over the present-day individuals. EXPLICIT_GAUSSIAN only. Call before
+ * orc_scenario_set_sampler. Returns 0 or -1. */
+int orc_scenario_set_eras(orc_scenario *sc, u32 n_past, const u32 *past_deme, const u32 *past_start_k) {
+    if (sc->kind != ORC_EXPLICIT_GAUSSIAN || n_past == 0 || sc->n_eras || sc->PC) return -1;
+    u32 n = sc->ncells;
+    for (u32 e = 0; e < n_past; ++e) {
+        if (past_start_k[e] == 0 || (e > 0 && past_start_k[e] <= past_start_k[e - 1])) return -1;
+        const u32 *older = past_deme + (size_t)e * n, *younger = e ? past_deme + (size_t)(e - 1) * n : sc->deme;
+        for (u32 c = 0; c < n; ++c) if (older[c] < younger[c]) return -1;
+    }
+    const u32 *oldest = past_deme + (size_t)(n_past - 1) * n;
+    u64 tot = 0;
+    for (u32 c = 0; c < n; ++c) tot += oldest[c];
+    if (tot >= (1ull << 32)) return -1;
+    for (u32 c = 0; c < n; ++c)     /* turnover scale wherever any era has habitat */
+        if (oldest[c] > 0 && sc->deme[c] == 0 && orc_turnover_scale(sc->lam[c], sc->delta_t, &sc->Cm[c], &sc->sh[c]) != 0) return -1;
+    sc->n_eras = n_past + 1;
+    sc->era_deme = (u32 *)malloc(sizeof(u32) * (size_t)sc->n_eras * n);
+    sc->era_start = (u32 *)malloc(sizeof(u32) * sc->n_eras);
+    memcpy(sc->era_deme, sc->deme, sizeof(u32) * n);
+    memcpy(sc->era_deme + n, past_deme, sizeof(u32) * (size_t)n_past * n);
+    sc->era_start[0] = 0;
+    for (u32 e = 0; e < n_past; ++e) sc->era_start[e + 1] = past_start_k[e];
+    sc->deme0 = sc->deme; sc->prefix0 = sc->prefix;
+    sc->deme = (u32 *)malloc(sizeof(u32) * n); sc->prefix = (u32 *)malloc(sizeof(u32) * ((size_t)n + 1));
+    tot = 0;
+    for (u32 c = 0; c < n; ++c) { sc->deme[c] = oldest[c]; sc->prefix[c] = (u32)tot; tot += oldest[c]; }
+    sc->prefix[n] = (u32)tot;
+    sc->n_locations = tot;           /* n_sampleable stays the present-day population */
+    return 0;
+}
+/* deme map in force during interval k */
+static const u32 *deme_at(const orc_scenario *sc, u32 k) {
+    if (!sc->n_eras) return sc->deme;
+    u32 e = 0;
+    while (e + 1 < sc->n_eras && sc->era_start[e + 1] <= k) ++e;
+    return sc->era_deme + (size_t)e * sc->ncells;
+}
 /* chooses the event-time sampler (DESIGN.md 2.4 / 2.7). Results depend on it: same law, different realisation. */
 int orc_scenario_set_sampler(orc_scenario *sc, int sampler) {
     if (sampler != 0 && sampler != 1) return -1;
@@ -379,7 +426,7 @@ static int bern(u64 x, u64 thr) { return (x >> 11) < thr; }
 u64 orc_thr(double p) { return (u64)floor(ldexp(p, 53)); }
 
 /* DESIGN.md 2.5 step 2. Returns 0 and the new (loc, cell), or -4 if resampling is exhausted. */
-static int disperse(const orc_scenario *sc, u64 thr_m, u64 s, u32 j, u32 cell, u32 *loc2, u32 *cell2, u64 *resamples) {
+static int disperse(const orc_scenario *sc, u64 thr_m, u64 s, u32 k, u32 j, u32 cell, u32 *loc2, u32 *cell2, u64 *resamples) {
     switch (sc->kind) {
     case ORC_NONSPATIAL:
         *loc2 = (u32)mulhi64(orc_draw_disp(s, j, 0), sc->n_locations); *cell2 = 0; return 0;
@@ -396,6 +443,7 @@ static int disperse(const orc_scenario *sc, u64 thr_m, u64 s, u32 j, u32 cell, u
         u32 idx = (d == 1) ? 0 : (u32)mulhi64(orc_draw_index(s, j), d);
         *cell2 = c2; *loc2 = sc->prefix[c2] + idx; return 0; }
     case ORC_EXPLICIT_GAUSSIAN: {
+        const u32 *deme_k = deme_at(sc, k);   /* the parent lived in the habitat of the event's time (L774, L1498) */
         u32 x0 = cell % sc->width, y0 = cell / sc->width;
         for (u32 r = 0; r < (1u << 20); ++r) {
             u64 x = orc_draw_disp(s, j, r);
@@ -404,7 +452,7 @@ static int disperse(const orc_scenario *sc, u64 thr_m, u64 s, u32 j, u32 cell, u
             i64 xx = ((i64)x0 + dx) % (i64)sc->width;  if (xx < 0) xx += sc->width;
             i64 yy = ((i64)y0 + dy) % (i64)sc->height; if (yy < 0) yy += sc->height;
             u32 c2 = (u32)yy * sc->width + (u32)xx;
-            u32 d = sc->deme[c2];
+            u32 d = deme_k[c2];
             if (d > 0) {
                 u32 idx = (d == 1) ? 0 : (u32)mulhi64(orc_draw_index(s, j), d);
                 *cell2 = c2; *loc2 = sc->prefix[c2] + idx; return 0;
@@ -422,7 +470,7 @@ int orc_debug_disperse(const orc_scenario *sc, u64 seed, double migration_unused
     u32 K[6]; orc_key_schedule(seed, K);
     u32 cell = (sc->kind == ORC_SPATIALLY_IMPLICIT) ? (loc >= sc->J_local) : cell_of_loc(sc, loc);
     u32 c2; u64 rs = 0;
-    return disperse(sc, orc_thr(sc->migration), orc_prime(K, loc, k), j, cell, loc2, &c2, &rs);
+    return disperse(sc, orc_thr(sc->migration), orc_prime(K, loc, k), k, j, cell, loc2, &c2, &rs);
 }
 
 /* ------------------------------------------------------------------------------------------- */
@@ -521,8 +569,14 @@ int orc_simulate(const orc_scenario *sc, u64 seed, double nu, const uint8_t *mas
     orc_event_key *term = (orc_event_key *)calloc(ns, sizeof(orc_event_key));
     u64 n = 0;
     for (u64 i = 0; i < sc->n_sampleable; ++i) if (!mask || mask[i]) {
-        loc[n] = (u32)i;
-        cell[n] = (sc->kind == ORC_SPATIALLY_IMPLICIT) ? 0 : cell_of_loc(sc, (u32)i);
+        if (sc->n_eras) {   /* i counts the present-day individuals; locations are canonical on the oldest map */
+            u32 lo = 0, hi = sc->ncells;
+            while (hi - lo > 1) { u32 mid = lo + (hi - lo) / 2; if (sc->prefix0[mid] <= (u32)i) lo = mid; else hi = mid; }
+            cell[n] = lo; loc[n] = sc->prefix[lo] + ((u32)i - sc->prefix0[lo]);
+        } else {
+            loc[n] = (u32)i;
+            cell[n] = (sc->kind == ORC_SPATIALLY_IMPLICIT) ? 0 : cell_of_loc(sc, (u32)i);
+        }
         if (sc->deme[cell[n]] == 0) { n = 0; break; }
         kk[n] = 0; ff[n] = -1; parent[n] = 0xFFFFFFFFu; ++n;
     }
@@ -571,7 +625,7 @@ int orc_simulate(const orc_scenario *sc, u64 seed, double nu, const uint8_t *mas
                     break;
                 }
                 u32 l2, c2;
-                r = disperse(sc, thr_m, s, j, c, &l2, &c2, &stats->resample_attempts);
+                r = disperse(sc, thr_m, s, kk[id], j, c, &l2, &c2, &stats->resample_attempts);
                 if (r != 0) { rc = r; break; }
                 sink_event(loc[id], kk[id], j, T, l2);
                 loc[id] = l2; cell[id] = c2;

@@ -116,7 +116,7 @@ class Scenario:
     """Mirror of the paper's scenario = habitat + turnover + dispersal (+ sizes)."""
 
     def __init__(self, kind, width=1, height=1, deme=None, uniform_deme=0, turnover=None, uniform_turnover=1.0,
-                 matrix=None, sigma=0.0, local_size=0, meta_size=0, migration=0.0, delta_t=2.0, sampler=0):
+                 matrix=None, sigma=0.0, local_size=0, meta_size=0, migration=0.0, delta_t=2.0, sampler=0, past_deme=None, past_start_k=None):
         self.kind = kind
         d = None if deme is None else np.ascontiguousarray(deme, dtype=np.uint32).ravel()
         t = None if turnover is None else np.ascontiguousarray(turnover, dtype=np.float64).ravel()
@@ -128,6 +128,13 @@ class Scenario:
         if not self._h:
             raise ValueError("oracle scenario: " + err.value.decode())
         L = lib(); L.orc_scenario_set_sampler.restype = C.c_int; L.orc_scenario_set_sampler.argtypes = [C.c_void_p, C.c_int]
+        if past_deme is not None:   # temporally varying habitat: eras 1.. of the past
+            pd = np.ascontiguousarray(past_deme, dtype=np.uint32).reshape(-1, width * height)
+            ps = np.ascontiguousarray(past_start_k, dtype=np.uint32).ravel()
+            assert len(ps) == pd.shape[0]
+            L.orc_scenario_set_eras.restype = C.c_int; L.orc_scenario_set_eras.argtypes = [C.c_void_p, C.c_uint32, C.c_void_p, C.c_void_p]
+            if L.orc_scenario_set_eras(self._h, pd.shape[0], _ptr(pd), _ptr(ps)) != 0:
+                raise ValueError("oracle scenario: bad eras (gaussian kind only, start_k increasing, habitat only lost towards the present)")
         if L.orc_scenario_set_sampler(self._h, int(sampler)) != 0:
             raise ValueError("oracle scenario: unknown sampler")
         self.sampler = int(sampler)

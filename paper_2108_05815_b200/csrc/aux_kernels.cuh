@@ -203,6 +203,14 @@ __global__ void __launch_bounds__(256) unique_write_kernel(const SimBuffers bf, 
         events[e] = ev;
     }
 }
+// pointer jumping over the "culled at an event another lineage executed" links: parent <- grandparent where the parent was culled
+// too. Every value a racing thread can read here is an ancestor, so the links stay a forest; k rounds divide the depth by 2^k.
+__global__ void __launch_bounds__(256) parent_jump_kernel(const SimBuffers bf, u32 n) {
+    u32 i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n || bf.state[i] != 2) return;
+    const u32 p = bf.parent[i];
+    if (bf.state[p] == 2) bf.parent[i] = bf.parent[p];
+}
 // resolve + label: follow the "culled at an event another lineage executed" links to a lineage that
 // ended by itself (links point to earlier arrivals at one event and time increases along a lineage: a forest)
 __global__ void __launch_bounds__(256) label_kernel(const SimBuffers bf, u32 n, const u32 *__restrict__ species_of, necsim_event *__restrict__ events,

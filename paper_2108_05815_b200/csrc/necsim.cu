@@ -8,6 +8,7 @@
 #include <string.h>
 #include <stdlib.h>
 #include <string>
+#include <new>
 #include <vector>
 #include <algorithm>
 
@@ -186,7 +187,17 @@ static int upload_neglog_tables(cudaStream_t st) {
     return NECSIM_OK;
 }
 
+// no exception crosses the C ABI: host-side allocations (the ncells^2 alias table of EXPLICIT_MATRIX ...) may throw
+#define NS_GUARDED(call, on_fail)                                                                        \
+    try { return (call); }                                                                               \
+    catch (const std::bad_alloc &) { on_fail; return fail(NECSIM_ERR_CAPACITY, "out of host memory"); }   \
+    catch (...) { on_fail; return fail(NECSIM_ERR_INVALID_ARG, "unexpected host exception"); }
+
+static int create_scenario_impl(const necsim_scenario_desc *d, void *d_workspace, size_t bytes, void *cuda_stream, necsim_scenario **out);
 extern "C" int necsim_create_scenario(const necsim_scenario_desc *d, void *d_workspace, size_t bytes, void *cuda_stream, necsim_scenario **out) {
+    NS_GUARDED(create_scenario_impl(d, d_workspace, bytes, cuda_stream, out), if (out) *out = NULL)
+}
+static int create_scenario_impl(const necsim_scenario_desc *d, void *d_workspace, size_t bytes, void *cuda_stream, necsim_scenario **out) {
     if (!out) return fail(NECSIM_ERR_INVALID_ARG, "out is NULL");
     *out = NULL;
     ScenarioLayout L;
@@ -335,8 +346,14 @@ extern "C" int necsim_create_scenario(const necsim_scenario_desc *d, void *d_wor
     necsim_scenario *h = new necsim_scenario();
     h->dev = sd; h->mu_max = mu_max; h->migration = (d->kind == NECSIM_SPATIALLY_IMPLICIT) ? d->migration : 0.0; h->n_individuals = sd.n_sampleable; h->ws_bytes = L.total; h->sm_count = sm_count;
     h->h_ctr = NULL; h->tables_uploaded = true;
+    for (int i = 0; i < 4; ++i) h->ev[i] = NULL;
     if (cudaHostAlloc((void **)&h->h_ctr, sizeof(SimCounters), cudaHostAllocDefault) != cudaSuccess) { delete h; return fail(NECSIM_ERR_CUDA, "cudaHostAlloc failed"); }
-    for (int i = 0; i < 4; ++i) if (cudaEventCreate(&h->ev[i]) != cudaSuccess) { delete h; return fail(NECSIM_ERR_CUDA, "cudaEventCreate failed"); }
+    for (int i = 0; i < 4; ++i)
+        if (cudaEventCreate(&h->ev[i]) != cudaSuccess) {   // free what exists: the pinned block and the events made so far
+            h->ev[i] = NULL;
+            necsim_destroy(h);
+            return fail(NECSIM_ERR_CUDA, "cudaEventCreate failed");
+        }
     *out = h;
     return NECSIM_OK;
 }
@@ -350,7 +367,7 @@ extern "C" int necsim_scenario_num_individuals(const necsim_scenario *scn, uint6
 extern "C" int necsim_destroy(necsim_scenario *scn) {
     if (!scn) return NECSIM_OK;
     if (scn->h_ctr) cudaFreeHost(scn->h_ctr);
-    for (int i = 0; i < 4; ++i) cudaEventDestroy(scn->ev[i]);
+    for (int i = 0; i < 4; ++i) if (scn->ev[i]) cudaEventDestroy(scn->ev[i]);
     delete scn;
     return NECSIM_OK;
 }
@@ -702,6 +719,11 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
         n_launch += 3;
         CU(cudaGetLastError());
     }
+    // six rounds of pointer jumping bound the walk of label_kernel to 1/64 of the longest chain of links
+    if (rp.dedup && hc->n_culled > 0) {
+        for (int r = 0; r < 6; ++r) parent_jump_kernel<<<(n_sampled + 255) / 256, 256, 0, st>>>(bf, n_sampled);
+        n_launch += 6;
+    }
     label_kernel<<<(n_sampled + 255) / 256, 256, 0, st>>>(bf, n_sampled, species_of, events, labels);
     n_launch += 1;
     CU(cudaGetLastError());
@@ -758,13 +780,13 @@ static int simulate_checked(necsim_scenario *scn, uint64_t seed, double nu, cons
 
 extern "C" int necsim_simulate(necsim_scenario *scn, uint64_t seed, double nu, const uint8_t *d_sample_mask, uint64_t n_sampled_capacity,
                                const necsim_sim_params *params, void *d_workspace, size_t bytes, void *cuda_stream, necsim_result *out) {
-    return simulate_checked(scn, seed, nu, d_sample_mask, false, n_sampled_capacity, params, d_workspace, bytes, cuda_stream, out, NULL, NULL);
+    NS_GUARDED(simulate_checked(scn, seed, nu, d_sample_mask, false, n_sampled_capacity, params, d_workspace, bytes, cuda_stream, out, NULL, NULL), (void)0)
 }
 
 extern "C" int necsim_simulate_host(necsim_scenario *scn, uint64_t seed, double nu, const uint8_t *h_sample_mask, uint64_t n_sampled_capacity,
                                     const necsim_sim_params *params, void *d_workspace, size_t bytes, void *cuda_stream, necsim_result *out,
                                     necsim_event *h_events, uint32_t *h_labels) {
-    return simulate_checked(scn, seed, nu, h_sample_mask, true, n_sampled_capacity, params, d_workspace, bytes, cuda_stream, out, h_events, h_labels);
+    NS_GUARDED(simulate_checked(scn, seed, nu, h_sample_mask, true, n_sampled_capacity, params, d_workspace, bytes, cuda_stream, out, h_events, h_labels), (void)0)
 }
 
 // ---------------------------------------------------------------------------------------------------

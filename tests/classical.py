@@ -53,3 +53,42 @@ def sad_of(labels):
     """species-abundance distribution: counts of species having abundance a (index a)."""
     _, counts = np.unique(labels, return_counts=True)
     return np.bincount(counts)
+
+
+def simulate_classical_timed(rng, start_locs, nu, disperse_at, rate=1.0):
+    """The same coalescence with the global clock simulated (uniform turnover `rate`): the n active lineages have events at total rate
+    n * rate, so the time to the next event is Exp(n * rate). disperse_at(rng, loc, t) -> parent location
+    for an event at time t (generations before the present): the landscape may depend on time (temporally varying habitat, L1498)."""
+    n = len(start_locs)
+    loc = list(start_locs)
+    active = list(range(n))
+    occupant = {l: i for i, l in enumerate(loc)}
+    parent = list(range(n))
+    species = [-1] * n
+    next_species = 0
+    t = 0.0
+    while active:
+        t += rng.exponential(1.0 / (rate * len(active)))
+        a = int(rng.integers(len(active)))
+        i = active[a]
+        if rng.random() < nu:
+            species[i] = next_species; next_species += 1
+            del occupant[loc[i]]
+            active[a] = active[-1]; active.pop()
+            continue
+        new = disperse_at(rng, loc[i], t)
+        if new == loc[i]:
+            continue
+        del occupant[loc[i]]
+        if new in occupant:
+            parent[i] = occupant[new]
+            active[a] = active[-1]; active.pop()
+        else:
+            loc[i] = new; occupant[new] = i
+    out = []
+    for i in range(n):
+        r = i
+        while species[r] < 0:
+            r = parent[r]
+        out.append(species[r])
+    return out
