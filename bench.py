@@ -29,14 +29,14 @@ from paper_2108_05815_b200 import dist as D    # noqa: E402
 
 METRIC = "lineage_events_per_s"
 UNIT = "events/s"
-MAKERS = dict(c1=I.c1_nonspatial, c2=I.c2_implicit, c3=I.c3_matrix, c4=I.c4_gaussian, c5=I.c5_stress, c6=I.c6_bigdeme)
+MAKERS = dict(c1=I.c1_nonspatial, c2=I.c2_implicit, c3=I.c3_matrix, c4=I.c4_gaussian, c5=I.c5_stress, c6=I.c6_bigdeme, c7=I.c7_habitat_loss)
 SMALL = dict(zip(("c1", "c2", "c3", "c4", "c5"), range(5)))
 # Algorithmic integer instructions per executed event (minimal 32-bit instruction sequence of
 # each primitive, weighted by the expected number of draws per event at mu = 2 and the measured attempts per event).
-I_EVENT = dict(c1=230, c2=232, c3=252, c4=263, c5=272, c6=259)   # c6: one attempt + 5 % resampling, index draw, deme32 gather
+I_EVENT = dict(c1=230, c2=232, c3=252, c4=263, c5=272, c6=259, c7=272)   # c6: one attempt + 5 % resampling, index draw, deme32 gather; c7 = c5's landscape with eras
 # The same count when the event-time search is decided by the binary32 filter (a time draw is then hash 12 +
 # advance 2 + lg2 / scale 4 + accumulate and compare 5 = 23 instead of 68): what the kernels must issue at the least.
-I_EVENT_FILTERED = dict(c1=118, c2=120, c3=140, c4=151, c5=160, c6=147)
+I_EVENT_FILTERED = dict(c1=118, c2=120, c3=140, c4=151, c5=160, c6=147, c7=160)
 # issue-slot peak: 148 SMs x 4 schedulers x 32 lanes x 1 instr/clk x sm_max_mhz (B300_MICROARCH "Pipe rates")
 def alu_peak(sm_count, sm_mhz):
     return sm_count * 4 * 32 * sm_mhz * 1e6
@@ -59,6 +59,8 @@ def profile_traffic(kernel, name, sampler):
 def make_cfg(name, small):
     if name == "c6":                                     # SURVEY NEXT-4 shape; --small: demes of ~360
         return I.c6_bigdeme(deme_mean=360, sample=0.05) if small else I.c6_bigdeme()
+    if name == "c7":                                     # temporally varying habitat
+        return I.c7_habitat_loss(side=128, blur_radius=4.0, nu=1e-3, sample=0.3, switch_k=40) if small else I.c7_habitat_loss()
     return I.small_configs()[SMALL[name]] if small else MAKERS[name]()
 
 
@@ -124,8 +126,11 @@ def unique_events(cfg, args):
     f = os.path.join(ROOT, "tests", "golden", "full_configs_poisson.json" if args.sampler == "poisson" else "full_configs.json")
     if args.small or not os.path.exists(f):
         return None
-    extra = os.path.join(ROOT, "tests", "golden", "full_config_c6.json")
-    records = json.load(open(f)) + (json.load(open(extra)) if (args.sampler == "exp" and os.path.exists(extra)) else [])
+    records = json.load(open(f))
+    for extra in ("full_config_c6.json", "full_config_c7.json"):
+        e = os.path.join(ROOT, "tests", "golden", extra)
+        if args.sampler == "exp" and os.path.exists(e):
+            records += json.load(open(e))
     for g in records:
         if g["name"] == cfg["name"]:
             return g["unique_events"]

@@ -61,6 +61,14 @@ typedef struct necsim_scenario_desc {
     uint64_t meta_size;       /* SPATIALLY_IMPLICIT: J_meta */
     double migration;         /* SPATIALLY_IMPLICIT: m in [0,1] */
     double delta_t;           /* repriming interval; 1/256 < lambda*delta_t <= 64 */
+    /* Temporally varying habitat, EXPLICIT_GAUSSIAN only. `deme` is the present (era 0);
+     * past_deme[e-1] (HOST [n_past_eras][width*height], n_past_eras <= 3) is the deme map of era e >= 1, in force for interval
+     * indices k >= past_start_k[e-1] (HOST [n_past_eras], strictly increasing, > 0). Habitat is only lost towards the present:
+     * every era's map contains the younger one cell by cell, else NECSIM_ERR_INVALID_ARG. Indexed locations (in events and the
+     * event stream) are then canonical on the OLDEST map; the sample mask ranges over the present-day individuals. 0 = static. */
+    uint32_t n_past_eras;
+    const uint32_t *past_deme;
+    const uint32_t *past_start_k;
 } necsim_scenario_desc;
 
 /*

@@ -15,6 +15,14 @@ __device__ __forceinline__ u32 queue_cell(const ScenarioDev &sc, u32 loc) {
     return sc.kind == 3 ? pack_xy(sc, c) : c;
 }
 
+// temporally varying habitat: the i-th present-day individual sits at (cell, i') of the present map; its indexed
+// location is canonical on the oldest map: prefix[cell] + i'
+__device__ __forceinline__ u32 era_start_loc(const ScenarioDev &sc, u32 i) {
+    u32 lo = 0, hi = sc.ncells;                      // invariant: prefix0[lo] <= i < prefix0[hi]
+    while (hi - lo > 1) { u32 mid = lo + ((hi - lo) >> 1); if (sc.prefix0[mid] <= i) lo = mid; else hi = mid; }
+    return sc.prefix[lo] + (i - sc.prefix0[lo]);
+}
+
 // S0, pass 1: number of sampled individuals per chunk
 __global__ void __launch_bounds__(256) mask_count_kernel(const uint8_t *__restrict__ mask, u64 n, u32 *__restrict__ chunk_count) {
     __shared__ u32 wsum[8];
@@ -103,6 +111,7 @@ __global__ void __launch_bounds__(256) mask_scatter_kernel(const ScenarioDev sc,
     while (bits) {
         u32 t = __ffs(bits) - 1; bits &= bits - 1;
         u32 loc = (u32)(base + t);
+        if (sc.n_eras) loc = era_start_loc(sc, loc);
         if (off < capacity) queue[off] = make_uint4(off, loc, queue_cell(sc, loc), 0u);
         ++off;
     }
@@ -111,7 +120,7 @@ __global__ void __launch_bounds__(256) mask_scatter_kernel(const ScenarioDev sc,
 // S0 without a mask: everyone is sampled
 __global__ void __launch_bounds__(256) all_sampled_kernel(const ScenarioDev sc, u32 n, uint4 *__restrict__ queue) {
     u32 i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) queue[i] = make_uint4(i, i, queue_cell(sc, i), 0u);
+    if (i < n) { const u32 loc = sc.n_eras ? era_start_loc(sc, i) : i; queue[i] = make_uint4(i, loc, queue_cell(sc, loc), 0u); }
 }
 
 // ---- S6 ------------------------------------------------------------------------------------------

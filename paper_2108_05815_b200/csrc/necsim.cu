@@ -109,13 +109,61 @@ struct necsim_scenario {
 };
 
 struct ScenarioLayout {
-    size_t off_hab8, off_deme32, off_prefix, off_pois, off_thin, off_scale, off_alias, off_gauss, off_hab64, total;
+    size_t off_hab8, off_deme32, off_prefix, off_pois, off_thin, off_scale, off_alias, off_gauss, off_hab64, off_era_hab8, off_era_deme32, off_prefix0, total;
+    u32 n_eras;
     u32 ncells, gauss_len, nbx, compact_deme;
     int R;
     bool uniform_deme, need_deme32, per_cell_turnover, compact;
 };
 
+// Temporally varying habitat: the per-cell tables are built for the OLDEST map (locations are canonical on it);
+// `eff` is the caller's description with that map as its deme map.
+struct EraView {
+    necsim_scenario_desc eff;
+    u32 n_eras;                       // 0 = static
+    const u32 *maps[4];               // maps[0] = the present ... maps[n_eras - 1] = the oldest
+    u32 start[4];
+    std::vector<u32> present;         // the present map when the caller gave uniform_deme only
+};
+static int era_view(const necsim_scenario_desc *d, EraView &v) {
+    v.eff = *d; v.n_eras = 0;
+    for (int e = 0; e < 4; ++e) { v.maps[e] = NULL; v.start[e] = 0xFFFFFFFFu; }
+    if (!d->n_past_eras) return NECSIM_OK;
+    if (d->kind != NECSIM_EXPLICIT_GAUSSIAN) return fail(NECSIM_ERR_UNSUPPORTED, "temporally varying habitat: EXPLICIT_GAUSSIAN only");
+    if (d->n_past_eras > 3 || !d->past_deme || !d->past_start_k) return fail(NECSIM_ERR_INVALID_ARG, "eras: at most 3 past eras, with their maps and start intervals");
+    if (d->width == 0 || d->height == 0 || (u64)d->width * d->height >= (1ull << 32)) return fail(NECSIM_ERR_INVALID_ARG, "bad width/height");
+    const size_t n = (size_t)d->width * d->height;
+    if (d->deme) v.maps[0] = d->deme;
+    else { v.present.assign(n, d->uniform_deme); v.maps[0] = v.present.data(); }
+    v.start[0] = 0;
+    for (u32 e = 1; e <= d->n_past_eras; ++e) {
+        v.maps[e] = d->past_deme + (size_t)(e - 1) * n; v.start[e] = d->past_start_k[e - 1];
+        if (v.start[e] == 0 || (e > 1 && v.start[e] <= v.start[e - 1])) return fail(NECSIM_ERR_INVALID_ARG, "eras: past_start_k must be > 0 and strictly increasing");
+        for (size_t c = 0; c < n; ++c)
+            if (v.maps[e][c] < v.maps[e - 1][c]) return fail(NECSIM_ERR_INVALID_ARG, "eras: habitat may only be lost towards the present (an older map must contain the younger one)");
+    }
+    v.n_eras = d->n_past_eras + 1;
+    v.eff.deme = v.maps[v.n_eras - 1]; v.eff.n_past_eras = 0; v.eff.past_deme = NULL; v.eff.past_start_k = NULL;
+    return NECSIM_OK;
+}
+
+static int scenario_layout_static(const necsim_scenario_desc *d, ScenarioLayout &L, bool allow_compact);
 static int scenario_layout(const necsim_scenario_desc *d, ScenarioLayout &L) {
+    if (!d) return fail(NECSIM_ERR_INVALID_ARG, "desc is NULL");
+    EraView v;
+    int rc = era_view(d, v);
+    if (rc) return rc;
+    rc = scenario_layout_static(&v.eff, L, v.n_eras == 0);
+    if (rc || !v.n_eras) return rc;
+    size_t off = L.total;
+    L.n_eras = v.n_eras;
+    L.off_era_hab8 = off; off = align256(off + (size_t)v.n_eras * L.ncells);
+    if (L.need_deme32) { L.off_era_deme32 = off; off = align256(off + 4 * (size_t)v.n_eras * L.ncells); }
+    L.off_prefix0 = off; off = align256(off + 4 * ((size_t)L.ncells + 1));
+    L.total = off;
+    return NECSIM_OK;
+}
+static int scenario_layout_static(const necsim_scenario_desc *d, ScenarioLayout &L, bool allow_compact) {
     if (!d) return fail(NECSIM_ERR_INVALID_ARG, "desc is NULL");
     memset(&L, 0, sizeof(L));
     if (d->kind < 0 || d->kind > 3) return fail(NECSIM_ERR_INVALID_ARG, "unknown scenario kind");
@@ -163,7 +211,7 @@ static int scenario_layout(const necsim_scenario_desc *d, ScenarioLayout &L) {
         u32 D = 0; bool same = true;
         if (L.uniform_deme) D = d->uniform_deme;
         else for (u32 c = 0; c < L.ncells && same; ++c) if (d->deme[c]) { if (!D) D = d->deme[c]; else same = (d->deme[c] == D); }
-        if (same && D) {
+        if (same && D && allow_compact) {
             L.compact = true; L.compact_deme = D; L.nbx = (d->width + 31u) / 32u;
             L.off_hab64 = off; off = align256(off + 8 * (size_t)L.nbx * d->height);
         }
@@ -197,12 +245,16 @@ static int create_scenario_impl(const necsim_scenario_desc *d, void *d_workspace
 extern "C" int necsim_create_scenario(const necsim_scenario_desc *d, void *d_workspace, size_t bytes, void *cuda_stream, necsim_scenario **out) {
     NS_GUARDED(create_scenario_impl(d, d_workspace, bytes, cuda_stream, out), if (out) *out = NULL)
 }
-static int create_scenario_impl(const necsim_scenario_desc *d, void *d_workspace, size_t bytes, void *cuda_stream, necsim_scenario **out) {
+static int create_scenario_impl(const necsim_scenario_desc *d_caller, void *d_workspace, size_t bytes, void *cuda_stream, necsim_scenario **out) {
     if (!out) return fail(NECSIM_ERR_INVALID_ARG, "out is NULL");
     *out = NULL;
     ScenarioLayout L;
-    int rc = scenario_layout(d, L);
+    int rc = scenario_layout(d_caller, L);
     if (rc) return rc;
+    EraView era;
+    rc = era_view(d_caller, era);
+    if (rc) return rc;
+    const necsim_scenario_desc *d = &era.eff;      // with eras: the oldest map is the deme map of every table below
     if (!d_workspace || bytes < L.total) return fail(NECSIM_ERR_WORKSPACE_TOO_SMALL, "scenario workspace too small");
     if (((uintptr_t)d_workspace & 255u) != 0) return fail(NECSIM_ERR_INVALID_ARG, "workspace must be 256-byte aligned");
     cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -312,6 +364,30 @@ static int create_scenario_impl(const necsim_scenario_desc *d, void *d_workspace
                 sd.hab64 = (const uint2 *)(base + L.off_hab64); sd.nbx = L.nbx; sd.compact_deme = L.compact_deme;
             }
         }
+    }
+    if (era.n_eras) {   // per-era habitat maps (the dispersal test of an event of era e) and the present map's prefix sums (S0)
+        std::vector<uint8_t> eh((size_t)era.n_eras * n);
+        std::vector<u32> ed, p0((size_t)n + 1);
+        if (L.need_deme32) ed.resize((size_t)era.n_eras * n);
+        for (u32 e = 0; e < era.n_eras; ++e)
+            for (u32 c = 0; c < n; ++c) {
+                eh[(size_t)e * n + c] = (uint8_t)std::min(era.maps[e][c], 255u);
+                if (L.need_deme32) ed[(size_t)e * n + c] = era.maps[e][c];
+            }
+        u64 tot0 = 0;
+        for (u32 c = 0; c < n; ++c) { p0[c] = (u32)tot0; tot0 += era.maps[0][c]; }
+        p0[n] = (u32)tot0;
+        if (tot0 == 0) return fail(NECSIM_ERR_INVALID_ARG, "eras: the present-day map has no habitat");
+        CU(cudaMemcpyAsync(base + L.off_era_hab8, eh.data(), eh.size(), cudaMemcpyHostToDevice, st));
+        if (L.need_deme32) CU(cudaMemcpyAsync(base + L.off_era_deme32, ed.data(), 4 * ed.size(), cudaMemcpyHostToDevice, st));
+        CU(cudaMemcpyAsync(base + L.off_prefix0, p0.data(), 4 * p0.size(), cudaMemcpyHostToDevice, st));
+        CU(cudaStreamSynchronize(st));
+        sd.n_eras = era.n_eras;
+        for (int e = 0; e < 4; ++e) sd.era_start[e] = era.start[e];
+        sd.era_hab8 = base + L.off_era_hab8;
+        sd.era_deme32 = L.need_deme32 ? (const u32 *)(base + L.off_era_deme32) : NULL;
+        sd.prefix0 = (const u32 *)(base + L.off_prefix0);
+        sd.n_sampleable = tot0;          // the sample mask ranges over the present-day individuals
     }
     sd.sampler = d->sampler;
     sd.margin = (float)(6.1035156e-05 * (1.0 + 1.0 / mu_min));   // NS_MARGIN * (1 + 1/mu_min)
@@ -907,7 +983,7 @@ __global__ void debug_disperse_kernel(const ScenarioDev sc, SeedKey key, u64 thr
     if (KIND == 3) cell = pack_xy(sc, cell);
     u64 X = prime(key, loc[i], k[i]) + (u64)j[i] * NS_GAMMA;
     u32 l2 = 0xFFFFFFFFu, c2 = 0, rs = 0;
-    disperse<KIND>(sc, thr_m, X, cell, l2, c2, gl, rs);
+    disperse<KIND>(sc, thr_m, X, cell, l2, c2, gl, rs, k[i]);
     loc_out[i] = l2;
 }
 

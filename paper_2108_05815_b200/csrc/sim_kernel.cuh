@@ -80,6 +80,20 @@ __device__ __forceinline__ u32 cell_deme(const ScenarioDev &sc, u32 cell) {
     return d;
 }
 __device__ __forceinline__ u32 cell_prefix(const ScenarioDev &sc, u32 cell) { return __ldg(&sc.prefix[cell]); }
+// temporally varying habitat: offset of the deme map in force during interval k inside the era tables (0 when static)
+__device__ __forceinline__ u32 era_offset(const ScenarioDev &sc, u32 k) {
+    if (!sc.n_eras) return 0u;
+    const u32 e = (k >= sc.era_start[1] ? 1u : 0u) + (k >= sc.era_start[2] ? 1u : 0u) + (k >= sc.era_start[3] ? 1u : 0u);
+    return e * sc.ncells;
+}
+// deme of a cell at interval k: the static tables, or the era's
+__device__ __forceinline__ u32 cell_deme_at(const ScenarioDev &sc, u32 cell, u32 k) {
+    if (!sc.n_eras) return cell_deme(sc, cell);
+    const u32 o = era_offset(sc, k) + cell;
+    u32 d = __ldg(&sc.era_hab8[o]);
+    if (d == 255u) d = __ldg(&sc.era_deme32[o]);
+    return d;
+}
 
 // cell of an indexed location: last cell with prefix[cell] <= loc (that cell has deme > 0)
 __device__ __forceinline__ u32 cell_of_loc(const ScenarioDev &sc, u32 loc) {
@@ -106,7 +120,7 @@ __device__ __forceinline__ u32 wrap_add(u32 x, int d, u32 size) {
 // resampling exhaustion. `resamples` counts rejected targets. KIND 3: cell / cell2 are packed (y << 16 | x).
 template <int KIND>
 __device__ __forceinline__ bool disperse(const ScenarioDev &sc, u64 thr_m, u64 X, u32 cell, u32 &loc2, u32 &cell2,
-                                         const GaussLut &gl, u32 &resamples) {
+                                         const GaussLut &gl, u32 &resamples, u32 k = 0) {
     if (KIND == 0) {  // NONSPATIAL: uniform over all J positions, self allowed (R12)
         loc2 = mulhi64_u32(draw_disp(X, 0), (u32)sc.n_locations);
         cell2 = 0;
@@ -135,7 +149,7 @@ __device__ __forceinline__ bool disperse(const ScenarioDev &sc, u64 thr_m, u64 X
             const u32 xx = wrap_add(x0, gauss_disp(gl, (u32)(x >> 32)), sc.width);
             const u32 yy = wrap_add(y0, gauss_disp(gl, (u32)x), sc.height);
             const u32 c2 = yy * sc.width + xx;
-            const u32 d = cell_deme(sc, c2);
+            const u32 d = cell_deme_at(sc, c2, k);
             if (d > 0) {
                 const u32 idx = (d == 1u) ? 0u : mulhi64_u32(draw_index(X), d);
                 cell2 = (yy << 16) | xx;
@@ -413,7 +427,7 @@ __global__ void __launch_bounds__(256) simulate_kernel(const ScenarioDev sc, con
                     d = (hb.x & bit) ? sc.compact_deme : 0u;
                     pfx = hb.y + sc.compact_deme * (u32)__popc(hb.x & (bit - 1u));
                 } else {
-                    d = cell_deme(sc, yy * sc.width + xx);
+                    d = cell_deme_at(sc, yy * sc.width + xx, k);
                 }
                 accept = d > 0u;
                 if (accept) {

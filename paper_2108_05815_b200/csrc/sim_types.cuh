@@ -35,6 +35,15 @@ struct ScenarioDev {
     int R;                     // displacement range: dx in [-R, R]
     u32 gauss_len;             // power of two >= 2R
     double delta_t;
+    // temporally varying habitat: n_eras > 0 -> era e holds for k >= era_start[e] (era_start[0] = 0, unused entries
+    // 0xFFFFFFFF). hab8 / deme32 / prefix are then those of the OLDEST map (locations are canonical on it); era_hab8[e * ncells + cell]
+    // (and era_deme32 where a deme >= 255) is the map the dispersal of an event of era e is tested against; prefix0 = prefix sums of
+    // the present-day map (S0: the sample mask ranges over the present-day individuals).
+    u32 n_eras;
+    u32 era_start[4];
+    const uint8_t *era_hab8;
+    const u32 *era_deme32;
+    const u32 *prefix0;
     float margin;              // search filter (exponential sampler): NS_MARGIN * (1 + 1/mu_min), mu_min over the habitat cells
 };
 

@@ -120,7 +120,7 @@ __device__ __forceinline__ bool tail_search_poisson(const SeedKey &key, const Sm
 // prefix of the cell, rate data of the cell. The gathers are issued back to back before anything consumes them.
 // FAST: no exact rescan of crowded guide buckets (far tails, probability ~ 2^-10): `bad` says that the target is unknown.
 template <bool PERCELL, int SAMP, bool COMPACT, bool FAST>
-__device__ __forceinline__ void gauss_target(const ScenarioDev &sc, const GaussLut &gl, u32 x0, u32 y0, u64 u, u32 &c2, u32 &d, u32 &pf, uint2 &cs, bool &bad) {
+__device__ __forceinline__ void gauss_target(const ScenarioDev &sc, const GaussLut &gl, u32 x0, u32 y0, u64 u, u32 k, u32 &c2, u32 &d, u32 &pf, uint2 &cs, bool &bad) {
     bool e1, e2;
     int dx = gauss_disp_fast(gl, (u32)(u >> 32), e1), dy = gauss_disp_fast(gl, (u32)u, e2);
     bad = !(e1 && e2);
@@ -145,8 +145,8 @@ __device__ __forceinline__ void gauss_target(const ScenarioDev &sc, const GaussL
             if (SAMP == 0) cs = ldg_v2_ordered(&sc.scale[ci]);
             else cs.x = ldg_u32_ordered(&sc.thin[ci]), cs.y = 0u;
         }
-        d = ldg_u8_ordered(&sc.hab8[ci]);
-        if (d == 255u) d = __ldg(&sc.deme32[ci]);
+        if (sc.n_eras) d = cell_deme_at(sc, ci, k);         // temporally varying habitat: the map of the event's interval
+        else { d = ldg_u8_ordered(&sc.hab8[ci]); if (d == 255u) d = __ldg(&sc.deme32[ci]); }
     }
 }
 
@@ -162,7 +162,7 @@ __device__ __forceinline__ u32 mulhi64_u32_parts(u32 xlo, u32 xhi, u32 d) {
 // attempt is accepted); bad = the target could not be determined here (crowded guide bucket): the round falls back.
 // xi = the index draw of the lane's candidate. Loads are issued before anything consumes them.
 template <int KIND, bool PERCELL, bool COMPACT>
-__device__ __forceinline__ void fast_slot_a(const ScenarioDev &sc, const GaussLut &gl, u32 sp_q, u32 lane, u32 bm, u32 cell, u64 ua, u32 xi_lo, u32 xi_hi,
+__device__ __forceinline__ void fast_slot_a(const ScenarioDev &sc, const GaussLut &gl, u32 sp_q, u32 lane, u32 bm, u32 cell, u32 kc, u64 ua, u32 xi_lo, u32 xi_hi,
                                             u32 &loc2, u32 &c2, uint2 &cs, bool &acc, bool &bad) {
     bad = false;
     if (KIND == 0) {
@@ -209,8 +209,9 @@ __device__ __forceinline__ void fast_slot_a(const ScenarioDev &sc, const GaussLu
             const u32 ci = yy * sc.width + xx;
             const u32 pf = ldg_u32_ordered(&sc.prefix[ci]);
             if (PERCELL) cs = ldg_v2_ordered(&sc.scale[ci]);
-            u32 d = ldg_u8_ordered(&sc.hab8[ci]);
-            if (d == 255u) d = __ldg(&sc.deme32[ci]);
+            u32 d;
+            if (sc.n_eras) d = cell_deme_at(sc, ci, kc);    // temporally varying habitat: the map of the candidate's interval
+            else { d = ldg_u8_ordered(&sc.hab8[ci]); if (d == 255u) d = __ldg(&sc.deme32[ci]); }
             acc = d > 0u;
             loc2 = pf + ((d == 1u) ? 0u : mulhi64_u32_parts(xi_lo, xi_hi, d));
         }
@@ -320,7 +321,7 @@ __global__ void __launch_bounds__(256, 2) tail_kernel(const ScenarioDev sc, cons
                     const u32 bm = __ballot_sync(NS_FULL, bern(ub, sp_q == 3u ? ep.thr_m : ep.thr_nu));   // bit 4c+1: speciation, 4c+3: migration
                     const u32 xi_lo = __shfl_sync(NS_FULL, (u32)ub, (int)(qb + 2u)), xi_hi = __shfl_sync(NS_FULL, ubh, (int)(qb + 2u));
                     u32 loc2o, c2o; uint2 cso = make_uint2(Cm, sh); bool acc, bad;
-                    fast_slot_a<KIND, PERCELL, COMPACT>(sc, gl, sp_q, lane, bm, cell, ua, xi_lo, xi_hi, loc2o, c2o, cso, acc, bad);
+                    fast_slot_a<KIND, PERCELL, COMPACT>(sc, gl, sp_q, lane, bm, cell, k + sp_dk, ua, xi_lo, xi_hi, loc2o, c2o, cso, acc, bad);
                     // slot B of the lanes with sp_q == 0: approximate offsets of the candidates (partial sums over the points of interval k)
                     // (the draw is tied to the target cell of slot A by an OR with zero: the table gathers, which have the longest latency,
                     // are then issued before this chain starts)
@@ -430,7 +431,7 @@ __global__ void __launch_bounds__(256, 2) tail_kernel(const ScenarioDev sc, cons
                         if (d == 255u) d = __ldg(&sc.deme32[c2]);
                     }
                 } else {
-                    gauss_target<PERCELL, SAMP, COMPACT, true>(sc, gl, cell & 0xFFFFu, cell >> 16, ua, c2, d, pf, cs, bad);
+                    gauss_target<PERCELL, SAMP, COMPACT, true>(sc, gl, cell & 0xFFFFu, cell >> 16, ua, k + sp_dk, c2, d, pf, cs, bad);
                 }
                 // the outcome of EVERY candidate from its own four lanes, before the search says which one it is: first accepted
                 // attempt (= the sequential algorithm's choice, R16), its cell and prefix, the index draw of the candidate
@@ -537,7 +538,7 @@ __global__ void __launch_bounds__(256, 2) tail_kernel(const ScenarioDev sc, cons
                             u32 c2 = 0, d = 0, pf = 0;
                             uint2 cs = make_uint2(Cm, sh);
                             bool bad_;
-                            if (lane >= 3u) gauss_target<PERCELL, SAMP, COMPACT, false>(sc, gl, x0, y0, u, c2, d, pf, cs, bad_);   // attempt r0 + lane - 3 (R16: redraw the whole (dx, dy) pair)
+                            if (lane >= 3u) gauss_target<PERCELL, SAMP, COMPACT, false>(sc, gl, x0, y0, u, k, c2, d, pf, cs, bad_);   // attempt r0 + lane - 3 (R16: redraw the whole (dx, dy) pair)
                             const u32 okm = __ballot_sync(NS_FULL, lane >= 3u && d > 0u);
                             if (okm) {
                                 const int w = first_bit(okm);    // first accepted attempt = the sequential algorithm's choice

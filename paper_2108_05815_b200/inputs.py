@@ -19,7 +19,7 @@ NONSPATIAL, SPATIALLY_IMPLICIT, EXPLICIT_MATRIX, EXPLICIT_GAUSSIAN = 0, 1, 2, 3
 def _base(name, kind, **kw):
     cfg = dict(name=name, kind=kind, width=1, height=1, deme=None, uniform_deme=0, turnover=None,
                uniform_turnover=1.0, matrix=None, sigma=0.0, local_size=0, meta_size=0, migration=0.0,
-               delta_t=2.0, nu=1e-3, seed=42, mask=None, sampler=0)
+               delta_t=2.0, nu=1e-3, seed=42, mask=None, sampler=0, past_deme=None, past_start_k=None)
     cfg.update(kw)
     return cfg
 
@@ -125,6 +125,24 @@ def c6_bigdeme(width=180, height=64, deme_mean=36_000, sigma=2.0, nu=1e-3, sampl
                  nu=nu, seed=seed, mask=mask)
 
 
+def c7_habitat_loss(side=4096, deme=4, sigma=5.0, nu=1e-5, sample=0.1, seed=42, noise_seed=3, mask_seed=7, blur_radius=16.0,
+                    frac_now=0.6, frac_past=0.85, switch_k=500):
+    """Temporally varying habitat: the C5 landscape after a habitat loss. Today frac_now of the cells
+    are habitat (C5's clustered map); before interval switch_k the same smoothed field was thresholded lower, so that frac_past of
+    the cells were habitat -- a superset of today's, cell by cell."""
+    now = clustered_habitat(side, frac_now, blur_radius, noise_seed)
+    past = clustered_habitat(side, frac_past, blur_radius, noise_seed)
+    assert not (now & ~past).any()
+    d_now = now.astype(np.uint32) * np.uint32(deme)
+    d_past = past.astype(np.uint32) * np.uint32(deme)
+    rng = np.random.Generator(np.random.PCG64(mask_seed))
+    mask = (rng.random(int(d_now.sum())) < sample).astype(np.uint8)
+    if mask.sum() == 0:
+        mask[0] = 1
+    return _base("C7-habitat-loss-%dx%d" % (side, side), EXPLICIT_GAUSSIAN, width=side, height=side, deme=d_now, sigma=sigma, nu=nu,
+                 seed=seed, mask=mask, past_deme=d_past[None, :], past_start_k=np.array([switch_k], np.uint32))
+
+
 def n_individuals(cfg):
     if cfg["kind"] == SPATIALLY_IMPLICIT:
         return int(cfg["local_size"])
@@ -138,7 +156,7 @@ def n_sampled(cfg):
 
 
 SCENARIO_KEYS = ("kind", "width", "height", "deme", "uniform_deme", "turnover", "uniform_turnover", "matrix",
-                 "sigma", "local_size", "meta_size", "migration", "delta_t", "sampler")
+                 "sigma", "local_size", "meta_size", "migration", "delta_t", "sampler", "past_deme", "past_start_k")
 
 
 def scenario_kwargs(cfg):

@@ -24,7 +24,8 @@ class ScenarioDesc(C.Structure):
     _fields_ = [("kind", C.c_int32), ("width", C.c_uint32), ("height", C.c_uint32), ("sampler", C.c_uint32), ("deme", C.c_void_p),
                 ("uniform_deme", C.c_uint32), ("turnover", C.c_void_p), ("uniform_turnover", C.c_double),
                 ("dispersal_matrix", C.c_void_p), ("sigma", C.c_double), ("local_size", C.c_uint64),
-                ("meta_size", C.c_uint64), ("migration", C.c_double), ("delta_t", C.c_double)]
+                ("meta_size", C.c_uint64), ("migration", C.c_double), ("delta_t", C.c_double),
+                ("n_past_eras", C.c_uint32), ("past_deme", C.c_void_p), ("past_start_k", C.c_void_p)]
 
 
 class SimParams(C.Structure):
@@ -137,7 +138,7 @@ class Scenario:
     """necsim_create_scenario / necsim_simulate / necsim_destroy (include/necsim.h)."""
 
     def __init__(self, kind, width=1, height=1, deme=None, uniform_deme=0, turnover=None, uniform_turnover=1.0, matrix=None,
-                 sigma=0.0, local_size=0, meta_size=0, migration=0.0, delta_t=2.0, sampler=0):
+                 sigma=0.0, local_size=0, meta_size=0, migration=0.0, delta_t=2.0, sampler=0, past_deme=None, past_start_k=None):
         torch = _torch()
         L = lib()
         self._h = None
@@ -154,6 +155,11 @@ class Scenario:
             a = np.ascontiguousarray(matrix, dtype=np.float64); keep.append(a); d.dispersal_matrix = a.ctypes.data
         d.sigma, d.local_size, d.meta_size = float(sigma), int(local_size), int(meta_size)
         d.migration, d.delta_t = float(migration), float(delta_t)
+        if past_deme is not None:   # temporally varying habitat
+            pd = np.ascontiguousarray(past_deme, dtype=np.uint32).reshape(-1, int(width) * int(height)); keep.append(pd)
+            ps = np.ascontiguousarray(past_start_k, dtype=np.uint32).ravel(); keep.append(ps)
+            assert len(ps) == pd.shape[0]
+            d.n_past_eras, d.past_deme, d.past_start_k = pd.shape[0], pd.ctypes.data, ps.ctypes.data
         nbytes = C.c_size_t()
         _check(L.necsim_scenario_workspace_size(C.byref(d), C.byref(nbytes)))
         self._ws = torch.empty(max(nbytes.value, 256), dtype=torch.uint8, device="cuda")

@@ -3,6 +3,7 @@
     python tests/golden/gen_golden.py            # rng_vectors.txt, neglog_vectors.txt, small_configs.json
     python tests/golden/gen_golden.py --full     # additionally full_configs.json (minutes to hours of CPU)
     python tests/golden/gen_golden.py --full-poisson   # additionally full_configs_poisson.json (sampler = 1)
+    python tests/golden/gen_golden.py --full-c6 / --full-c7   # big-deme workload / habitat-loss workload
 """
 import json
 import os
@@ -78,5 +79,7 @@ if __name__ == "__main__":
         configs(I.full_configs(), "full_configs.json", epoch_events=50_000_000)
     if "--full-c6" in sys.argv:           # SURVEY NEXT-4 big-deme workload at full size (about 10 minutes of CPU)
         configs([I.c6_bigdeme()], "full_config_c6.json", epoch_events=50_000_000)
+    if "--full-c7" in sys.argv:           # temporally varying habitat: the C5 landscape after a habitat loss
+        configs([I.c7_habitat_loss()], "full_config_c7.json", epoch_events=50_000_000)
     if "--full-poisson" in sys.argv:      # the Poisson event-time sampler on the same five configs
         configs(I.full_configs(), "full_configs_poisson.json", epoch_events=50_000_000, sampler=1)

@@ -87,3 +87,24 @@ def test_bigdeme_full_size_matches_oracle(O):
     assert digest(got) == g["digest"]
     assert got["stats"]["n_events_raw"] >= g["unique_events"]
     sc.close()
+
+
+def test_habitat_loss_full_size_matches_oracle(O):
+    """Temporally varying habitat at full size: the C5 landscape after a habitat loss
+    (bench.py --config c7) against tests/golden/full_config_c7.json (oracle only)."""
+    from paper_2108_05815_b200 import inputs as I, necsim as ns
+    f = os.path.join(HERE, "golden", "full_config_c7.json")
+    if not os.path.exists(f):
+        pytest.skip("full_config_c7.json not generated")
+    g = json.load(open(f))[0]
+    cfg = I.c7_habitat_loss()
+    assert g["name"] == cfg["name"]
+    sc = ns.Scenario(**I.scenario_kwargs(cfg))
+    got = sc.simulate(cfg["seed"], cfg["nu"], cfg["mask"])
+    assert got["richness"] == g["richness"] and len(got["labels"]) == g["n_sampled"]
+    assert [int(v) for v in got["labels"][:16]] == g["labels_head"]
+    rows = lambda a: [[int(e["loc"]), int(e["k"]), int(e["j"]), int(e["f"]), int(e["abundance"])] for e in a]
+    assert rows(got["events"][:5]) == g["first_events"] and rows(got["events"][-5:]) == g["last_events"]
+    assert digest(got) == g["digest"]
+    assert got["stats"]["n_events_raw"] >= g["unique_events"]
+    sc.close()
