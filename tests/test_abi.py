@@ -23,12 +23,18 @@ def test_library_exports_every_declared_symbol():
     assert set(names) == set(necsim.EXPORTS)
 
 
-def test_struct_sizes_match_header():
+def test_struct_sizes_match_header(tmp_path):
+    """The ctypes mirrors have the sizes a C compiler gives the structs of include/necsim.h (gcc compiles a probe)."""
+    import subprocess
     from paper_2108_05815_b200 import necsim
-    assert ctypes.sizeof(necsim.ScenarioDesc) == 96
-    assert ctypes.sizeof(necsim.SimParams) == 64
-    assert necsim.EVENT_DTYPE.itemsize == 32
-    assert ctypes.sizeof(necsim.Result) == 216
+    src = tmp_path / "probe.c"
+    src.write_text('#include <stdio.h>\n#include "necsim.h"\nint main(void) { printf("%zu %zu %zu %zu\\n", sizeof(necsim_scenario_desc), '
+                   'sizeof(necsim_sim_params), sizeof(necsim_event), sizeof(necsim_result)); return 0; }\n')
+    exe = tmp_path / "probe"
+    subprocess.check_call(["gcc", "-I", os.path.join(ROOT, "include"), str(src), "-o", str(exe)])
+    sizes = [int(v) for v in subprocess.check_output([str(exe)], text=True).split()]
+    assert sizes == [ctypes.sizeof(necsim.ScenarioDesc), ctypes.sizeof(necsim.SimParams), necsim.EVENT_DTYPE.itemsize, ctypes.sizeof(necsim.Result)]
+    assert sizes[2] == 32
 
 
 def test_error_paths_without_gpu():
