@@ -29,14 +29,14 @@ from paper_2108_05815_b200 import dist as D    # noqa: E402
 
 METRIC = "lineage_events_per_s"
 UNIT = "events/s"
-MAKERS = dict(c1=I.c1_nonspatial, c2=I.c2_implicit, c3=I.c3_matrix, c4=I.c4_gaussian, c5=I.c5_stress, c6=I.c6_bigdeme, c7=I.c7_habitat_loss)
+MAKERS = dict(c3t=lambda: I.c3_matrix(side=64, deme=1000), c1=I.c1_nonspatial, c2=I.c2_implicit, c3=I.c3_matrix, c4=I.c4_gaussian, c5=I.c5_stress, c6=I.c6_bigdeme, c7=I.c7_habitat_loss)
 SMALL = dict(zip(("c1", "c2", "c3", "c4", "c5"), range(5)))
 # Algorithmic integer instructions per executed event (minimal 32-bit instruction sequence of
 # each primitive, weighted by the expected number of draws per event at mu = 2 and the measured attempts per event).
-I_EVENT = dict(c1=230, c2=232, c3=252, c4=263, c5=272, c6=259, c7=272)   # c6: one attempt + 5 % resampling, index draw, deme32 gather; c7 = c5's landscape with eras
+I_EVENT = dict(c3t=252, c1=230, c2=232, c3=252, c4=263, c5=272, c6=259, c7=272)   # c6: one attempt + 5 % resampling, index draw, deme32 gather; c7 = c5's landscape with eras
 # The same count when the event-time search is decided by the binary32 filter (a time draw is then hash 12 +
 # advance 2 + lg2 / scale 4 + accumulate and compare 5 = 23 instead of 68): what the kernels must issue at the least.
-I_EVENT_FILTERED = dict(c1=118, c2=120, c3=140, c4=151, c5=160, c6=147, c7=160)
+I_EVENT_FILTERED = dict(c3t=140, c1=118, c2=120, c3=140, c4=151, c5=160, c6=147, c7=160)
 # issue-slot peak: 148 SMs x 4 schedulers x 32 lanes x 1 instr/clk x sm_max_mhz (B300_MICROARCH "Pipe rates")
 def alu_peak(sm_count, sm_mhz):
     return sm_count * 4 * 32 * sm_mhz * 1e6
@@ -59,6 +59,8 @@ def profile_traffic(kernel, name, sampler):
 def make_cfg(name, small):
     if name == "c6":                                     # SURVEY NEXT-4 shape; --small: demes of ~360
         return I.c6_bigdeme(deme_mean=360, sample=0.05) if small else I.c6_bigdeme()
+    if name == "c3t":                                    # C3's shape with demes of 1000: 4.1e6 lineages on the 128 MiB alias table (throughput probe)
+        return I.c3_matrix(side=13, deme=50) if small else I.c3_matrix(side=64, deme=1000)
     if name == "c7":                                     # temporally varying habitat
         return I.c7_habitat_loss(side=128, blur_radius=4.0, nu=1e-3, sample=0.3, switch_k=40) if small else I.c7_habitat_loss()
     return I.small_configs()[SMALL[name]] if small else MAKERS[name]()
@@ -155,6 +157,84 @@ def reference_arm(args, cfg, name):
                       "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
 
 
+def probe_arm(args, cfg, name, sc, ns, torch, d_mask, n_s):
+    """Micro-workloads for profiling (one kernel launch of interest each)."""
+    if args.probe == "mode_t":
+        n_ev = args.probe_events or 200
+        p = ns.make_params(dedup=False, max_steps=n_ev, tail_threshold=1)
+        for _ in range(1 + max(args.steps, 1)):
+            r = sc.simulate_raw(cfg["seed"], cfg["nu"], d_mask, n_s, p)
+        v = r.n_events_raw / (r.ms_simulate * 1e-3)
+        print(json.dumps({"probe": "mode_t", "workload": cfg["name"], "event_time_sampler": args.sampler, "lineages": int(r.n_lineages), "events_per_lineage": n_ev,
+                          "ms": r.ms_simulate, "events": int(r.n_events_raw), "events_per_s": v, "roofline_frac": v * I_EVENT[name] / alu_peak(148, 1965.0)}))
+    else:
+        n_ev, n_lin = args.probe_events or 20000, 148
+        rng = np.random.Generator(np.random.PCG64(5))
+        mask = np.zeros(sc.n_individuals, np.uint8); mask[rng.choice(sc.n_individuals, n_lin, replace=False)] = 1
+        dm = torch.from_numpy(mask).cuda()
+        out = {"probe": "tail_latency", "workload": cfg["name"], "event_time_sampler": args.sampler, "lineages": n_lin, "events_per_lineage": n_ev}
+        for dedup in (True, False):
+            p = ns.make_params(tail_threshold=10**9, max_steps=n_ev, dedup=dedup, block_threads=32)
+            for _ in range(1 + max(args.steps, 1)):
+                r = sc.simulate_raw(cfg["seed"], 0.0, dm, n_lin, p)
+            out["dedup_on" if dedup else "dedup_off"] = {"ms": r.ms_simulate_tail, "us_per_sequential_event": r.ms_simulate_tail * 1e3 / n_ev,
+                                                          "exact_rounds_per_event": int(r.n_tail_rounds_exact) / max(int(r.n_events_tail), 1)}
+        print(json.dumps(out))
+
+
+def partitioned_arm(args, cfg, name, sc, ns, torch, dist, world, rank, local, flush, params):
+    """The isolated-partitions path: rank r simulates its contiguous share of the sample with no communication,
+    then one all-gather of the species tables and necsim_merge_species on every rank. value = distinct events of the WHOLE sample per
+    second of the slowest rank (strong scaling); duplication = events executed by all ranks / distinct events (the paper's
+    duplication factor, L1469)."""
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def step():
+        flush.fill_(1)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        out = D.simulate_partitioned(sc, cfg["seed"], cfg["nu"], cfg["mask"], rank=rank, world=world, params=params)
+        e1.record(); e1.synchronize()
+        return out, e0.elapsed_time(e1)
+
+    for _ in range(args.warmup):
+        step()
+    sampler = ClockSampler(local)
+    sampler.start()
+    barrier()
+    ms, ms_merge, ev, launches, out = 0.0, 0.0, 0, 0, None
+    for _ in range(args.steps):
+        out, dt = step()
+        ms += dt; ms_merge += out["ms_merge"]
+        if out["local"] is not None:
+            ev += out["local"].n_events_raw; launches += out["local"].n_kernel_launches + 57     # + the merge's kernels (18 radix passes x 3, unpack, flag, write)
+    barrier()
+    clocks = sampler.stop()
+    (ms, ms_merge), (ev_all,) = D.aggregate([ms, ms_merge], [float(ev)], device="cuda")
+    if rank == 0:
+        K = args.steps
+        uniq = unique_events(cfg, args)
+        value = (uniq * K if uniq else ev_all) / (ms * 1e-3)
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": args.warmup, "ms_per_step": ms / K,
+                "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "int64", "data": "synthetic",
+                "value_kind": "distinct events of the whole sample / device time of the slowest rank" if uniq else "raw executed events of all ranks / device time",
+                "config": {"workload": cfg["name"], "event_time_sampler": args.sampler, "nu": cfg["nu"], "mode": "MODE-S, isolated partitions + merge",
+                           "l2": "256 MiB flush write between steps", "parallelism": "partitions x%d" % world},
+                "clocks": clocks, "gpu_launches": int(launches),
+                "richness": int(out["richness"]), "raw_events_all_ranks_per_step": ev_all / K,
+                "duplication_factor": (ev_all / K) / uniq if uniq else None,
+                "merge": {"ms_per_step": ms_merge / K, "what": "all-gather of the species tables (32 B per species) + necsim_merge_species + label translation"},
+                "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": int(0 if cfg["mask"] is None else len(cfg["mask"])), "d2h_bytes_per_step": 0,
+                        "note": "the partition mask is built on the host and copied in inside the timed region; results stay on the device"}}
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -166,6 +246,15 @@ def main():
     ap.add_argument("--sampler", default="exp", choices=["exp", "poisson"],
                     help="event-time sampler of the scenario (DESIGN.md 2.4 / 2.7): same law, different realisation")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--probe", default=None, choices=["mode_t", "tail_latency"],
+                    help="run ONE micro-workload instead of the bench step and print a small JSON line (the ncu captures of profiles/ use "
+                         "these): mode_t = the saturated launch alone (dedup off, --probe-events events per lineage, per-lane kernel); "
+                         "tail_latency = 148 lineages, --probe-events events each, one lineage per warp on its own SM: microseconds per sequential event")
+    ap.add_argument("--probe-events", type=int, default=0, help="events per lineage of a --probe run (default 200 / 20000)")
+    ap.add_argument("--mode", default="replicas", choices=["replicas", "partitioned"],
+                    help="N > 1 (and N = 1): replicas = every rank an independent replicate (weak scaling, the default); partitioned = the "
+                         "sample split over the ranks as isolated partitions, ONE all-gather of the species tables and a device-side merge "
+                         "(PAPER.md L1082-1086; DESIGN.md section 8) -- strong scaling of one simulation")
     ap.add_argument("--event-stream", type=int, default=0, metavar="LOG2_CAP",
                     help="also time the path with the full event stream recorded (SURVEY NEXT-3; DESIGN.md 6.4): the stream holds up to "
                          "2^LOG2_CAP distinct events, the per-epoch ring 2^min(LOG2_CAP, 28) records")
@@ -202,6 +291,10 @@ def main():
     h_labels = torch.empty(n_s, dtype=torch.int32).pin_memory().numpy().view(np.uint32)
     params = ns.make_params()
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")      # > 126 MB L2
+    if args.probe:
+        return probe_arm(args, cfg, name, sc, ns, torch, d_mask, n_s)
+    if args.mode == "partitioned":
+        return partitioned_arm(args, cfg, name, sc, ns, torch, dist, world, rank, local, flush, params)
 
     def barrier():
         if world > 1:
@@ -260,6 +353,8 @@ def main():
         # about 40 % of the path's instructions are multiplies) -- below the issue-slot peak because IMAD.WIDE is not full rate
         peak_meas = int_meas["hash_round_mix"]
         traffic, traffic_src = profile_traffic(dom_name, name, args.sampler)
+        # random 32-byte-sector gather peaks: the denominators for the table gathers (alias matrix, habitat, dedup cache)
+        gather_meas = {"l2_32MiB_GBs": ns.gather_peak(32 << 20)[0] / 1e9, "hbm_4GiB_GBs": ns.gather_peak(4 << 30)[0] / 1e9}
         # MODE-T: the saturated workload (dedup off, every lineage advanced 200 events): where the ALU roofline is meaningful
         rt = sc.simulate_raw(seed, cfg["nu"], d_mask, n_s, ns.make_params(dedup=False, max_steps=200))
         mode_t = rt.n_events_raw / (rt.ms_simulate * 1e-3)
@@ -294,7 +389,8 @@ def main():
                              "instr_per_event_check": "profiles/r2_sass_mix_simulate_kernel_c5.md (executed instructions per event by pipe, ncu source counters)",
                              "note": "latency-bound by construction: one lineage per warp walks a serial chain of ~ln(S)/nu events (DESIGN.md 6.3)",
                              "peak_source": "derived: SMs x 4 schedulers x 32 lanes x sm_max_mhz (DESIGN.md section 6); peak_measured: necsim_debug_int_peak in this run",
-                             "measured_int_peaks_Tinstr_s": {k: v / 1e12 for k, v in int_meas.items()}},
+                             "measured_int_peaks_Tinstr_s": {k: v / 1e12 for k, v in int_meas.items()},
+                             "measured_random_sector_gather_peaks": gather_meas},
                 "mode_t": {"value": mode_t, "unit": UNIT, "what": "dedup off, 200 events per lineage, saturated machine",
                            "roofline_frac": mode_t * I_EVENT[name] / peak, "frac_measured": mode_t * I_EVENT[name] / peak_meas,
                            "frac_filtered_count": mode_t * I_EVENT_FILTERED[name] / peak,

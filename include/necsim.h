@@ -242,6 +242,11 @@ int necsim_debug_next_event_poisson(const necsim_scenario *scn, uint64_t seed, c
                                     void *cuda_stream);
 /* copies the Poisson cdf thresholds PC[256] and the per-cell thinning thresholds [ncells] to HOST (any may be NULL) */
 int necsim_debug_poisson_table(const necsim_scenario *scn, uint64_t *h_pc, uint32_t *h_thin, double *mu_max, void *cuda_stream);
+/* random-gather peak micro-benchmark ("a measured L2 random-sector peak"): every thread of a full-occupancy grid reads 8 bytes
+ * from loads_per_thread pseudo-random 32-byte sectors of the caller's table (DEVICE, table_bytes long: smaller than L2 = the L2
+ * random-sector peak, much larger = the HBM random-sector peak). Returns sector bytes (32 per load) per second. d_sink: DEVICE, 4 bytes. */
+int necsim_debug_gather_peak(const void *d_table /*DEVICE*/, uint64_t table_bytes, uint32_t loads_per_thread, uint32_t *d_sink /*DEVICE*/,
+                             void *cuda_stream, double *sector_bytes_per_s /*HOST out*/, float *ms /*HOST out*/);
 /* integer-pipe peak micro-benchmark: runs `iters` iterations of an unrolled chain of
  * independent IMAD.WIDE / LOP3 / SHF / IADD3 on every SM; kind 0 = mixed hash-like, 1 = IMAD only,
  * 2 = ALU (LOP3/SHF/IADD3) only. d_sink: DEVICE, 4 bytes of the caller (keeps the chains alive; never written in practice).

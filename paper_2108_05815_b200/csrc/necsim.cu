@@ -1166,6 +1166,48 @@ __global__ void __launch_bounds__(256) int_peak_kernel(u32 iters, u32 *sink) {
     if (r == 0x12345678u) sink[0] = r;   // keeps the chains alive
 }
 
+// random 32-byte-sector gather peak (the denominator for the alias-table and habitat gathers): every thread reads 8 bytes
+// from `loads` pseudo-random 32-byte sectors of a table of `sectors` sectors, 8 independent loads in flight
+__global__ void __launch_bounds__(256) gather_peak_kernel(const uint2 *table, u64 sectors, u32 loads, u32 *sink) {
+    u64 x = ((u64)blockIdx.x * blockDim.x + threadIdx.x) * NS_GAMMA + 0x9E3779B97F4A7C15ull;
+    u32 acc = 0;
+    for (u32 i = 0; i < loads; i += 8) {
+        uint2 v[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            x = x * 6364136223846793005ull + 1442695040888963407ull;
+            const u64 sct = __umul64hi(x, sectors);
+            asm volatile("ld.global.nc.v2.u32 {%0, %1}, [%2];" : "=r"(v[u].x), "=r"(v[u].y) : "l"(table + 4 * sct));
+        }
+#pragma unroll
+        for (int u = 0; u < 8; ++u) acc ^= v[u].x + v[u].y;
+    }
+    if (acc == 0x12345678u) sink[0] = acc;
+}
+extern "C" int necsim_debug_gather_peak(const void *d_table, uint64_t table_bytes, uint32_t loads_per_thread, uint32_t *d_sink, void *cuda_stream,
+                                        double *sector_bytes_per_s, float *ms_out) {
+    if (!d_table || !d_sink || table_bytes < 32 || loads_per_thread == 0) return fail(NECSIM_ERR_INVALID_ARG, "bad argument");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int dev_id = 0, sm = 0;
+    CU(cudaGetDevice(&dev_id));
+    CU(cudaDeviceGetAttribute(&sm, cudaDevAttrMultiProcessorCount, dev_id));
+    cudaEvent_t e0, e1;
+    CU(cudaEventCreate(&e0)); CU(cudaEventCreate(&e1));
+    const u32 grid = (u32)sm * 8u, block = 256u, loads = (loads_per_thread + 7u) & ~7u;
+    for (int rep = 0; rep < 2; ++rep) {
+        if (rep == 1) CU(cudaEventRecord(e0, st));
+        gather_peak_kernel<<<grid, block, 0, st>>>((const uint2 *)d_table, table_bytes / 32, loads, d_sink);
+    }
+    CU(cudaEventRecord(e1, st));
+    CU(cudaStreamSynchronize(st));
+    float ms = 0.f;
+    CU(cudaEventElapsedTime(&ms, e0, e1));
+    if (ms_out) *ms_out = ms;
+    if (sector_bytes_per_s) *sector_bytes_per_s = 32.0 * (double)loads * (double)grid * (double)block / ((double)ms * 1e-3);
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    return NECSIM_OK;
+}
+
 extern "C" int necsim_debug_int_peak(int kind, uint32_t iters, uint32_t *d_sink, void *cuda_stream, double *thread_instr_per_s, float *ms_out) {
     if (!d_sink) return fail(NECSIM_ERR_INVALID_ARG, "d_sink is NULL (a 4-byte device buffer of the caller)");
     cudaStream_t st = (cudaStream_t)cuda_stream;

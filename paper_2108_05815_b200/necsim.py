@@ -17,7 +17,7 @@ EXPORTS = ["necsim_scenario_workspace_size", "necsim_create_scenario", "necsim_s
            "necsim_simulate_workspace_size", "necsim_simulate", "necsim_simulate_host", "necsim_destroy", "necsim_last_error",
            "necsim_debug_draw", "necsim_debug_neglog", "necsim_debug_next_event", "necsim_debug_disperse", "necsim_debug_tables",
            "necsim_debug_int_peak", "necsim_debug_next_event_poisson", "necsim_debug_poisson_table",
-           "necsim_merge_workspace_size", "necsim_merge_species", "necsim_debug_approx_time"]
+           "necsim_merge_workspace_size", "necsim_merge_species", "necsim_debug_approx_time", "necsim_debug_gather_peak"]
 
 
 class ScenarioDesc(C.Structure):
@@ -89,6 +89,7 @@ def lib():
         L.necsim_debug_next_event_poisson.argtypes = [vp, u64] + [vp] * 8 + [u64, vp]
         L.necsim_debug_poisson_table.argtypes = [vp] * 5
         L.necsim_debug_approx_time.argtypes = [vp, u32, u32, vp, vp, vp, u64, vp]
+        L.necsim_debug_gather_peak.argtypes = [vp, u64, u32, vp, vp, vp, vp]
         L.necsim_merge_workspace_size.argtypes = [u64, vp]
         L.necsim_merge_species.argtypes = [vp, u64, vp, C.c_size_t, vp, vp, vp, vp]
         _lib = L
@@ -362,6 +363,17 @@ def debug_next_event(seed, loc, k, f_last, Cm, sh):
     _check(lib().necsim_debug_next_event(int(seed), dl.data_ptr(), dk.data_ptr(), df.data_ptr(), dc.data_ptr(), ds.data_ptr(), ko.data_ptr(),
                                          jo.data_ptr(), To.data_ptr(), rc.data_ptr(), n, _stream_ptr(torch)))
     return (ko.cpu().numpy().view(np.uint32), jo.cpu().numpy().view(np.uint32), To.cpu().numpy().view(np.uint64), rc.cpu().numpy())
+
+
+def gather_peak(table_bytes, loads_per_thread=256):
+    """Random 32-byte-sector gather micro-benchmark over a table of table_bytes: returns (sector bytes per second, ms)."""
+    torch = _torch()
+    table = torch.zeros(int(table_bytes), dtype=torch.uint8, device="cuda")
+    sink = torch.zeros(1, dtype=torch.int32, device="cuda")
+    v, ms = C.c_double(), C.c_float()
+    _check(lib().necsim_debug_gather_peak(C.c_void_p(table.data_ptr()), int(table_bytes), int(loads_per_thread), C.c_void_p(sink.data_ptr()),
+                                          _stream_ptr(torch), C.byref(v), C.byref(ms)))
+    return v.value, ms.value
 
 
 def int_peak(kind, iters=4096):

@@ -69,3 +69,13 @@ def test_product_arm_event_stream_leg():
     r = json.loads(lines[0])
     s = r["event_stream"]
     assert s["ms_per_step"] > 0 and s["distinct_events"] >= r["richness"] > 0 and s["distinct_events_per_s"] > 0 and s["epochs"] >= 1
+
+
+@pytest.mark.gpu
+def test_product_arm_partitioned_mode():
+    """--mode partitioned drives dist.simulate_partitioned (isolated partitions + merge) and prints the same line shape."""
+    lines = run_bench("--small", "--config", "c4", "--mode", "partitioned", "--steps", "2", "--warmup", "3")
+    assert len(lines) == 1
+    r = json.loads(lines[0])
+    assert r["config"]["parallelism"] == "partitions x1" and r["scaling"] == "strong" and r["n_gpus"] == 1
+    assert r["value"] > 0 and r["gpu_launches"] > 0 and r["merge"]["ms_per_step"] > 0 and r["richness"] > 0

@@ -21,6 +21,14 @@ def _worker(rank, world, port, out):
     tab = torch.full((32 * (rank + 2),), rank + 1, dtype=torch.uint8)
     cat, offsets = D.gather_tables(tab)
     assert offsets == [0, 2] and cat.numel() == 32 * 5 and bool((cat[:64] == 1).all()) and bool((cat[64:] == 2).all())
+    # uneven and EMPTY shards: rank 1 contributes no species table at all
+    tab2 = torch.full((32 * 3,), 7, dtype=torch.uint8) if rank == 0 else torch.empty(0, dtype=torch.uint8)
+    cat2, off2 = D.gather_tables(tab2)
+    assert off2 == [0, 3] and cat2.numel() == 96 and bool((cat2 == 7).all())
+    # label translation of this rank's lineages through a merged map (the step after the gather)
+    dmap = torch.arange(10, 15, dtype=torch.int64)                      # merged rank of each of the 5 gathered records
+    lab = torch.tensor([0, 1, -1] if rank == 0 else [2, 0, -1], dtype=torch.int64)
+    assert D.translate_labels(lab, dmap, offsets[rank]).tolist() == ([10, 11, -1] if rank == 0 else [14, 12, -1])
     out[rank] = (seed, times, units, D.throughput(units[0], times[0]))
     dist.barrier()
     dist.destroy_process_group()
