@@ -93,11 +93,11 @@ typedef struct necsim_sim_params {
                                   the paper probes every step_slice steps) */
     uint32_t record_events;    /* 1 = also produce the full event stream (PAPER.md 6.2 L813-906, 7.1.3 L958-967):
                                   every distinct executed event (speciation and dispersal), sorted by (k, f, loc, j) */
-    uint32_t stream_sort_bytes;/* record_events: the radix sort of an epoch's records covers k and the leading 1..6 bytes of f; records
+    uint32_t stream_sort_bytes;/* record_events: the radix sort of an epoch's records covers k and the leading 1..5 bytes of f; records
                                   that agree there are ordered by insertion (few, unless this is small). 0 = default: per epoch, the fewest
                                   bytes that leave about two records or fewer per value of that prefix. The
                                   stream does not depend on it */
-    uint64_t event_ring_capacity;   /* records one epoch may produce (incl. redundant ones); 0 = 2^24. Each takes 36 bytes of workspace */
+    uint64_t event_ring_capacity;   /* records one epoch may produce (incl. redundant ones); 0 = 2^24. Each takes 60 bytes of workspace */
     uint64_t event_stream_capacity; /* distinct events of the whole run; 0 = 2^26. Each takes 24 bytes of workspace */
 } necsim_sim_params;
 

@@ -261,60 +261,169 @@ __global__ void __launch_bounds__(256) merge_write_kernel(const SimBuffers bf, c
 }
 
 // ---- full event stream: one epoch's ring, sorted and made unique, appended to the run's stream -------
-__global__ void __launch_bounds__(256) iota_kernel(u32 *perm, u32 n) {
-    u32 i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) perm[i] = i;
-}
-// The ring is radix-sorted on a prefix of its key only: k and the top `fbytes` bytes of f. Records that share the prefix are
-// adjacent and few (redundant executions of one event, and distinct events whose offsets agree in the leading bits), so the
-// first thread of such a run puts it into full (f, loc, j) order by insertion. Runs of sentinels stay as they are.
-__device__ __forceinline__ bool stream_less(const SimBuffers &bf, u32 a, u32 b) {   // same k: order by (f, loc, j)
-    const u64 fa = bf.term_f[a], fb = bf.term_f[b];
-    if (fa != fb) return fa < fb;
-    const u32 la = bf.term_loc[a], lb = bf.term_loc[b];
-    if (la != lb) return la < lb;
-    return bf.term_j[a] < bf.term_j[b];
-}
-// Also writes the head flags of the sorted ring: 1 for the first record of every distinct event, 0 for its redundant copies
-// (adjacent after the sort) and for sentinel records (k = the epoch's k_stop: reserved but unused slots, sorted last).
-__global__ void __launch_bounds__(256) stream_ties_kernel(const SimBuffers bf, u32 *__restrict__ perm, u32 n, u32 k_sentinel, u32 fbytes,
-                                                          u32 *__restrict__ flag) {
-    const u32 i = blockIdx.x * blockDim.x + threadIdx.x, lane = threadIdx.x & 31u;
-    const bool in = i < n;
-    const u32 sh = 48u - 8u * fbytes;
-    const u32 id = in ? perm[i] : 0u, k = in ? bf.term_k[id] : k_sentinel;
-    const u64 fp = in ? bf.term_f[id] >> sh : 0ull;
-    // the previous record's prefix comes from the neighbouring lane (a record a run's first thread is moving at this moment
-    // is still one of that run: the answer is the same)
-    u32 pk = __shfl_up_sync(NS_FULL, k, 1);
-    u64 pf = __shfl_up_sync(NS_FULL, fp, 1);
-    if (in && lane == 0 && i != 0) { const u32 pv = perm[i - 1]; pk = bf.term_k[pv]; pf = bf.term_f[pv] >> sh; }
-    if (!in) return;
-    if (k == k_sentinel) { flag[i] = 0u; return; }
-    if (i != 0 && pk == k && pf == fp) return;   // not the first of its run
-    flag[i] = 1u;
-    u32 e = i + 1;
-    for (; e < n; ++e) {
-        const u32 x = perm[e];
-        if (bf.term_k[x] != k || (bf.term_f[x] >> sh) != fp) break;
-        u32 q = e;
-        while (q > i && stream_less(bf, x, perm[q - 1])) { perm[q] = perm[q - 1]; --q; }
-        perm[q] = x;
+// The ring holds one 32-byte record per executed event and, beside it, the record's 64-bit time key (k - k_start) << 40 | f >> 8.
+// The sort never touches the records: LSD radix passes over (key, index) pairs, 12 bytes read and 12 written per record and pass,
+// fully coalesced; only k and the leading `fbytes` bytes of f are sorted on. Records that agree there are adjacent and few (redundant
+// executions of one event, and distinct events whose offsets share those bits); the first thread of such a run orders it by the full
+// (f, loc, j) with the records gathered through the index (one 32-byte sector each). Runs longer than NS_RUN_INLINE go to a warp.
+#define NS_RUN_INLINE 16u
+#define NS_PAIR_TILE 4096u          // pairs per block and pass: 16 per digit on average, so that a digit's pairs leave the block as one run
+__global__ void __launch_bounds__(256) pair_hist_kernel(const u64 *__restrict__ keys, u32 n, u32 shift, u32 *__restrict__ hist, u32 nblocks) {
+    __shared__ u32 h[256];
+    h[threadIdx.x] = 0;
+    __syncthreads();
+    const u32 start = blockIdx.x * NS_PAIR_TILE;
+    for (u32 r = 0; r < NS_PAIR_TILE; r += 256u) {
+        const u32 i = start + r + threadIdx.x;
+        if (i < n) atomicAdd(&h[(u32)(keys[i] >> shift) & 255u], 1u);
     }
-    for (u32 p = i + 1; p < e; ++p) flag[p] = same_event(bf, perm[p], perm[p - 1]) ? 0u : 1u;
+    __syncthreads();
+    hist[threadIdx.x * nblocks + blockIdx.x] = h[threadIdx.x];
 }
-// bf.term_* alias the ring's key arrays; uidx = the head flags scanned exclusively, *total = their sum: the heads are written
-__global__ void __launch_bounds__(256) stream_write_kernel(const SimBuffers bf, const u32 *__restrict__ rec_loc2, const u32 *__restrict__ perm, u32 n,
-                                                           const u32 *__restrict__ uidx, const u32 *__restrict__ total, u64 base, u64 cap, u32 *__restrict__ s_loc,
+// stable scatter of the pairs (after an exclusive scan of hist); idx_in == NULL: the identity (first pass). A warp ranks its 512
+// consecutive pairs against its own digit counters, the block orders the tile by digit in shared memory, and every digit's pairs
+// are then written to their place in one coalesced run (a direct scatter from registers writes 8 useful bytes per 32-byte sector).
+__global__ void __launch_bounds__(256) pair_scatter_kernel(const u64 *__restrict__ keys_in, const u32 *__restrict__ idx_in, u64 *__restrict__ keys_out,
+                                                           u32 *__restrict__ idx_out, u32 n, u32 shift, const u32 *__restrict__ hist, u32 nblocks) {
+    extern __shared__ unsigned char pair_smem[];
+    u64 *skey = (u64 *)pair_smem;                           // [NS_PAIR_TILE]
+    u32 *sidx = (u32 *)(skey + NS_PAIR_TILE);               // [NS_PAIR_TILE]
+    u32 (*wcount)[256] = (u32 (*)[256])(sidx + NS_PAIR_TILE);   // [8][256]
+    u32 *bdo = (u32 *)(wcount + 8);                         // [256] first position of a digit inside the ordered tile
+    u32 *gbase = bdo + 256;                                 // [256] global position of the tile's first pair of a digit
+    const u32 lane = threadIdx.x & 31u, w = threadIdx.x >> 5;
+    for (u32 ww = 0; ww < 8; ++ww) wcount[ww][threadIdx.x] = 0;
+    __syncthreads();
+    const u32 tile0 = blockIdx.x * NS_PAIR_TILE, start = tile0 + w * (NS_PAIR_TILE / 8u);
+    u64 key[16];
+    u32 item[16], dr[16];                               // dr = digit | rank inside the warp's 512 positions << 9
+#pragma unroll
+    for (u32 r = 0; r < 16; ++r) {
+        const u32 i = start + r * 32u + lane;
+        const bool valid = i < n;
+        key[r] = valid ? keys_in[i] : 0ull;
+        item[r] = valid ? (idx_in ? idx_in[i] : i) : 0u;
+        const u32 d = valid ? (u32)(key[r] >> shift) & 255u : 256u + lane;    // invalid lanes never match anyone
+        const u32 peers = __match_any_sync(NS_FULL, d);
+        const u32 before = __popc(peers & lanemask_lt());
+        const u32 rank = valid ? wcount[w][d] + before : 0u;
+        __syncwarp();
+        if (valid && before == 0) wcount[w][d] = rank + __popc(peers);
+        __syncwarp();
+        dr[r] = d | (rank << 9);
+    }
+    __syncthreads();
+    // digit threadIdx.x: the tile's count, the warps' offsets inside the digit, the digit's first position in the ordered tile
+    u32 tot = 0;
+    for (u32 ww = 0; ww < 8; ++ww) { const u32 c = wcount[ww][threadIdx.x]; wcount[ww][threadIdx.x] = tot; tot += c; }
+    u32 x = tot;                                        // exclusive scan of the 256 digit counts over the block
+    for (int o = 1; o < 32; o <<= 1) { const u32 y = __shfl_up_sync(NS_FULL, x, o); if ((int)lane >= o) x += y; }
+    __shared__ u32 wtot[8];
+    if (lane == 31) wtot[w] = x;
+    __syncthreads();
+    u32 off = x - tot;
+    for (u32 ww = 0; ww < w; ++ww) off += wtot[ww];
+    bdo[threadIdx.x] = off;
+    gbase[threadIdx.x] = hist[threadIdx.x * nblocks + blockIdx.x];
+    __syncthreads();
+#pragma unroll
+    for (u32 r = 0; r < 16; ++r) {
+        const u32 d = dr[r] & 511u;
+        if (d < 256u) { const u32 p = bdo[d] + wcount[w][d] + (dr[r] >> 9); skey[p] = key[r]; sidx[p] = item[r]; }
+    }
+    __syncthreads();
+    const u32 cnt = min(NS_PAIR_TILE, n - tile0);
+    for (u32 t = threadIdx.x; t < cnt; t += 256u) {
+        const u64 k = skey[t];
+        const u32 d = (u32)(k >> shift) & 255u;
+        const u32 o = gbase[d] + (t - bdo[d]);
+        keys_out[o] = k; idx_out[o] = sidx[t];
+    }
+}
+#define NS_PAIR_SMEM (NS_PAIR_TILE * 12u + 8u * 256u * 4u + 2u * 256u * 4u)
+// order of two records of the same interval k: by (f, loc, j)
+__device__ __forceinline__ bool rec_less(const uint4 *__restrict__ rec, u32 a, u32 b) {
+    const uint4 a1 = rec[2u * a + 1u], b1 = rec[2u * b + 1u];
+    const u64 fa = ((u64)a1.y << 32) | a1.x, fb = ((u64)b1.y << 32) | b1.x;
+    if (fa != fb) return fa < fb;
+    const uint4 a0 = rec[2u * a], b0 = rec[2u * b];
+    if (a0.x != b0.x) return a0.x < b0.x;
+    return a0.z < b0.z;
+}
+__device__ __forceinline__ bool rec_same(const uint4 *__restrict__ rec, u32 a, u32 b) {
+    const uint4 a0 = rec[2u * a], b0 = rec[2u * b], a1 = rec[2u * a + 1u], b1 = rec[2u * b + 1u];
+    return a0.x == b0.x && a0.y == b0.y && a0.z == b0.z && a1.x == b1.x && a1.y == b1.y;
+}
+// Runs of equal key prefix (key >> pshift): head flags (1 = first record of a distinct event; redundant copies, adjacent after the
+// sort, and sentinels get 0) and the full order inside a run. Only the first thread of a run writes idx[i..e) and
+// flag[i..e); everybody else reads the keys, which this kernel never changes. Long runs are queued for stream_long_runs_kernel.
+__global__ void __launch_bounds__(256) stream_ties_kernel(const u64 *__restrict__ keys, u32 *__restrict__ idx, const uint4 *__restrict__ rec, u32 n, u32 pshift,
+                                                          u32 *__restrict__ flag, u32 *__restrict__ long_runs, u32 *__restrict__ n_long, u32 long_cap) {
+    const u32 i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const u64 key = keys[i];
+    if (key == ~0ull) { flag[i] = 0u; return; }          // reserved but unused ring slot
+    const u64 kp = key >> pshift;
+    if (i != 0 && (keys[i - 1] >> pshift) == kp) return; // not the first of its run
+    u32 e = i + 1;
+    while (e < n && (keys[e] >> pshift) == kp) ++e;
+    if (e == i + 1) { flag[i] = 1u; return; }            // the usual case: nothing shares the prefix
+    if (e - i > NS_RUN_INLINE) {
+        const u32 slot = atomicAdd(n_long, 1u);
+        if (slot < long_cap) { long_runs[2u * slot] = i; long_runs[2u * slot + 1u] = e - i; return; }
+    }
+    for (u32 p = i + 1; p < e; ++p) {                    // insertion sort of idx[i..e) by (f, loc, j)
+        const u32 x = idx[p];
+        u32 q = p;
+        while (q > i && rec_less(rec, x, idx[q - 1])) { idx[q] = idx[q - 1]; --q; }
+        idx[q] = x;
+    }
+    flag[i] = 1u;
+    for (u32 p = i + 1; p < e; ++p) flag[p] = rec_same(rec, idx[p], idx[p - 1]) ? 0u : 1u;
+}
+// One warp per long run. Long runs are almost always copies of ONE event (many lineages on a shared path, dedup off or a small
+// cache): that is checked first in a single sweep. Otherwise the run is ordered by ranking every record against all others.
+__global__ void __launch_bounds__(256) stream_long_runs_kernel(u32 *__restrict__ idx, const uint4 *__restrict__ rec, u32 *__restrict__ flag,
+                                                               const u32 *__restrict__ long_runs, const u32 *__restrict__ n_long, u32 long_cap, u32 *__restrict__ tmp) {
+    const u32 lane = threadIdx.x & 31u, warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarps = (gridDim.x * blockDim.x) >> 5;
+    const u32 nl = min(*n_long, long_cap);
+    for (u32 r = warp; r < nl; r += nwarps) {
+        const u32 i = long_runs[2u * r], L = long_runs[2u * r + 1u];
+        const u32 first = idx[i];
+        bool same = true;
+        for (u32 p = lane; p < L; p += 32u) same = same && rec_same(rec, idx[i + p], first);
+        if (__all_sync(NS_FULL, same)) {
+            for (u32 p = lane; p < L; p += 32u) flag[i + p] = p == 0u ? 1u : 0u;
+            continue;
+        }
+        for (u32 p = lane; p < L; p += 32u) {            // rank of record p: records before it in (f, loc, j), ties by position
+            const u32 x = idx[i + p];
+            u32 rank = 0;
+            for (u32 q = 0; q < L; ++q) {
+                const u32 y = idx[i + q];
+                if (rec_less(rec, y, x) || (q < p && !rec_less(rec, x, y))) ++rank;
+            }
+            tmp[i + rank] = x;
+        }
+        __syncwarp();
+        for (u32 p = lane; p < L; p += 32u) idx[i + p] = tmp[i + p];
+        __syncwarp();
+        for (u32 p = lane; p < L; p += 32u) flag[i + p] = (p == 0u || !rec_same(rec, idx[i + p], idx[i + p - 1u])) ? 1u : 0u;
+    }
+}
+// uidx = the head flags scanned exclusively, *total = their sum: the heads are appended to the stream (SoA, coalesced writes)
+__global__ void __launch_bounds__(256) stream_write_kernel(const uint4 *__restrict__ rec, const u32 *__restrict__ idx, u32 n, const u32 *__restrict__ uidx,
+                                                           const u32 *__restrict__ total, u64 base, u64 cap, u32 *__restrict__ s_loc,
                                                            u32 *__restrict__ s_k, u32 *__restrict__ s_j, u64 *__restrict__ s_f, u32 *__restrict__ s_loc2) {
-    u32 i = blockIdx.x * blockDim.x + threadIdx.x;
+    const u32 i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const u32 u = uidx[i], nx = (i + 1 < n) ? uidx[i + 1] : *total;
     if (nx == u) return;
     const u64 o = base + u;
     if (o >= cap) return;
-    const u32 id = perm[i];
-    s_loc[o] = bf.term_loc[id]; s_k[o] = bf.term_k[id]; s_j[o] = bf.term_j[id]; s_f[o] = bf.term_f[id]; s_loc2[o] = rec_loc2[id];
+    const u32 id = idx[i];
+    const uint4 r0 = rec[2u * id], r1 = rec[2u * id + 1u];
+    s_loc[o] = r0.x; s_k[o] = r0.y; s_j[o] = r0.z; s_loc2[o] = r0.w; s_f[o] = ((u64)r1.y << 32) | r1.x;
 }
 
 __global__ void copy_u32_kernel(u32 *a, const u32 *src, u32 n) {

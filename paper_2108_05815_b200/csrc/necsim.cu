@@ -474,7 +474,7 @@ static int resolve_params(const necsim_scenario *scn, const necsim_sim_params *p
     if (r.max_steps > 0xFFFFFFFFull) return fail(NECSIM_ERR_INVALID_ARG, "max_steps must fit 32 bits");
     r.tail_threshold = p->tail_threshold;
     r.record = p->record_events != 0;
-    if (p->stream_sort_bytes > 6) return fail(NECSIM_ERR_INVALID_ARG, "stream_sort_bytes must be in [0, 6]");
+    if (p->stream_sort_bytes > 5) return fail(NECSIM_ERR_INVALID_ARG, "stream_sort_bytes must be in [0, 5]");
     r.stream_fbytes = p->stream_sort_bytes;   // 0 = chosen per epoch
     r.ring_cap = r.record ? (p->event_ring_capacity ? p->event_ring_capacity : (1ull << 24)) : 0;
     r.stream_cap = r.record ? (p->event_stream_capacity ? p->event_stream_capacity : (1ull << 26)) : 0;
@@ -488,7 +488,7 @@ static int resolve_params(const necsim_scenario *scn, const necsim_sim_params *p
 struct SimLayout {
     size_t off_ctr, off_qa, off_qb, off_cache, off_term_loc, off_term_k, off_term_j, off_steps, off_parent, off_ring, off_term_f,
         off_state, off_events, off_labels, off_species, off_perm_a, off_perm_b, off_flag, off_hist, off_chunk, off_mask,
-        off_scan, off_rec_loc, off_rec_k, off_rec_j, off_rec_l2, off_rec_f, off_st_loc, off_st_k, off_st_j, off_st_l2, off_st_f, total;
+        off_scan, off_rec, off_key_a, off_key_b, off_long, off_st_loc, off_st_k, off_st_j, off_st_l2, off_st_f, total;
     u32 n_chunks, sort_blocks;
 };
 
@@ -509,8 +509,8 @@ static void sim_layout(u64 n_individuals, u64 cap, const ResolvedParams &rp, Sim
     L.off_hist = take(4 * 256 * (size_t)L.sort_blocks); L.off_chunk = take(4 * ((size_t)L.n_chunks + 1));
     L.off_mask = take(n_individuals);
     L.off_scan = take(4 * ((std::max<size_t>(256 * (size_t)L.sort_blocks, sort_n) + NS_SCAN_TILE - 1) / NS_SCAN_TILE + 1));
-    L.off_rec_loc = take(4 * rp.ring_cap); L.off_rec_k = take(4 * rp.ring_cap); L.off_rec_j = take(4 * rp.ring_cap);
-    L.off_rec_l2 = take(4 * rp.ring_cap); L.off_rec_f = take(8 * rp.ring_cap);
+    L.off_rec = take(32 * rp.ring_cap); L.off_key_a = take(8 * rp.ring_cap); L.off_key_b = take(8 * rp.ring_cap);
+    L.off_long = take(8 * (rp.ring_cap / NS_RUN_INLINE + 1));
     L.off_st_loc = take(4 * rp.stream_cap); L.off_st_k = take(4 * rp.stream_cap); L.off_st_j = take(4 * rp.stream_cap);
     L.off_st_l2 = take(4 * rp.stream_cap); L.off_st_f = take(8 * rp.stream_cap);
     L.total = off;
@@ -591,13 +591,16 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
     u32 *perm_a = (u32 *)(base + L.off_perm_a), *perm_b = (u32 *)(base + L.off_perm_b), *flag = (u32 *)(base + L.off_flag);
     uint8_t *digit = (uint8_t *)flag;   // the head flags are written after the sort: the same memory holds a pass's digits
     u32 *hist = (u32 *)(base + L.off_hist), *chunk = (u32 *)(base + L.off_chunk), *scan_tmp = (u32 *)(base + L.off_scan);
-    bf.rec_loc = (u32 *)(base + L.off_rec_loc); bf.rec_k = (u32 *)(base + L.off_rec_k); bf.rec_j = (u32 *)(base + L.off_rec_j);
-    bf.rec_loc2 = (u32 *)(base + L.off_rec_l2); bf.rec_f = (u64 *)(base + L.off_rec_f); bf.rec_cap = (u32)rp.ring_cap;
+    bf.rec = (uint4 *)(base + L.off_rec); bf.rec_key = (u64 *)(base + L.off_key_a); bf.rec_cap = (u32)rp.ring_cap;
+    u64 *key_a = (u64 *)(base + L.off_key_a), *key_b = (u64 *)(base + L.off_key_b);
+    u32 *long_runs = (u32 *)(base + L.off_long);
+    const u32 long_cap = (u32)(rp.ring_cap / NS_RUN_INLINE + 1);
     u32 *st_loc = (u32 *)(base + L.off_st_loc), *st_k = (u32 *)(base + L.off_st_k), *st_j = (u32 *)(base + L.off_st_j), *st_l2 = (u32 *)(base + L.off_st_l2);
     u64 *st_f = (u64 *)(base + L.off_st_f);
     u64 stream_n = 0;
     SimCounters *hc = scn->h_ctr;
 
+    if (rp.record) CU(cudaFuncSetAttribute(pair_scatter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)NS_PAIR_SMEM));
     CU(cudaEventRecord(scn->ev[0], st));
     CU(cudaMemsetAsync(bf.ctr, 0, sizeof(SimCounters), st));
     CU(cudaMemsetAsync(bf.state, 0, cap, st));
@@ -672,6 +675,7 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
             }
             double span = w / ((double)active * scn->mu_max);
             u64 sp = span < 1.0 ? 1ull : (span > 1e9 ? 1000000000ull : (u64)span);
+            if (rp.record) sp = std::min<u64>(sp, (1ull << 24) - 1);   // the record's time key has 24 bits for k - k_start
             u64 h = (u64)k_start + sp;
             k_stop = h >= 0xFFFFFFFFull ? 0xFFFFFFFFu : (u32)h;
         }
@@ -695,11 +699,13 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
             grid = (u32)std::min<u64>(full_grid, (warps + warps_per_block - 1) / warps_per_block);
         }
         ep.rec_chunk = 1;
-        if (rp.record && tail) {   // chunked ring reservation: at most a quarter of the ring may sit in unused reservations
-            const u64 warps = std::min<u64>(active, (u64)grid * warps_per_block);
-            ep.rec_chunk = (u32)std::max<u64>(1, std::min<u64>(NS_REC_CHUNK, rp.ring_cap / (4 * std::max<u64>(warps, 1))));
+        if (rp.record) {   // chunked ring reservation: at most a quarter (tail) / an eighth (per-lane kernel) of the ring may sit in unused reservations
+            const u64 warps = std::max<u64>(1, std::min<u64>(active, (u64)grid * warps_per_block));
+            if (tail) ep.rec_chunk = (u32)std::max<u64>(1, std::min<u64>(NS_REC_CHUNK, rp.ring_cap / (4 * warps)));
+            else ep.rec_chunk = (u32)std::min<u64>(1024, rp.ring_cap / (8 * warps));      // < 64: the kernel reserves exactly what a pass needs
         }
         bf.q_in = q_in; bf.q_out = q_out; bf.q_in_count = active;
+        bf.k_base = rp.record ? k_start : 0u;    // REC kernels: the time key of a record holds k - k_start
         // tail epochs with a horizon: a few thousand synchronous lineages need few slots, keep the footprint (2 MiB) inside L2
         // next to the tables. The tail without a horizon drifts apart in simulated time and needs the long memory of the full cache.
         bf.cache_mask = rp.dedup ? ((tail && !unbounded) ? std::min(full_cache_mask, (1u << 17) - 1u) : full_cache_mask) : 0u;
@@ -727,30 +733,30 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
             // disjoint windows of simulated time, so the concatenation is globally ordered (Water-Level, G.1 L2157-2187).
             const u32 nr = hc->n_rec;
             if (nr > rp.ring_cap) return fail(NECSIM_ERR_CAPACITY, "event ring overflowed: raise event_ring_capacity");
-            SimBuffers vb = bf;
-            vb.term_loc = bf.rec_loc; vb.term_k = bf.rec_k; vb.term_j = bf.rec_j; vb.term_f = bf.rec_f;
-            const u32 nb = (nr + NS_SORT_TILE - 1) / NS_SORT_TILE, g256 = (nr + 255) / 256;
-            iota_kernel<<<g256, 256, 0, st>>>(perm_a, nr);
-            u32 *src = perm_a, *dst = perm_b;
-            vb.k_base = ep.k_start;
-            const u32 kmax = k_stop - ep.k_start;   // sentinels carry k = k_stop
-            // radix passes over k (the bytes in use) and the leading bytes of f only; the few records that agree there are put in
-            // (f, loc, j) order by stream_ties_kernel
-            // default: the fewest leading bytes of f that leave about two records or fewer per prefix value (measured on C6: 3 bytes
-            // 347 ms, 4 bytes 369 ms, 2 bytes 691 ms -- short runs cost the tie pass less than another radix pass)
-            u32 fbytes = rp.stream_fbytes ? rp.stream_fbytes : 1u;
+            const u32 nb = (nr + NS_PAIR_TILE - 1) / NS_PAIR_TILE, g256 = (nr + 255) / 256;
+            const u32 kmax = k_stop - ep.k_start;   // (k - k_start) < kmax for every record; the sentinel key ~0 sorts last
+            // LSD radix passes over the key bytes that matter: the leading `fbytes` bytes of f (key bytes 5 - fbytes .. 4) and the
+            // bytes of k in use (key bytes 5 ..). Default: the fewest bytes of f that leave about two records or fewer per prefix value
+            // (short runs cost the tie pass less than another radix pass).
+            u32 fbytes = rp.stream_fbytes ? std::min(rp.stream_fbytes, 5u) : 1u;
             if (!rp.stream_fbytes)
-                while (fbytes < 6 && (double)nr > 2.0 * (double)kmax * (double)(1ull << (8 * fbytes))) ++fbytes;
-            for (u32 b = 14u - fbytes; b < 18; ++b) {
-                if (b >= 14 && (kmax >> (8 * (b - 14))) == 0) continue;
-                radix_hist_kernel<<<nb, 256, 0, st>>>(vb, src, nr, b, hist, nb, digit);
+                while (fbytes < 5 && (double)nr > 2.0 * (double)kmax * (double)(1ull << (8 * fbytes))) ++fbytes;
+            u64 *ksrc = key_a, *kdst = key_b;
+            u32 *isrc = NULL, *idst = perm_a, *iother = perm_b;
+            for (u32 b = 5u - fbytes; b < 8; ++b) {
+                if (b >= 5 && (kmax >> (8 * (b - 5))) == 0) continue;
+                pair_hist_kernel<<<nb, 256, 0, st>>>(ksrc, nr, 8 * b, hist, nb);
                 n_launch += 2 + scan_u32(hist, 256 * nb, scan_tmp, NULL, st);
-                radix_scatter_kernel<<<nb, 256, 0, st>>>(src, dst, nr, hist, nb, digit);
-                std::swap(src, dst);
+                pair_scatter_kernel<<<nb, 256, NS_PAIR_SMEM, st>>>(ksrc, isrc, kdst, idst, nr, 8 * b, hist, nb);
+                std::swap(ksrc, kdst);
+                isrc = idst; std::swap(idst, iother);
             }
-            stream_ties_kernel<<<g256, 256, 0, st>>>(vb, src, nr, k_stop, fbytes, flag);
+            // isrc / ksrc: sorted by the key prefix; idst: free scratch of the same size
+            CU(cudaMemsetAsync(&bf.ctr->n_long, 0, 4, st));
+            stream_ties_kernel<<<g256, 256, 0, st>>>(ksrc, isrc, bf.rec, nr, 8 * (5u - fbytes), flag, long_runs, &bf.ctr->n_long, long_cap);
+            stream_long_runs_kernel<<<(u32)scn->sm_count * 4u, 256, 0, st>>>(isrc, bf.rec, flag, long_runs, &bf.ctr->n_long, long_cap, idst);
             n_launch += scan_u32(flag, nr, scan_tmp, &bf.ctr->q_head, st) - 1;   // q_head reused: distinct events of the epoch
-            stream_write_kernel<<<g256, 256, 0, st>>>(vb, bf.rec_loc2, src, nr, flag, &bf.ctr->q_head, stream_n, rp.stream_cap, st_loc, st_k, st_j, st_f, st_l2);
+            stream_write_kernel<<<g256, 256, 0, st>>>(bf.rec, isrc, nr, flag, &bf.ctr->q_head, stream_n, rp.stream_cap, st_loc, st_k, st_j, st_f, st_l2);
             n_launch += 4;
             CU(cudaGetLastError());
             u32 heads = 0;
@@ -767,6 +773,7 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
     (void)params; (void)bytes;
 
     // ---- S6: speciation records -> species (sort / unique / rank), labels, abundances ----------------
+    bf.k_base = 0;
     const u32 n_spec = hc->n_spec;
     const u32 j_max = hc->j_max;
     u32 richness = 0;

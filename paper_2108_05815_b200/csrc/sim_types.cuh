@@ -57,6 +57,8 @@ struct SimCounters {
     u32 n_unfinished;
     u32 n_sampled;             // written by the init kernels
     u32 n_rec;                 // event-stream records written this epoch (NEXT-3)
+    u32 n_long;                // long runs of equal key prefix queued for stream_long_runs_kernel (NEXT-3)
+    u32 pad_;
     u64 n_events;              // events executed (raw)
     u64 n_culled;
     u64 resamples;
@@ -73,9 +75,11 @@ struct SimBuffers {
     u32 *term_loc, *term_k, *term_j, *steps, *parent, *spec_ring;
     u64 *term_f;
     uint8_t *state;            // 0 active, 1 speciated, 2 culled, 3 stopped by max_steps
-    // event-stream ring of one epoch (REC kernels): origin loc, k, j, offset f, parent loc (0xFFFFFFFF = speciation)
-    u32 *rec_loc, *rec_k, *rec_j, *rec_loc2;
-    u64 *rec_f;
+    // event-stream ring of one epoch (REC kernels): one 32-byte record per executed event, written with two 16-byte stores --
+    // rec[2i] = {origin loc, k, j, parent loc (0xFFFFFFFF = speciation)}, rec[2i+1] = {f lo, f hi, 0, 0} -- and its 64-bit time key
+    // rec_key[i] = (k - k_start) << 40 | f >> 8, which the per-epoch sort works on (coalesced (key, index) pairs, no gathers)
+    uint4 *rec;
+    u64 *rec_key;
     u32 rec_cap;
     u32 k_base;                // radix passes sort k - k_base (0 for the species table; the epoch's k_start for the stream ring)
     SimCounters *ctr;

@@ -251,12 +251,12 @@ __global__ void __launch_bounds__(256, 2) tail_kernel(const ScenarioDev sc, cons
     unsigned long long c_events = 0, c_culled = 0, c_resamples = 0, c_exact = 0;   // warp-uniform
     u32 w_resamples = 0;                                                        // fast rounds: flushed into c_resamples per lineage
     // event-stream ring (REC): the warp reserves ep.rec_chunk (<= NS_REC_CHUNK) slots at a time, so that it waits for an atomic's return once per
-    // chunk and not once per event; slots left over at the end are filled with sentinels (k = k_stop, which no event of the epoch has) the host-side pass drops
+    // chunk and not once per event; slots left over at the end get the sentinel key ~0, which sorts last and is dropped
     u32 rec_next = 0, rec_left = 0;
     auto record = [&](u32 r_loc, u32 r_k, u32 r_j, u64 r_f, u32 r_l2) {   // lane 0 only
         if (rec_left == 0u) { rec_next = atomicAdd(&bf.ctr->n_rec, ep.rec_chunk); rec_left = ep.rec_chunk; }
         const u32 ri = rec_next++; --rec_left;
-        if (ri < bf.rec_cap) { bf.rec_loc[ri] = r_loc; bf.rec_k[ri] = r_k; bf.rec_j[ri] = r_j; bf.rec_f[ri] = r_f; bf.rec_loc2[ri] = r_l2; }
+        if (ri < bf.rec_cap) store_record(bf, ri, r_loc, r_k, r_j, r_f, r_l2);
     };
 
     for (;;) {
@@ -593,7 +593,7 @@ __global__ void __launch_bounds__(256, 2) tail_kernel(const ScenarioDev sc, cons
         const u32 nx = __shfl_sync(NS_FULL, rec_next, 0), lf = __shfl_sync(NS_FULL, rec_left, 0);
         for (u32 q = lane; q < lf; q += 32u) {
             const u32 ri = nx + q;
-            if (ri < bf.rec_cap) { bf.rec_loc[ri] = 0xFFFFFFFFu; bf.rec_k[ri] = ep.k_stop; bf.rec_j[ri] = 0xFFFFFFFFu; bf.rec_f[ri] = ~0ull; bf.rec_loc2[ri] = 0xFFFFFFFFu; }
+            if (ri < bf.rec_cap) bf.rec_key[ri] = ~0ull;          // sentinel: sorts last, dropped
         }
     }
     if (lane == 0) {

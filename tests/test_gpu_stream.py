@@ -18,7 +18,7 @@ def test_stream_matches_oracle(O, kernel, sampler):
         sc = ns.Scenario(**kw)
         # stream_sort_bytes = 1: most records agree on the radix-sorted key prefix, so the order comes from the tie pass
         for knobs in (dict(), dict(event_ring_capacity=60_000, epoch_events=3000, dedup_log2_slots=8), dict(dedup=False, event_ring_capacity=2**22),
-                      dict(stream_sort_bytes=1), dict(stream_sort_bytes=6, event_ring_capacity=60_000, epoch_events=3000)):
+                      dict(stream_sort_bytes=1), dict(stream_sort_bytes=5, event_ring_capacity=60_000, epoch_events=3000)):
             if knobs.get("dedup") is False and cfg["nu"] < 1e-3:
                 continue
             got = sc.simulate(cfg["seed"], cfg["nu"], cfg["mask"], record_events=True, event_stream_capacity=2**21,
@@ -39,7 +39,7 @@ def test_stream_capacity_errors(O):
     with pytest.raises(ns.NecsimError):
         sc.simulate(cfg["seed"], cfg["nu"], cfg["mask"], record_events=True, event_ring_capacity=64)
     with pytest.raises(ns.NecsimError):
-        sc.simulate(cfg["seed"], cfg["nu"], cfg["mask"], record_events=True, stream_sort_bytes=7)
+        sc.simulate(cfg["seed"], cfg["nu"], cfg["mask"], record_events=True, stream_sort_bytes=6)
     out = sc.simulate(cfg["seed"], cfg["nu"], cfg["mask"])        # the handle still works
     assert out["richness"] > 0
     sc.close()
