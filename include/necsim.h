@@ -85,7 +85,11 @@ typedef struct necsim_sim_params {
                                   half the cache slots and never fewer than 64 events per active lineage; the tail kernel runs as
                                   one launch without a horizon (with record_events: x64 per epoch, capped by the ring) */
     uint64_t max_steps;        /* 0 = unlimited; else a lineage stops after this many executed events
-                                  ("unfinished": label 0xFFFFFFFF) -- the MODE-T throughput workload */
+                                  ("unfinished": label 0xFFFFFFFF) -- the MODE-T throughput workload. With the duplicate
+                                  culling on, WHICH lineages reach the cap depends on the launch shape (the cache is lossy: a
+                                  lineage the oracle culls at its first shared event may run on here and hit the cap first), so
+                                  only the labels of lineages with state 1 are reproducible then; with dedup = 2 (off) every
+                                  per-lineage record is (tests/test_gpu_parity.py) */
     uint32_t tail_threshold;   /* switch to the low-latency tail kernel (one lineage per warp) when active lineages <= this;
                                   0 = default (four lineages per resident warp) */
     uint32_t dedup_probe;      /* 0 = default (4); else 1 + log2 of the probe period: 1 = every event, 2 = every 2nd, 3 = every 4th,

@@ -198,8 +198,8 @@ __device__ __forceinline__ void fast_slot_a(const ScenarioDev &sc, const GaussLu
         yy = min(yy, yy - sc.height); yy = min(yy, yy - sc.height);
         c2 = (yy << 16) | xx;
         if (COMPACT) {
-            const uint2 hb = ldg_v2_ordered(&sc.hab64[yy * sc.nbx + (xx >> 5)]);
-            if (PERCELL) cs = ldg_v2_ordered(&sc.scale[yy * sc.width + xx]);
+            const uint2 hb = __ldg(&sc.hab64[yy * sc.nbx + (xx >> 5)]);
+            if (PERCELL) cs = __ldg(&sc.scale[yy * sc.width + xx]);
             const u32 D = sc.compact_deme;
             const u32 idx = (D == 1u) ? 0u : mulhi64_u32_parts(xi_lo, xi_hi, D);     // in flight with the gather
             const u32 bit = 1u << (xx & 31u);
@@ -245,7 +245,7 @@ __global__ void __launch_bounds__(256, 2) tail_kernel(const ScenarioDev sc, cons
     const u64 sp_a_add = (KIND == 3 ? (u64)sp_q : 0ull) * NS_GAMMA;                       // slot A: attempt sp_q
     const u64 sp_b_xor = sp_q == 0 ? 0ull : sp_q == 1 ? NS_L_SPEC : sp_q == 2 ? NS_L_INDEX : NS_L_MIGR;   // slot B
     const bool sp_in_k = lane < 4u * NS_SPEC_NJ;
-    const bool sp_add4 = sp_in_k && lane >= 4u, sp_add8 = sp_in_k && lane >= 8u, sp_add16 = sp_in_k && lane >= 16u;
+    const bool sp_add4 = sp_in_k && lane >= 4u, sp_add8 = sp_in_k && lane >= 8u, sp_add12 = sp_in_k && lane >= 12u, sp_add16 = sp_in_k && lane >= 16u;
     const u32 kmask = (1u << (4u * NS_SPEC_NJ)) - 1u;
     const u32 qb = lane & ~3u;
     unsigned long long c_events = 0, c_culled = 0, c_resamples = 0, c_exact = 0;   // warp-uniform
@@ -326,9 +326,15 @@ __global__ void __launch_bounds__(256, 2) tail_kernel(const ScenarioDev sc, cons
                     // (the draw is tied to the target cell of slot A by an OR with zero: the table gathers, which have the longest latency,
                     // are then issued before this chain starts)
                     float a = sp_q == 0u ? approx_exp_time(ubh | (c2o & ep.zero), ln2_over_mu) : 0.0f;
-                    { const float y = __shfl_up_sync(NS_FULL, a, 4); if (sp_add4) a += y; }
-                    { const float y = __shfl_up_sync(NS_FULL, a, 8); if (sp_add8) a += y; }
-                    { const float y = __shfl_up_sync(NS_FULL, a, 16); if (sp_add16) a += y; }
+                    {   // five partial sums in two shuffle levels: a_j + a_{j-1} + a_{j-2}, then + the same sum three candidates below
+                        const float y1 = __shfl_up_sync(NS_FULL, a, 4), y2 = __shfl_up_sync(NS_FULL, a, 8);
+                        float b3 = a;
+                        if (sp_add4) b3 += y1;
+                        if (sp_add8) b3 += y2;
+                        const float y3 = __shfl_up_sync(NS_FULL, b3, 12);
+                        a = b3;
+                        if (sp_add12) a += y3;
+                    }
                     const float mc = margin + fm_last;
                     const bool ins = a < 1.0f - margin, outs = a > 1.0f + margin;
                     bool aft = a > fa_last + mc, bef = a < fa_last - mc;
