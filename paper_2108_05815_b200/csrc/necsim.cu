@@ -213,7 +213,7 @@ static int scenario_layout_static(const necsim_scenario_desc *d, ScenarioLayout 
         else for (u32 c = 0; c < L.ncells && same; ++c) if (d->deme[c]) { if (!D) D = d->deme[c]; else same = (d->deme[c] == D); }
         if (same && D && allow_compact) {
             L.compact = true; L.compact_deme = D; L.nbx = (d->width + 31u) / 32u;
-            L.off_hab64 = off; off = align256(off + 8 * (size_t)L.nbx * d->height);
+            L.off_hab64 = off; off = align256(off + 8 * (size_t)L.nbx * 16u * ((d->height + 15u) / 16u));
         }
     }
     L.total = off ? off : 256;
@@ -352,12 +352,12 @@ static int create_scenario_impl(const necsim_scenario_desc *d_caller, void *d_wo
             CU(cudaStreamSynchronize(st));
             sd.gauss = (const u32 *)(base + L.off_gauss); sd.R = L.R; sd.gauss_len = L.gauss_len;
             if (L.compact) {   // {habitat mask, prefix at the block's first cell} per 32-cell block of a row
-                std::vector<uint2> hb((size_t)L.nbx * d->height);
+                std::vector<uint2> hb((size_t)L.nbx * 16u * ((d->height + 15u) / 16u), make_uint2(0u, 0u));   // tiled, see sim_types.cuh
                 for (u32 y = 0; y < d->height; ++y)
                     for (u32 b = 0; b < L.nbx; ++b) {
                         u32 m = 0;
                         for (u32 t = 0; t < 32u && b * 32u + t < d->width; ++t) if (hab8[(size_t)y * d->width + b * 32u + t]) m |= 1u << t;
-                        hb[(size_t)y * L.nbx + b] = make_uint2(m, prefix[(size_t)y * d->width + b * 32u]);
+                        hb[(((size_t)(y >> 4) * L.nbx + b) << 4) | (y & 15u)] = make_uint2(m, prefix[(size_t)y * d->width + b * 32u]);
                     }
                 CU(cudaMemcpyAsync(base + L.off_hab64, hb.data(), 8 * hb.size(), cudaMemcpyHostToDevice, st));
                 CU(cudaStreamSynchronize(st));

@@ -95,6 +95,11 @@ __device__ __forceinline__ u32 cell_deme_at(const ScenarioDev &sc, u32 cell, u32
     return d;
 }
 
+// entry of the compact habitat table that holds cell (xx, yy): the table is tiled, 16 rows of one 32-cell block per 128-byte line
+// (sim_types.cuh), so that the targets of one origin's dispersal attempts fall into a handful of lines
+__device__ __forceinline__ u32 hab64_index(const ScenarioDev &sc, u32 xx, u32 yy) {
+    return ((((yy >> 4) * sc.nbx + (xx >> 5)) << 4) | (yy & 15u));
+}
 // cell of an indexed location: last cell with prefix[cell] <= loc (that cell has deme > 0)
 __device__ __forceinline__ u32 cell_of_loc(const ScenarioDev &sc, u32 loc) {
     if (sc.kind == 0 || sc.kind == 1) return 0;      // non-spatial; implicit: only the local community is sampled
@@ -433,7 +438,7 @@ __global__ void __launch_bounds__(256) simulate_kernel(const ScenarioDev sc, con
                 const u32 yy = wrap_add(cell >> 16, gauss_disp(gl, (u32)x), sc.height);
                 u32 d, pfx = 0;
                 if (COMPACT) {   // deme and prefix of the target from one 8-byte read of the compact habitat table
-                    const uint2 hb = __ldg(&sc.hab64[yy * sc.nbx + (xx >> 5)]);
+                    const uint2 hb = __ldg(&sc.hab64[hab64_index(sc, xx, yy)]);
                     const u32 bit = 1u << (xx & 31u);
                     d = (hb.x & bit) ? sc.compact_deme : 0u;
                     pfx = hb.y + sc.compact_deme * (u32)__popc(hb.x & (bit - 1u));

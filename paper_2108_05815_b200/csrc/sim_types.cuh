@@ -23,7 +23,10 @@ struct ScenarioDev {
     // 32-cell block of a row {habitat bit mask, prefix sum at the block's first cell}. deme and prefix of a cell come out of
     // ONE 8-byte read: deme = bit ? compact_deme : 0, prefix = base + compact_deme * popc(mask below the bit). 128x smaller
     // than hab8 + prefix (C5: 4 MB instead of 84 MB), so a lineage's neighbourhood stays in L1 and the table in L2.
-    const uint2 *hab64;        // [height * nbx]
+    // Tiled: entry of block b of row y at ((y / 16) * nbx + b) * 16 + y % 16, i.e. one 128-byte line holds the same block of 16
+    // consecutive rows. The 32 gathers of a tail round (targets within a few sigma of one origin) then touch a handful of lines
+    // instead of one line per row: a warp's gather is served line by line.
+    const uint2 *hab64;        // [ceil(height / 16) * nbx * 16]
     u32 nbx;                   // 32-cell blocks per row = ceil(width / 32)
     u32 compact_deme;
     const uint2 *scale;        // [ncells] (Cm, sh) when per_cell_turnover

@@ -129,7 +129,7 @@ __device__ __forceinline__ void gauss_target(const ScenarioDev &sc, const GaussL
     const u32 yy = wrap_add(y0, dy, sc.height);
     c2 = (yy << 16) | xx;
     if (COMPACT) {
-        const uint2 hb = ldg_v2_ordered(&sc.hab64[yy * sc.nbx + (xx >> 5)]);
+        const uint2 hb = ldg_v2_ordered(&sc.hab64[hab64_index(sc, xx, yy)]);
         if (PERCELL) {
             const u32 ci = yy * sc.width + xx;
             if (SAMP == 0) cs = ldg_v2_ordered(&sc.scale[ci]);
@@ -198,7 +198,7 @@ __device__ __forceinline__ void fast_slot_a(const ScenarioDev &sc, const GaussLu
         yy = min(yy, yy - sc.height); yy = min(yy, yy - sc.height);
         c2 = (yy << 16) | xx;
         if (COMPACT) {
-            const uint2 hb = __ldg(&sc.hab64[yy * sc.nbx + (xx >> 5)]);
+            const uint2 hb = __ldg(&sc.hab64[hab64_index(sc, xx, yy)]);
             if (PERCELL) cs = __ldg(&sc.scale[yy * sc.width + xx]);
             const u32 D = sc.compact_deme;
             const u32 idx = (D == 1u) ? 0u : mulhi64_u32_parts(xi_lo, xi_hi, D);     // in flight with the gather
