@@ -163,8 +163,8 @@ __device__ __forceinline__ u32 mulhi64_u32_parts(u32 xlo, u32 xhi, u32 d) {
 // xi = the index draw of the lane's candidate. Loads are issued before anything consumes them.
 template <int KIND, bool PERCELL, bool COMPACT>
 __device__ __forceinline__ void fast_slot_a(const ScenarioDev &sc, const GaussLut &gl, u32 sp_q, u32 lane, u32 bm, u32 cell, u32 kc, u64 ua, u32 xi_lo, u32 xi_hi,
-                                            u32 &loc2, u32 &c2, uint2 &cs, bool &acc, bool &bad) {
-    bad = false;
+                                            u32 &loc2, u32 &c2, uint2 &cs, bool &acc, bool &bad, u32 &tie) {
+    bad = false; tie = 0u;
     if (KIND == 0) {
         loc2 = mulhi64_u32(ua, (u32)sc.n_locations); c2 = 0u; acc = sp_q == 0u;
     } else if (KIND == 1) {
@@ -205,6 +205,7 @@ __device__ __forceinline__ void fast_slot_a(const ScenarioDev &sc, const GaussLu
             const u32 bit = 1u << (xx & 31u);
             acc = (hb.x & bit) != 0u;
             loc2 = hb.y + D * (u32)__popc(hb.x & (bit - 1u)) + idx;
+            tie = hb.x;
         } else {
             const u32 ci = yy * sc.width + xx;
             const u32 pf = ldg_u32_ordered(&sc.prefix[ci]);
@@ -281,14 +282,15 @@ __global__ void __launch_bounds__(256, 2) tail_kernel(const ScenarioDev sc, cons
         // pending duplicate check: the exchange of the last probing event (lane 0 holds its result)
         bool pend = false, p_T_known = true;
         u64 pold_lo = ~0ull, pold_hi = ~0ull;
+        u32 p_lane = 0;                                    // the lane that issued the pending exchange and holds its result (warp-uniform)
         u32 p_loc = 0, p_k = 0, p_j = 0, p_l2 = 0;
         u64 p_T = 0;
         // consumes the pending exchange: true = this lineage is a duplicate at the pending event (culled, recorded)
         auto resolve_pending = [&]() -> bool {
             if (!DEDUP || !pend) return false;
             pend = false;
-            const u32 ox = __shfl_sync(NS_FULL, (u32)pold_lo, 0), oy = __shfl_sync(NS_FULL, (u32)(pold_lo >> 32), 0);
-            const u32 oz = __shfl_sync(NS_FULL, (u32)pold_hi, 0), ow = __shfl_sync(NS_FULL, (u32)(pold_hi >> 32), 0);
+            const u32 ox = __shfl_sync(NS_FULL, (u32)pold_lo, (int)p_lane), oy = __shfl_sync(NS_FULL, (u32)(pold_lo >> 32), (int)p_lane);
+            const u32 oz = __shfl_sync(NS_FULL, (u32)pold_hi, (int)p_lane), ow = __shfl_sync(NS_FULL, (u32)(pold_hi >> 32), (int)p_lane);
             if (ox == p_loc && oy == p_k && oz == p_j && ow != id) {   // another lineage executed it first (L687, L697)
                 if (FAST && !p_T_known) { const uint2 pr = rate_of_loc<PERCELL>(sc, p_loc); p_T = exact_offset(ep.key, smt, p_loc, p_k, p_j, pr.x, pr.y); }
                 if (lane == 0) {
@@ -313,19 +315,33 @@ __global__ void __launch_bounds__(256, 2) tail_kernel(const ScenarioDev sc, cons
                 // ---- fast rounds: the search in binary32 with a margin (see approx_exp_time), every candidate's outcome from its own four
                 // lanes. The loop commits clean events (99 %: candidate in the set, unambiguous comparisons, an attempt accepted, no
                 // speciation, no duplicate, no step cap) and leaves at the first round that is not, which the general code below redoes.
+                // A duplicate check still pending from the general code is settled first (rare: the loop is entered once per ~40 events and
+                // one event in eight probes). Inside the loop the pending event is then always the last committed one, (e_loc, k, e_j), its
+                // result sits in lane p_lane, and the step count includes it (steps_all; `steps` counts confirmed events only).
+                if (DEDUP && pend) { if (resolve_pending()) break; }
+                u32 steps_all = steps;
+                bool lpend = false;
                 for (;;) {
                     const u64 X = prime(ep.key, loc, k + sp_dk) + sp_cand_add;
                     u64 ua, ub;
                     hashF2((X ^ NS_L_DISP) + sp_a_add, X ^ sp_b_xor, ua, ub);
+                    // duplicate check of the candidate, decided per lane ahead of the selection: whether its event probes the cache, and where.
+                    // The winner's first lane issues the exchange itself and keeps the result (no shuffle of X, no hash after the vote).
+                    const u32 ch = DEDUP ? cache_hash(X) : 0u;
+                    const u32 prm = DEDUP ? __ballot_sync(NS_FULL, cache_probes(ch, ep.probe_mask)) : 0u;
                     const u32 ubh = (u32)(ub >> 32);
+                    ua |= (u64)(ubh & ep.zero);       // keeps the two evaluations interleaved (slot A's chain is the longer one and would go first)
                     const u32 bm = __ballot_sync(NS_FULL, bern(ub, sp_q == 3u ? ep.thr_m : ep.thr_nu));   // bit 4c+1: speciation, 4c+3: migration
                     const u32 xi_lo = __shfl_sync(NS_FULL, (u32)ub, (int)(qb + 2u)), xi_hi = __shfl_sync(NS_FULL, ubh, (int)(qb + 2u));
-                    u32 loc2o, c2o; uint2 cso = make_uint2(Cm, sh); bool acc, bad;
-                    fast_slot_a<KIND, PERCELL, COMPACT>(sc, gl, sp_q, lane, bm, cell, k + sp_dk, ua, xi_lo, xi_hi, loc2o, c2o, cso, acc, bad);
+                    u32 loc2o, c2o, tie; uint2 cso = make_uint2(Cm, sh); bool acc, bad;
+                    fast_slot_a<KIND, PERCELL, COMPACT>(sc, gl, sp_q, lane, bm, cell, k + sp_dk, ua, xi_lo, xi_hi, loc2o, c2o, cso, acc, bad, tie);
                     // slot B of the lanes with sp_q == 0: approximate offsets of the candidates (partial sums over the points of interval k)
                     // (the draw is tied to the target cell of slot A by an OR with zero: the table gathers, which have the longest latency,
                     // are then issued before this chain starts)
                     float a = sp_q == 0u ? approx_exp_time(ubh | (c2o & ep.zero), ln2_over_mu) : 0.0f;
+                    // (the partial sums are tied to the gathered table entry by an OR with zero: ptxas otherwise places the gather, whose
+                    // consumers come late, behind the whole shuffle / compare / ballot chain, and its latency ends up on the lineage's chain
+                    // instead of under it. With the tie the gather is issued first and the logarithms run while it is in flight.)
                     {   // five partial sums in two shuffle levels: a_j + a_{j-1} + a_{j-2}, then + the same sum three candidates below
                         const float y1 = __shfl_up_sync(NS_FULL, a, 4), y2 = __shfl_up_sync(NS_FULL, a, 8);
                         float b3 = a;
@@ -335,6 +351,7 @@ __global__ void __launch_bounds__(256, 2) tail_kernel(const ScenarioDev sc, cons
                         a = b3;
                         if (sp_add12) a += y3;
                     }
+                    if (COMPACT) a = __uint_as_float(__float_as_uint(a) | (tie & ep.zero));
                     const float mc = margin + fm_last;
                     const bool ins = a < 1.0f - margin, outs = a > 1.0f + margin;
                     bool aft = a > fa_last + mc, bef = a < fa_last - mc;
@@ -347,11 +364,10 @@ __global__ void __launch_bounds__(256, 2) tail_kernel(const ScenarioDev sc, cons
                     const u32 evm = __ballot_sync(NS_FULL, sp_q == 0u && ins && (sp_in_k ? aft : kvalid));
                     const u32 crm = __ballot_sync(NS_FULL, sp_q == 0u && outs);
                     const u32 okm = __ballot_sync(NS_FULL, acc);
-                    // trouble: an ambiguous comparison anywhere, or an undetermined target
-                    // trouble: an ambiguous comparison anywhere, or (lane 0, which holds the result of the pending
-                    // exchange) a match there: another lineage executed the pending event first and this one is a duplicate
+                    // trouble: an ambiguous comparison anywhere, or (the lane that holds the result of the pending exchange) a match there:
+                    // another lineage executed the pending event first and this one is a duplicate
                     bool culled = false;
-                    if (DEDUP) culled = lane == 0 && pend && (u32)pold_lo == p_loc && (u32)(pold_lo >> 32) == p_k && (u32)pold_hi == p_j && (u32)(pold_hi >> 32) != id;
+                    if (DEDUP) culled = lane == p_lane && lpend && (u32)pold_lo == e_loc && (u32)(pold_lo >> 32) == k && (u32)pold_hi == e_j && (u32)(pold_hi >> 32) != id;
                     const u32 trm = __ballot_sync(NS_FULL, (sp_q == 0u && amb) || culled);
                     const u32 badm = KIND == 3 ? __ballot_sync(NS_FULL, bad) : 0u;
                     // every candidate's outcome: the first accepted attempt of its four lanes (the sequential algorithm's choice, R16)
@@ -366,7 +382,7 @@ __global__ void __launch_bounds__(256, 2) tail_kernel(const ScenarioDev sc, cons
                     const u32 wl = (u32)first_bit(wm | 0x80000000u);
                     const u32 q4 = 15u << wl;
                     const u32 spec_w = (KIND == 1 && cell == 0) ? 0u : ((bm >> wl) & 2u);
-                    const u32 steps_e = steps + (pend ? 2u : 1u);       // step count after this event
+                    const u32 steps_e = steps_all + 1u;                 // step count after this event
                     // clean: a winner, no trouble at the time lanes or in the winner's lanes, an attempt accepted, no speciation, no step cap
                     const bool clean = wm != 0u && ((trm & 0x11111111u) | (badm & q4) | spec_w) == 0u && (okm & q4) != 0u && steps_e < cap_at;
                     if (!__all_sync(NS_FULL, clean)) break;
@@ -377,15 +393,12 @@ __global__ void __launch_bounds__(256, 2) tail_kernel(const ScenarioDev sc, cons
                     const u32 loc2 = __shfl_sync(NS_FULL, loc2q, (int)wl), cell2 = __shfl_sync(NS_FULL, cq, (int)wl);
                     const float a_w = __shfl_sync(NS_FULL, a, (int)wl);
                     if (KIND == 3) w_resamples += (u32)first_bit((okm >> wl) & 15u);
-                    if (DEDUP) {
-                        if (pend) { steps++; pend = false; }                      // the pending event was really executed
-                        const u64 Xw = __shfl_sync(NS_FULL, X, (int)wl);
-                        const u32 h = cache_hash(Xw);
-                        const bool probes = cache_probes(h, ep.probe_mask);
-                        atomic_exch_128_if(probes && lane == 0, &bf.cache[h & bf.cache_mask], make_uint4(loc, k2, j2, id), pold_lo, pold_hi);
-                        if (probes) { p_loc = loc; p_k = k2; p_j = j2; p_T_known = false; pend = true; }
-                        else steps++;
-                    } else steps++;
+                    steps_all = steps_e;
+                    if (DEDUP) {                                       // (a clean round has confirmed the event that was pending)
+                        lpend = (prm >> wl) & 1u;
+                        atomic_exch_128_if(lpend && lane == wl, &bf.cache[ch & bf.cache_mask], make_uint4(loc, k2, j2, id), pold_lo, pold_hi);
+                        if (lpend) p_lane = wl;
+                    }
                     e_loc = loc; e_j = j2; e_Cm = Cm; e_sh = sh; f_exact = false; fa_last = a_w; fm_last = margin;
                     if (PERCELL) {
                         Cm = __shfl_sync(NS_FULL, Cmq, (int)wl); sh = __shfl_sync(NS_FULL, shq, (int)wl);
@@ -394,6 +407,12 @@ __global__ void __launch_bounds__(256, 2) tail_kernel(const ScenarioDev sc, cons
                     }
                     k = k2; loc = loc2; cell = cell2;
                 }
+                steps = steps_all;
+                if (DEDUP && lpend) {          // hand the pending check over to the general code, which keeps the result in lane 0
+                    steps = steps_all - 1u; pend = true; p_loc = e_loc; p_k = k; p_j = e_j; p_T_known = false;
+                    pold_lo = __shfl_sync(NS_FULL, pold_lo, (int)p_lane); pold_hi = __shfl_sync(NS_FULL, pold_hi, (int)p_lane);
+                }
+                p_lane = 0u;
                 // the round that was not clean is done below in exact arithmetic, from the exact lower bound
                 if (!f_exact) { f_last = (i64)exact_offset(ep.key, smt, e_loc, k, e_j, e_Cm, e_sh); f_exact = true; }
                 c_exact++;
