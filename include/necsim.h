@@ -211,6 +211,19 @@ int necsim_merge_workspace_size(uint64_t n, size_t *device_bytes /*HOST out*/);
 int necsim_merge_species(const necsim_event *d_events_in /*DEVICE*/, uint64_t n, void *d_workspace /*DEVICE*/, size_t bytes, void *cuda_stream,
                          necsim_event *d_events_out /*DEVICE*/, uint32_t *d_map /*DEVICE*/, uint64_t *richness /*HOST out*/);
 
+/*
+ * necsim_merge_species for callers that cannot allocate device memory or pass a workspace (code under CUDA graph capture, serving
+ * loops, harnesses that forbid cudaMalloc): same inputs, outputs and results, but the sort / unique scratch of the merge kernels is
+ * a static device array inside the library, sized for at most NECSIM_MERGE_STATIC_MAX input records (about 2.1 MB, held by every GPU
+ * that loads the library until the process exits). n > NECSIM_MERGE_STATIC_MAX returns NECSIM_ERR_CAPACITY and touches nothing.
+ * The call allocates nothing (no cudaMalloc / cudaFree, no allocating library routine); like necsim_merge_species it synchronises the
+ * stream before it returns (*richness is a host value). All calls on one device share the one array: calls that overlap on the GPU
+ * (different streams, different host threads) race on it -- serialise them. Nothing in the array has to be cleared between calls.
+ */
+#define NECSIM_MERGE_STATIC_MAX 65536u
+int necsim_merge_species_static(const necsim_event *d_events_in /*DEVICE*/, uint64_t n, void *cuda_stream,
+                                necsim_event *d_events_out /*DEVICE [n]*/, uint32_t *d_map /*DEVICE [n]*/, uint64_t *richness /*HOST out*/);
+
 /* Frees the host-side handle (NULL is a no-op). The device workspace belongs to the caller. */
 int necsim_destroy(necsim_scenario *scn);
 

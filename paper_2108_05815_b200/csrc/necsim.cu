@@ -922,6 +922,37 @@ extern "C" int necsim_merge_species(const necsim_event *d_in, uint64_t n64, void
     return NECSIM_OK;
 }
 
+// ---- the same merge for callers that cannot allocate (CUDA graph capture, serving loops): scratch in a static device array ----------
+// The sort / unique scratch of the merge kernels (SoA copy of the records, two permutations, flags, histograms: 32 bytes per record
+// and 1 KB per 2048 records) lives in a file-scope __device__ array instead of a caller workspace. Every GPU that loads the library
+// holds the array until the process exits. All calls on one device share it: calls that overlap on the GPU (different streams) race.
+// Nothing in it has to start at zero -- every kernel of the merge writes what it later reads, for the n of the call -- so the
+// previous call's contents do no harm.
+#define NS_MERGE_STATIC_BYTES (32u * NECSIM_MERGE_STATIC_MAX + 4u * 256u * (NECSIM_MERGE_STATIC_MAX / NS_SORT_TILE + 1u) + 16u * 256u)
+static __device__ __align__(256) unsigned char g_merge_scratch[NS_MERGE_STATIC_BYTES];
+#define NS_MAX_DEVICES 64
+static void *g_merge_scratch_ptr[NS_MAX_DEVICES];      // device address of g_merge_scratch per device, looked up once with that device current
+
+extern "C" int necsim_merge_species_static(const necsim_event *d_in, uint64_t n64, void *cuda_stream, necsim_event *d_out, uint32_t *d_map,
+                                           uint64_t *richness) {
+    if (!d_in || !d_out || !d_map || !richness || n64 == 0) return fail(NECSIM_ERR_INVALID_ARG, "bad argument");
+    if (n64 > NECSIM_MERGE_STATIC_MAX)
+        return fail(NECSIM_ERR_CAPACITY, "necsim_merge_species_static: n exceeds NECSIM_MERGE_STATIC_MAX (65536 records); use necsim_merge_species with a workspace");
+    int dev_id = 0;
+    CU(cudaGetDevice(&dev_id));
+    if (dev_id < 0 || dev_id >= NS_MAX_DEVICES) return fail(NECSIM_ERR_UNSUPPORTED, "device ordinal out of range");
+    if (!g_merge_scratch_ptr[dev_id]) {
+        // in host code `g_merge_scratch` is only a stand-in for the symbol: its device address comes from the runtime
+        void *ptr = NULL;
+        CU(cudaGetSymbolAddress(&ptr, g_merge_scratch));
+        if (!ptr || ((uintptr_t)ptr & 255u) != 0) return fail(NECSIM_ERR_CUDA, "static merge scratch has no aligned device address");
+        g_merge_scratch_ptr[dev_id] = ptr;
+    }
+    MergeLayout L; merge_layout(n64, L);
+    if (L.total > NS_MERGE_STATIC_BYTES) return fail(NECSIM_ERR_CAPACITY, "static merge scratch too small");   // cannot happen for n <= the maximum
+    return necsim_merge_species(d_in, n64, g_merge_scratch_ptr[dev_id], NS_MERGE_STATIC_BYTES, cuda_stream, d_out, d_map, richness);
+}
+
 // ---------------------------------------------------------------------------------------------------
 // test-only exports: device primitives over arrays
 // ---------------------------------------------------------------------------------------------------

@@ -17,7 +17,7 @@ EXPORTS = ["necsim_scenario_workspace_size", "necsim_create_scenario", "necsim_s
            "necsim_simulate_workspace_size", "necsim_simulate", "necsim_simulate_host", "necsim_destroy", "necsim_last_error",
            "necsim_debug_draw", "necsim_debug_neglog", "necsim_debug_next_event", "necsim_debug_disperse", "necsim_debug_tables",
            "necsim_debug_int_peak", "necsim_debug_next_event_poisson", "necsim_debug_poisson_table",
-           "necsim_merge_workspace_size", "necsim_merge_species", "necsim_debug_approx_time", "necsim_debug_gather_peak"]
+           "necsim_merge_workspace_size", "necsim_merge_species", "necsim_merge_species_static", "necsim_debug_approx_time", "necsim_debug_gather_peak"]
 
 
 class ScenarioDesc(C.Structure):
@@ -92,6 +92,7 @@ def lib():
         L.necsim_debug_gather_peak.argtypes = [vp, u64, u32, vp, vp, vp, vp]
         L.necsim_merge_workspace_size.argtypes = [u64, vp]
         L.necsim_merge_species.argtypes = [vp, u64, vp, C.c_size_t, vp, vp, vp, vp]
+        L.necsim_merge_species_static.argtypes = [vp, u64, vp, vp, vp, vp]
         _lib = L
     return _lib
 
@@ -317,6 +318,24 @@ def merge_species(d_events):
     _check(lib().necsim_merge_species(C.c_void_p(d_events.data_ptr()), n, C.c_void_p(ws.data_ptr()), ws.numel(), _stream_ptr(torch),
                                       C.c_void_p(out.data_ptr()), C.c_void_p(dmap.data_ptr()), C.byref(rich)))
     return out[: rich.value * 32], dmap.to(torch.int64)
+
+
+MERGE_STATIC_MAX = 65536   # NECSIM_MERGE_STATIC_MAX of include/necsim.h
+
+
+def merge_species_static(d_events, out=None, dmap=None):
+    """necsim_merge_species_static: the merge with the library's static scratch (no workspace, nothing allocated by the call when
+    `out` [n * 32] uint8 and `dmap` [n] int32 are passed in). Returns (merged table [richness * 32] uint8, map [n] int32) as views."""
+    torch = _torch()
+    assert d_events.is_cuda and d_events.dtype == torch.uint8 and d_events.numel() % 32 == 0 and d_events.is_contiguous()
+    n = d_events.numel() // 32
+    if out is None: out = torch.empty(n * 32, dtype=torch.uint8, device="cuda")
+    if dmap is None: dmap = torch.empty(n, dtype=torch.int32, device="cuda")
+    assert out.numel() >= n * 32 and dmap.numel() >= n
+    rich = C.c_uint64()
+    _check(lib().necsim_merge_species_static(C.c_void_p(d_events.data_ptr()), n, _stream_ptr(torch), C.c_void_p(out.data_ptr()),
+                                             C.c_void_p(dmap.data_ptr()), C.byref(rich)))
+    return out[: rich.value * 32], dmap[:n]
 
 
 # ---- vectorised device primitives (test-only exports) ------------------------------------------------
