@@ -280,29 +280,39 @@ __global__ void __launch_bounds__(256) pair_hist_kernel(const u64 *__restrict__ 
     __syncthreads();
     hist[threadIdx.x * nblocks + blockIdx.x] = h[threadIdx.x];
 }
-// stable scatter of the pairs (after an exclusive scan of hist); idx_in == NULL: the identity (first pass). A warp ranks its 512
+// stable scatter of the pairs (after an exclusive scan of hist); idx_in == NULL: the identity (first pass). A warp ranks its 256
 // consecutive pairs against its own digit counters, the block orders the tile by digit in shared memory, and every digit's pairs
 // are then written to their place in one coalesced run (a direct scatter from registers writes 8 useful bytes per 32-byte sector).
-__global__ void __launch_bounds__(256) pair_scatter_kernel(const u64 *__restrict__ keys_in, const u32 *__restrict__ idx_in, u64 *__restrict__ keys_out,
-                                                           u32 *__restrict__ idx_out, u32 n, u32 shift, const u32 *__restrict__ hist, u32 nblocks) {
+// 512 threads x 8 pairs: with 16 pairs per thread in registers the kernel ran two blocks of 256 threads per SM (25 % of the warp slots,
+// 14 % of the issue slots, 25 % of the HBM peak: ncu, profiles/r2_ncu_stream_kernels_c6.md); now three blocks of 512.
+#define NS_PAIR_THREADS 512u
+#define NS_PAIR_WARPS (NS_PAIR_THREADS / 32u)
+#define NS_PAIR_ROUNDS (NS_PAIR_TILE / NS_PAIR_THREADS)
+__global__ void __launch_bounds__(NS_PAIR_THREADS, 3) pair_scatter_kernel(const u64 *__restrict__ keys_in, const u32 *__restrict__ idx_in, u64 *__restrict__ keys_out,
+                                                                          u32 *__restrict__ idx_out, u32 n, u32 shift, const u32 *__restrict__ hist, u32 nblocks) {
     extern __shared__ unsigned char pair_smem[];
     u64 *skey = (u64 *)pair_smem;                           // [NS_PAIR_TILE]
     u32 *sidx = (u32 *)(skey + NS_PAIR_TILE);               // [NS_PAIR_TILE]
-    u32 (*wcount)[256] = (u32 (*)[256])(sidx + NS_PAIR_TILE);   // [8][256]
-    u32 *bdo = (u32 *)(wcount + 8);                         // [256] first position of a digit inside the ordered tile
+    u32 (*wcount)[256] = (u32 (*)[256])(sidx + NS_PAIR_TILE);   // [NS_PAIR_WARPS][256]
+    u32 *bdo = (u32 *)(wcount + NS_PAIR_WARPS);             // [256] first position of a digit inside the ordered tile
     u32 *gbase = bdo + 256;                                 // [256] global position of the tile's first pair of a digit
+    u32 *wtot = gbase + 256;                                // [8]
     const u32 lane = threadIdx.x & 31u, w = threadIdx.x >> 5;
-    for (u32 ww = 0; ww < 8; ++ww) wcount[ww][threadIdx.x] = 0;
+    for (u32 t = threadIdx.x; t < NS_PAIR_WARPS * 256u; t += NS_PAIR_THREADS) (&wcount[0][0])[t] = 0;
     __syncthreads();
-    const u32 tile0 = blockIdx.x * NS_PAIR_TILE, start = tile0 + w * (NS_PAIR_TILE / 8u);
-    u64 key[16];
-    u32 item[16], dr[16];                               // dr = digit | rank inside the warp's 512 positions << 9
+    const u32 tile0 = blockIdx.x * NS_PAIR_TILE, start = tile0 + w * (NS_PAIR_TILE / NS_PAIR_WARPS);
+    u64 key[NS_PAIR_ROUNDS];
+    u32 item[NS_PAIR_ROUNDS], dr[NS_PAIR_ROUNDS];       // dr = digit | rank inside the warp's 256 positions << 9
 #pragma unroll
-    for (u32 r = 0; r < 16; ++r) {
+    for (u32 r = 0; r < NS_PAIR_ROUNDS; ++r) {          // the loads first: all of a thread's pairs are in flight together
         const u32 i = start + r * 32u + lane;
         const bool valid = i < n;
         key[r] = valid ? keys_in[i] : 0ull;
         item[r] = valid ? (idx_in ? idx_in[i] : i) : 0u;
+    }
+#pragma unroll
+    for (u32 r = 0; r < NS_PAIR_ROUNDS; ++r) {
+        const bool valid = start + r * 32u + lane < n;
         const u32 d = valid ? (u32)(key[r] >> shift) & 255u : 256u + lane;    // invalid lanes never match anyone
         const u32 peers = __match_any_sync(NS_FULL, d);
         const u32 before = __popc(peers & lanemask_lt());
@@ -313,34 +323,37 @@ __global__ void __launch_bounds__(256) pair_scatter_kernel(const u64 *__restrict
         dr[r] = d | (rank << 9);
     }
     __syncthreads();
-    // digit threadIdx.x: the tile's count, the warps' offsets inside the digit, the digit's first position in the ordered tile
-    u32 tot = 0;
-    for (u32 ww = 0; ww < 8; ++ww) { const u32 c = wcount[ww][threadIdx.x]; wcount[ww][threadIdx.x] = tot; tot += c; }
-    u32 x = tot;                                        // exclusive scan of the 256 digit counts over the block
-    for (int o = 1; o < 32; o <<= 1) { const u32 y = __shfl_up_sync(NS_FULL, x, o); if ((int)lane >= o) x += y; }
-    __shared__ u32 wtot[8];
-    if (lane == 31) wtot[w] = x;
+    // digit threadIdx.x (threads 0..255): the tile's count, the warps' offsets inside the digit, the digit's first position in the ordered tile
+    u32 tot = 0, x = 0;
+    if (threadIdx.x < 256u) {
+        for (u32 ww = 0; ww < NS_PAIR_WARPS; ++ww) { const u32 c = wcount[ww][threadIdx.x]; wcount[ww][threadIdx.x] = tot; tot += c; }
+        x = tot;                                        // exclusive scan of the 256 digit counts over the first 8 warps
+        for (int o = 1; o < 32; o <<= 1) { const u32 y = __shfl_up_sync(NS_FULL, x, o); if ((int)lane >= o) x += y; }
+        if (lane == 31) wtot[w] = x;
+    }
     __syncthreads();
-    u32 off = x - tot;
-    for (u32 ww = 0; ww < w; ++ww) off += wtot[ww];
-    bdo[threadIdx.x] = off;
-    gbase[threadIdx.x] = hist[threadIdx.x * nblocks + blockIdx.x];
+    if (threadIdx.x < 256u) {
+        u32 off = x - tot;
+        for (u32 ww = 0; ww < w; ++ww) off += wtot[ww];
+        bdo[threadIdx.x] = off;
+        gbase[threadIdx.x] = hist[threadIdx.x * nblocks + blockIdx.x];
+    }
     __syncthreads();
 #pragma unroll
-    for (u32 r = 0; r < 16; ++r) {
+    for (u32 r = 0; r < NS_PAIR_ROUNDS; ++r) {
         const u32 d = dr[r] & 511u;
         if (d < 256u) { const u32 p = bdo[d] + wcount[w][d] + (dr[r] >> 9); skey[p] = key[r]; sidx[p] = item[r]; }
     }
     __syncthreads();
     const u32 cnt = min(NS_PAIR_TILE, n - tile0);
-    for (u32 t = threadIdx.x; t < cnt; t += 256u) {
+    for (u32 t = threadIdx.x; t < cnt; t += NS_PAIR_THREADS) {
         const u64 k = skey[t];
         const u32 d = (u32)(k >> shift) & 255u;
         const u32 o = gbase[d] + (t - bdo[d]);
         keys_out[o] = k; idx_out[o] = sidx[t];
     }
 }
-#define NS_PAIR_SMEM (NS_PAIR_TILE * 12u + 8u * 256u * 4u + 2u * 256u * 4u)
+#define NS_PAIR_SMEM (NS_PAIR_TILE * 12u + NS_PAIR_WARPS * 256u * 4u + 2u * 256u * 4u + 64u)
 // order of two records of the same interval k: by (f, loc, j)
 __device__ __forceinline__ bool rec_less(const uint4 *__restrict__ rec, u32 a, u32 b) {
     const uint4 a1 = rec[2u * a + 1u], b1 = rec[2u * b + 1u];

@@ -747,7 +747,7 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
                 if (b >= 5 && (kmax >> (8 * (b - 5))) == 0) continue;
                 pair_hist_kernel<<<nb, 256, 0, st>>>(ksrc, nr, 8 * b, hist, nb);
                 n_launch += 2 + scan_u32(hist, 256 * nb, scan_tmp, NULL, st);
-                pair_scatter_kernel<<<nb, 256, NS_PAIR_SMEM, st>>>(ksrc, isrc, kdst, idst, nr, 8 * b, hist, nb);
+                pair_scatter_kernel<<<nb, NS_PAIR_THREADS, NS_PAIR_SMEM, st>>>(ksrc, isrc, kdst, idst, nr, 8 * b, hist, nb);
                 std::swap(ksrc, kdst);
                 isrc = idst; std::swap(idst, iother);
             }
