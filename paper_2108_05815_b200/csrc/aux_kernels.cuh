@@ -71,8 +71,16 @@ __global__ void __launch_bounds__(1024) scan_tile_kernel(u32 *__restrict__ a, u3
     const u32 lane = threadIdx.x & 31u, w = threadIdx.x >> 5;
     const u32 base = blockIdx.x * NS_SCAN_TILE + threadIdx.x * 8u;
     u32 v[8], t = 0;
+    const bool full = base + 8u <= n;                  // (a is 32-byte aligned at base: two 16-byte loads instead of eight strided words)
+    if (full) {
+        const uint4 p0 = *(const uint4 *)(a + base), p1 = *(const uint4 *)(a + base + 4u);
+        v[0] = p0.x; v[1] = p0.y; v[2] = p0.z; v[3] = p0.w; v[4] = p1.x; v[5] = p1.y; v[6] = p1.z; v[7] = p1.w;
+    } else {
 #pragma unroll
-    for (int q = 0; q < 8; ++q) { v[q] = (base + q < n) ? a[base + q] : 0u; t += v[q]; }
+        for (int q = 0; q < 8; ++q) v[q] = (base + q < n) ? a[base + q] : 0u;
+    }
+#pragma unroll
+    for (int q = 0; q < 8; ++q) t += v[q];
     u32 x = t;
     for (int o = 1; o < 32; o <<= 1) { u32 y = __shfl_up_sync(NS_FULL, x, o); if ((int)lane >= o) x += y; }
     if (lane == 31) wsum[w] = x;
@@ -85,11 +93,24 @@ __global__ void __launch_bounds__(1024) scan_tile_kernel(u32 *__restrict__ a, u3
     }
     __syncthreads();
     u32 run = wsum[w] + (x - t);
+    if (full) {
+        u32 e[8];
 #pragma unroll
-    for (int q = 0; q < 8; ++q) { if (base + q < n) a[base + q] = run; run += v[q]; }
+        for (int q = 0; q < 8; ++q) { e[q] = run; run += v[q]; }
+        *(uint4 *)(a + base) = make_uint4(e[0], e[1], e[2], e[3]); *(uint4 *)(a + base + 4u) = make_uint4(e[4], e[5], e[6], e[7]);
+    } else {
+#pragma unroll
+        for (int q = 0; q < 8; ++q) { if (base + q < n) a[base + q] = run; run += v[q]; }
+    }
 }
 __global__ void __launch_bounds__(1024) scan_add_kernel(u32 *__restrict__ a, u32 n, const u32 *__restrict__ sums) {
     const u32 base = blockIdx.x * NS_SCAN_TILE + threadIdx.x * 8u, add = sums[blockIdx.x];
+    if (base + 8u <= n) {
+        uint4 p0 = *(const uint4 *)(a + base), p1 = *(const uint4 *)(a + base + 4u);
+        p0.x += add; p0.y += add; p0.z += add; p0.w += add; p1.x += add; p1.y += add; p1.z += add; p1.w += add;
+        *(uint4 *)(a + base) = p0; *(uint4 *)(a + base + 4u) = p1;
+        return;
+    }
 #pragma unroll
     for (int q = 0; q < 8; ++q) if (base + q < n) a[base + q] += add;
 }
@@ -268,14 +289,17 @@ __global__ void __launch_bounds__(256) merge_write_kernel(const SimBuffers bf, c
 // (f, loc, j) with the records gathered through the index (one 32-byte sector each). Runs longer than NS_RUN_INLINE go to a warp.
 #define NS_RUN_INLINE 16u
 #define NS_PAIR_TILE 4096u          // pairs per block and pass: 16 per digit on average, so that a digit's pairs leave the block as one run
-__global__ void __launch_bounds__(256) pair_hist_kernel(const u64 *__restrict__ keys, u32 n, u32 shift, u32 *__restrict__ hist, u32 nblocks) {
+// Keys: the ring's 64-bit keys, or (compact sort) 32-bit keys ck = (u32)(key >> cshift) that hold the interval and the leading bits of
+// f in one word: 8-byte pairs instead of 12-byte ones. The first compact pass reads the 64-bit keys and writes the 32-bit ones.
+template <typename KIN>
+__global__ void __launch_bounds__(256) pair_hist_kernel(const KIN *__restrict__ keys, u32 n, u32 cshift, u32 shift, u32 *__restrict__ hist, u32 nblocks) {
     __shared__ u32 h[256];
     h[threadIdx.x] = 0;
     __syncthreads();
     const u32 start = blockIdx.x * NS_PAIR_TILE;
     for (u32 r = 0; r < NS_PAIR_TILE; r += 256u) {
         const u32 i = start + r + threadIdx.x;
-        if (i < n) atomicAdd(&h[(u32)(keys[i] >> shift) & 255u], 1u);
+        if (i < n) atomicAdd(&h[(u32)((keys[i] >> cshift) >> shift) & 255u], 1u);
     }
     __syncthreads();
     hist[threadIdx.x * nblocks + blockIdx.x] = h[threadIdx.x];
@@ -288,10 +312,11 @@ __global__ void __launch_bounds__(256) pair_hist_kernel(const u64 *__restrict__ 
 #define NS_PAIR_THREADS 512u
 #define NS_PAIR_WARPS (NS_PAIR_THREADS / 32u)
 #define NS_PAIR_ROUNDS (NS_PAIR_TILE / NS_PAIR_THREADS)
-__global__ void __launch_bounds__(NS_PAIR_THREADS, 3) pair_scatter_kernel(const u64 *__restrict__ keys_in, const u32 *__restrict__ idx_in, u64 *__restrict__ keys_out,
-                                                                          u32 *__restrict__ idx_out, u32 n, u32 shift, const u32 *__restrict__ hist, u32 nblocks) {
-    extern __shared__ unsigned char pair_smem[];
-    u64 *skey = (u64 *)pair_smem;                           // [NS_PAIR_TILE]
+template <typename KIN, typename KOUT>
+__global__ void __launch_bounds__(NS_PAIR_THREADS, 3) pair_scatter_kernel(const KIN *__restrict__ keys_in, const u32 *__restrict__ idx_in, KOUT *__restrict__ keys_out,
+                                                                          u32 *__restrict__ idx_out, u32 n, u32 cshift, u32 shift, const u32 *__restrict__ hist, u32 nblocks) {
+    extern __shared__ __align__(16) unsigned char pair_smem[];
+    KOUT *skey = (KOUT *)pair_smem;                         // [NS_PAIR_TILE]
     u32 *sidx = (u32 *)(skey + NS_PAIR_TILE);               // [NS_PAIR_TILE]
     u32 (*wcount)[256] = (u32 (*)[256])(sidx + NS_PAIR_TILE);   // [NS_PAIR_WARPS][256]
     u32 *bdo = (u32 *)(wcount + NS_PAIR_WARPS);             // [256] first position of a digit inside the ordered tile
@@ -301,13 +326,13 @@ __global__ void __launch_bounds__(NS_PAIR_THREADS, 3) pair_scatter_kernel(const 
     for (u32 t = threadIdx.x; t < NS_PAIR_WARPS * 256u; t += NS_PAIR_THREADS) (&wcount[0][0])[t] = 0;
     __syncthreads();
     const u32 tile0 = blockIdx.x * NS_PAIR_TILE, start = tile0 + w * (NS_PAIR_TILE / NS_PAIR_WARPS);
-    u64 key[NS_PAIR_ROUNDS];
+    KOUT key[NS_PAIR_ROUNDS];
     u32 item[NS_PAIR_ROUNDS], dr[NS_PAIR_ROUNDS];       // dr = digit | rank inside the warp's 256 positions << 9
 #pragma unroll
     for (u32 r = 0; r < NS_PAIR_ROUNDS; ++r) {          // the loads first: all of a thread's pairs are in flight together
         const u32 i = start + r * 32u + lane;
         const bool valid = i < n;
-        key[r] = valid ? keys_in[i] : 0ull;
+        key[r] = valid ? (KOUT)(keys_in[i] >> cshift) : (KOUT)0;
         item[r] = valid ? (idx_in ? idx_in[i] : i) : 0u;
     }
 #pragma unroll
@@ -347,13 +372,13 @@ __global__ void __launch_bounds__(NS_PAIR_THREADS, 3) pair_scatter_kernel(const 
     __syncthreads();
     const u32 cnt = min(NS_PAIR_TILE, n - tile0);
     for (u32 t = threadIdx.x; t < cnt; t += NS_PAIR_THREADS) {
-        const u64 k = skey[t];
+        const KOUT k = skey[t];
         const u32 d = (u32)(k >> shift) & 255u;
         const u32 o = gbase[d] + (t - bdo[d]);
         keys_out[o] = k; idx_out[o] = sidx[t];
     }
 }
-#define NS_PAIR_SMEM (NS_PAIR_TILE * 12u + NS_PAIR_WARPS * 256u * 4u + 2u * 256u * 4u + 64u)
+#define NS_PAIR_SMEM(keybytes) (NS_PAIR_TILE * ((keybytes) + 4u) + NS_PAIR_WARPS * 256u * 4u + 2u * 256u * 4u + 64u)
 // order of two records of the same interval k: by (f, loc, j)
 __device__ __forceinline__ bool rec_less(const uint4 *__restrict__ rec, u32 a, u32 b) {
     const uint4 a1 = rec[2u * a + 1u], b1 = rec[2u * b + 1u];
@@ -370,13 +395,14 @@ __device__ __forceinline__ bool rec_same(const uint4 *__restrict__ rec, u32 a, u
 // Runs of equal key prefix (key >> pshift): head flags (1 = first record of a distinct event; redundant copies, adjacent after the
 // sort, and sentinels get 0) and the full order inside a run. Only the first thread of a run writes idx[i..e) and
 // flag[i..e); everybody else reads the keys, which this kernel never changes. Long runs are queued for stream_long_runs_kernel.
-__global__ void __launch_bounds__(256) stream_ties_kernel(const u64 *__restrict__ keys, u32 *__restrict__ idx, const uint4 *__restrict__ rec, u32 n, u32 pshift,
-                                                          u32 *__restrict__ flag, u32 *__restrict__ long_runs, u32 *__restrict__ n_long, u32 long_cap) {
+template <typename K>
+__global__ void __launch_bounds__(256) stream_ties_kernel(const K *__restrict__ keys, u32 *__restrict__ idx, const uint4 *__restrict__ rec, u32 n, u32 pshift,
+                                                          uint8_t *__restrict__ flag, u32 *__restrict__ long_runs, u32 *__restrict__ n_long, u32 long_cap) {
     const u32 i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    const u64 key = keys[i];
-    if (key == ~0ull) { flag[i] = 0u; return; }          // reserved but unused ring slot
-    const u64 kp = key >> pshift;
+    const K key = keys[i];
+    if (key == (K)~(K)0) { flag[i] = 0u; return; }       // reserved but unused ring slot
+    const K kp = key >> pshift;
     if (i != 0 && (keys[i - 1] >> pshift) == kp) return; // not the first of its run
     u32 e = i + 1;
     while (e < n && (keys[e] >> pshift) == kp) ++e;
@@ -396,7 +422,7 @@ __global__ void __launch_bounds__(256) stream_ties_kernel(const u64 *__restrict_
 }
 // One warp per long run. Long runs are almost always copies of ONE event (many lineages on a shared path, dedup off or a small
 // cache): that is checked first in a single sweep. Otherwise the run is ordered by ranking every record against all others.
-__global__ void __launch_bounds__(256) stream_long_runs_kernel(u32 *__restrict__ idx, const uint4 *__restrict__ rec, u32 *__restrict__ flag,
+__global__ void __launch_bounds__(256) stream_long_runs_kernel(u32 *__restrict__ idx, const uint4 *__restrict__ rec, uint8_t *__restrict__ flag,
                                                                const u32 *__restrict__ long_runs, const u32 *__restrict__ n_long, u32 long_cap, u32 *__restrict__ tmp) {
     const u32 lane = threadIdx.x & 31u, warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarps = (gridDim.x * blockDim.x) >> 5;
     const u32 nl = min(*n_long, long_cap);
@@ -424,19 +450,46 @@ __global__ void __launch_bounds__(256) stream_long_runs_kernel(u32 *__restrict__
         for (u32 p = lane; p < L; p += 32u) flag[i + p] = (p == 0u || !rec_same(rec, idx[i + p], idx[i + p - 1u])) ? 1u : 0u;
     }
 }
-// uidx = the head flags scanned exclusively, *total = their sum: the heads are appended to the stream (SoA, coalesced writes)
-__global__ void __launch_bounds__(256) stream_write_kernel(const uint4 *__restrict__ rec, const u32 *__restrict__ idx, u32 n, const u32 *__restrict__ uidx,
-                                                           const u32 *__restrict__ total, u64 base, u64 cap, u32 *__restrict__ s_loc,
+// The head flags are bytes. A block owns NS_WRITE_TILE consecutive records: stream_count_kernel sums their flags into bsum[block], the
+// host scans bsum (one entry per 2048 records instead of a scan over one word per record), stream_write_kernel recomputes the positions
+// inside its tile with ballots and appends the heads to the stream (SoA, coalesced writes; the 32-byte records come through the index).
+#define NS_WRITE_TILE 2048u
+__global__ void __launch_bounds__(256) stream_count_kernel(const uint8_t *__restrict__ flag, u32 n, u32 *__restrict__ bsum) {
+    __shared__ u32 ws[8];
+    const u32 i0 = blockIdx.x * NS_WRITE_TILE + threadIdx.x * 8u;
+    u32 c = 0;
+    if (i0 + 8u <= n) { const uint2 v = *(const uint2 *)(flag + i0); c = __popc(v.x & 0x01010101u) + __popc(v.y & 0x01010101u); }
+    else for (u32 t = i0; t < n; ++t) c += flag[t] & 1u;
+    for (int o = 16; o; o >>= 1) c += __shfl_down_sync(NS_FULL, c, o);
+    if ((threadIdx.x & 31u) == 0) ws[threadIdx.x >> 5] = c;
+    __syncthreads();
+    if (threadIdx.x == 0) { u32 t = 0; for (u32 w = 0; w < 8; ++w) t += ws[w]; bsum[blockIdx.x] = t; }
+}
+__global__ void __launch_bounds__(256) stream_write_kernel(const uint4 *__restrict__ rec, const u32 *__restrict__ idx, u32 n, const uint8_t *__restrict__ flag,
+                                                           const u32 *__restrict__ bsum, u64 base, u64 cap, u32 *__restrict__ s_loc,
                                                            u32 *__restrict__ s_k, u32 *__restrict__ s_j, u64 *__restrict__ s_f, u32 *__restrict__ s_loc2) {
-    const u32 i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    const u32 u = uidx[i], nx = (i + 1 < n) ? uidx[i + 1] : *total;
-    if (nx == u) return;
-    const u64 o = base + u;
-    if (o >= cap) return;
-    const u32 id = idx[i];
-    const uint4 r0 = rec[2u * id], r1 = rec[2u * id + 1u];
-    s_loc[o] = r0.x; s_k[o] = r0.y; s_j[o] = r0.z; s_loc2[o] = r0.w; s_f[o] = ((u64)r1.y << 32) | r1.x;
+    __shared__ u32 ws[8];
+    const u32 lane = threadIdx.x & 31u, w = threadIdx.x >> 5;
+    u32 run = bsum[blockIdx.x];                          // heads before this block (bsum is scanned exclusively)
+    for (u32 sub = 0; sub < NS_WRITE_TILE; sub += 256u) {
+        const u32 i = blockIdx.x * NS_WRITE_TILE + sub + threadIdx.x;
+        const bool head = i < n && (flag[i] & 1u);
+        const u32 b = __ballot_sync(NS_FULL, head);
+        if (lane == 0) ws[w] = __popc(b);
+        __syncthreads();
+        u32 woff = 0, tot = 0;
+        for (u32 q = 0; q < 8; ++q) { const u32 c = ws[q]; if (q < w) woff += c; tot += c; }
+        __syncthreads();
+        if (head) {
+            const u64 o = base + run + woff + __popc(b & lanemask_lt());
+            if (o < cap) {
+                const u32 id = idx[i];
+                const uint4 r0 = rec[2u * id], r1 = rec[2u * id + 1u];
+                s_loc[o] = r0.x; s_k[o] = r0.y; s_j[o] = r0.z; s_loc2[o] = r0.w; s_f[o] = ((u64)r1.y << 32) | r1.x;
+            }
+        }
+        run += tot;
+    }
 }
 
 __global__ void copy_u32_kernel(u32 *a, const u32 *src, u32 n) {

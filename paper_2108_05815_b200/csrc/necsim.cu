@@ -600,7 +600,11 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
     u64 stream_n = 0;
     SimCounters *hc = scn->h_ctr;
 
-    if (rp.record) CU(cudaFuncSetAttribute(pair_scatter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)NS_PAIR_SMEM));
+    if (rp.record) {
+        CU(cudaFuncSetAttribute(pair_scatter_kernel<u64, u64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)NS_PAIR_SMEM(8u)));
+        CU(cudaFuncSetAttribute(pair_scatter_kernel<u64, u32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)NS_PAIR_SMEM(4u)));
+        CU(cudaFuncSetAttribute(pair_scatter_kernel<u32, u32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)NS_PAIR_SMEM(4u)));
+    }
     CU(cudaEventRecord(scn->ev[0], st));
     CU(cudaMemsetAsync(bf.ctr, 0, sizeof(SimCounters), st));
     CU(cudaMemsetAsync(bf.state, 0, cap, st));
@@ -735,28 +739,58 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
             if (nr > rp.ring_cap) return fail(NECSIM_ERR_CAPACITY, "event ring overflowed: raise event_ring_capacity");
             const u32 nb = (nr + NS_PAIR_TILE - 1) / NS_PAIR_TILE, g256 = (nr + 255) / 256;
             const u32 kmax = k_stop - ep.k_start;   // (k - k_start) < kmax for every record; the sentinel key ~0 sorts last
-            // LSD radix passes over the key bytes that matter: the leading `fbytes` bytes of f (key bytes 5 - fbytes .. 4) and the
-            // bytes of k in use (key bytes 5 ..). Default: the fewest bytes of f that leave about two records or fewer per prefix value
-            // (short runs cost the tie pass less than another radix pass).
-            u32 fbytes = rp.stream_fbytes ? std::min(rp.stream_fbytes, 5u) : 1u;
-            if (!rp.stream_fbytes)
-                while (fbytes < 5 && (double)nr > 2.0 * (double)kmax * (double)(1ull << (8 * fbytes))) ++fbytes;
-            u64 *ksrc = key_a, *kdst = key_b;
+            // LSD radix passes over (key, index) pairs. Compact sort (the default when the epoch spans fewer than 2^16 intervals): the
+            // interval and the leading bits of f are packed into ONE 32-bit key, ck = key >> (8 + kbits) -- 8-byte pairs instead of
+            // 12-byte ones, and all 32 - kbits leading bits of f take part (fewer ties than with whole bytes of f). Only the top
+            // `passes` bytes of ck are sorted on: the fewest that leave about two records or fewer per prefix value (short runs cost the
+            // tie pass less than another radix pass). A forced `stream_sort_bytes` keeps the 64-bit keys (k bytes + that many bytes of f).
+            uint8_t *flag8 = (uint8_t *)flag;
+            u32 kbits = 1; while ((1ull << kbits) < (u64)kmax + 1ull) ++kbits;     // k - k_start <= kmax - 1 < 2^kbits - 1: all ones = the sentinel only
+            const bool compact_keys = !rp.stream_fbytes && kbits <= 16u;
             u32 *isrc = NULL, *idst = perm_a, *iother = perm_b;
-            for (u32 b = 5u - fbytes; b < 8; ++b) {
-                if (b >= 5 && (kmax >> (8 * (b - 5))) == 0) continue;
-                pair_hist_kernel<<<nb, 256, 0, st>>>(ksrc, nr, 8 * b, hist, nb);
-                n_launch += 2 + scan_u32(hist, 256 * nb, scan_tmp, NULL, st);
-                pair_scatter_kernel<<<nb, NS_PAIR_THREADS, NS_PAIR_SMEM, st>>>(ksrc, isrc, kdst, idst, nr, 8 * b, hist, nb);
-                std::swap(ksrc, kdst);
-                isrc = idst; std::swap(idst, iother);
-            }
-            // isrc / ksrc: sorted by the key prefix; idst: free scratch of the same size
             CU(cudaMemsetAsync(&bf.ctr->n_long, 0, 4, st));
-            stream_ties_kernel<<<g256, 256, 0, st>>>(ksrc, isrc, bf.rec, nr, 8 * (5u - fbytes), flag, long_runs, &bf.ctr->n_long, long_cap);
-            stream_long_runs_kernel<<<(u32)scn->sm_count * 4u, 256, 0, st>>>(isrc, bf.rec, flag, long_runs, &bf.ctr->n_long, long_cap, idst);
-            n_launch += scan_u32(flag, nr, scan_tmp, &bf.ctr->q_head, st) - 1;   // q_head reused: distinct events of the epoch
-            stream_write_kernel<<<g256, 256, 0, st>>>(bf.rec, isrc, nr, flag, &bf.ctr->q_head, stream_n, rp.stream_cap, st_loc, st_k, st_j, st_f, st_l2);
+            if (compact_keys) {
+                u32 fbits = 0; while (fbits < 32u - kbits && (double)nr > 2.0 * (double)kmax * (double)(1ull << fbits)) ++fbits;
+                const u32 passes = std::min(4u, std::max(1u, (kbits + fbits + 7u) / 8u));
+                const u32 cshift = 8u + kbits;
+                u32 *k32a = (u32 *)key_b, *k32b = (u32 *)key_b + rp.ring_cap, *ksrc32 = NULL, *kdst32 = k32a;
+                for (u32 b = 4u - passes; b < 4u; ++b) {
+                    if (!ksrc32) {
+                        pair_hist_kernel<u64><<<nb, 256, 0, st>>>(key_a, nr, cshift, 8 * b, hist, nb);
+                        n_launch += 2 + scan_u32(hist, 256 * nb, scan_tmp, NULL, st);
+                        pair_scatter_kernel<u64, u32><<<nb, NS_PAIR_THREADS, NS_PAIR_SMEM(4u), st>>>(key_a, isrc, kdst32, idst, nr, cshift, 8 * b, hist, nb);
+                    } else {
+                        pair_hist_kernel<u32><<<nb, 256, 0, st>>>(ksrc32, nr, 0, 8 * b, hist, nb);
+                        n_launch += 2 + scan_u32(hist, 256 * nb, scan_tmp, NULL, st);
+                        pair_scatter_kernel<u32, u32><<<nb, NS_PAIR_THREADS, NS_PAIR_SMEM(4u), st>>>(ksrc32, isrc, kdst32, idst, nr, 0, 8 * b, hist, nb);
+                    }
+                    ksrc32 = kdst32; kdst32 = (ksrc32 == k32a) ? k32b : k32a;
+                    isrc = idst; std::swap(idst, iother);
+                }
+                stream_ties_kernel<u32><<<g256, 256, 0, st>>>(ksrc32, isrc, bf.rec, nr, 8 * (4u - passes), flag8, long_runs, &bf.ctr->n_long, long_cap);
+            } else {
+                // the leading `fbytes` bytes of f (key bytes 5 - fbytes .. 4) and the bytes of k in use (key bytes 5 ..)
+                u32 fbytes = rp.stream_fbytes ? std::min(rp.stream_fbytes, 5u) : 1u;
+                if (!rp.stream_fbytes)
+                    while (fbytes < 5 && (double)nr > 2.0 * (double)kmax * (double)(1ull << (8 * fbytes))) ++fbytes;
+                u64 *ksrc = key_a, *kdst = key_b;
+                for (u32 b = 5u - fbytes; b < 8; ++b) {
+                    if (b >= 5 && (kmax >> (8 * (b - 5))) == 0) continue;
+                    pair_hist_kernel<u64><<<nb, 256, 0, st>>>(ksrc, nr, 0, 8 * b, hist, nb);
+                    n_launch += 2 + scan_u32(hist, 256 * nb, scan_tmp, NULL, st);
+                    pair_scatter_kernel<u64, u64><<<nb, NS_PAIR_THREADS, NS_PAIR_SMEM(8u), st>>>(ksrc, isrc, kdst, idst, nr, 0, 8 * b, hist, nb);
+                    std::swap(ksrc, kdst);
+                    isrc = idst; std::swap(idst, iother);
+                }
+                stream_ties_kernel<u64><<<g256, 256, 0, st>>>(ksrc, isrc, bf.rec, nr, 8 * (5u - fbytes), flag8, long_runs, &bf.ctr->n_long, long_cap);
+            }
+            // isrc: the records' indices sorted by the key prefix; idst: free scratch of the same size
+            stream_long_runs_kernel<<<(u32)scn->sm_count * 4u, 256, 0, st>>>(isrc, bf.rec, flag8, long_runs, &bf.ctr->n_long, long_cap, idst);
+            const u32 nwt = (nr + NS_WRITE_TILE - 1) / NS_WRITE_TILE;
+            u32 *bsum = hist;                                // the histograms are done with: heads per tile of 2048 records
+            stream_count_kernel<<<nwt, 256, 0, st>>>(flag8, nr, bsum);
+            n_launch += scan_u32(bsum, nwt, scan_tmp, &bf.ctr->q_head, st);   // q_head reused: distinct events of the epoch
+            stream_write_kernel<<<nwt, 256, 0, st>>>(bf.rec, isrc, nr, flag8, bsum, stream_n, rp.stream_cap, st_loc, st_k, st_j, st_f, st_l2);
             n_launch += 4;
             CU(cudaGetLastError());
             u32 heads = 0;

@@ -179,7 +179,11 @@ class Scenario:
             lib().necsim_destroy(self._h)
             self._h = None
 
-    __del__ = close
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:       # interpreter shutdown: the module globals may be gone already
+            pass
 
     def _workspace(self, cap, params):
         torch = _torch()
