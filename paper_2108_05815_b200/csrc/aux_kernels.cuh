@@ -297,10 +297,14 @@ __global__ void __launch_bounds__(256) pair_hist_kernel(const KIN *__restrict__ 
     h[threadIdx.x] = 0;
     __syncthreads();
     const u32 start = blockIdx.x * NS_PAIR_TILE;
-    for (u32 r = 0; r < NS_PAIR_TILE; r += 256u) {
-        const u32 i = start + r + threadIdx.x;
-        if (i < n) atomicAdd(&h[(u32)((keys[i] >> cshift) >> shift) & 255u], 1u);
+    u32 d[NS_PAIR_TILE / 256u];
+#pragma unroll
+    for (u32 r = 0; r < NS_PAIR_TILE / 256u; ++r) {   // all loads of the thread in flight before the first atomic
+        const u32 i = start + r * 256u + threadIdx.x;
+        d[r] = i < n ? (u32)((keys[i] >> cshift) >> shift) & 255u : 256u;
     }
+#pragma unroll
+    for (u32 r = 0; r < NS_PAIR_TILE / 256u; ++r) if (d[r] < 256u) atomicAdd(&h[d[r]], 1u);
     __syncthreads();
     hist[threadIdx.x * nblocks + blockIdx.x] = h[threadIdx.x];
 }

@@ -602,7 +602,6 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
 
     if (rp.record) {
         CU(cudaFuncSetAttribute(pair_scatter_kernel<u64, u64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)NS_PAIR_SMEM(8u)));
-        CU(cudaFuncSetAttribute(pair_scatter_kernel<u64, u32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)NS_PAIR_SMEM(4u)));
         CU(cudaFuncSetAttribute(pair_scatter_kernel<u32, u32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)NS_PAIR_SMEM(4u)));
     }
     CU(cudaEventRecord(scn->ev[0], st));
@@ -710,6 +709,11 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
         }
         bf.q_in = q_in; bf.q_out = q_out; bf.q_in_count = active;
         bf.k_base = rp.record ? k_start : 0u;    // REC kernels: the time key of a record holds k - k_start
+        // compact sort keys (see the stream pipeline below): decided before the launch, the kernels write the 32-bit keys themselves
+        u32 kbits = 1;
+        if (rp.record) { const u64 km = (u64)k_stop - (u64)k_start; while ((1ull << kbits) < km + 1ull) ++kbits; }
+        const bool compact_keys = rp.record && !rp.stream_fbytes && kbits <= 16u;
+        bf.key_shift = compact_keys ? 8u + kbits : 0u;
         // tail epochs with a horizon: a few thousand synchronous lineages need few slots, keep the footprint (2 MiB) inside L2
         // next to the tables. The tail without a horizon drifts apart in simulated time and needs the long memory of the full cache.
         bf.cache_mask = rp.dedup ? ((tail && !unbounded) ? std::min(full_cache_mask, (1u << 17) - 1u) : full_cache_mask) : 0u;
@@ -740,30 +744,21 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
             const u32 nb = (nr + NS_PAIR_TILE - 1) / NS_PAIR_TILE, g256 = (nr + 255) / 256;
             const u32 kmax = k_stop - ep.k_start;   // (k - k_start) < kmax for every record; the sentinel key ~0 sorts last
             // LSD radix passes over (key, index) pairs. Compact sort (the default when the epoch spans fewer than 2^16 intervals): the
-            // interval and the leading bits of f are packed into ONE 32-bit key, ck = key >> (8 + kbits) -- 8-byte pairs instead of
+            // interval and the leading bits of f are packed into ONE 32-bit key, ck = key >> (8 + kbits), written by the recording kernels -- 8-byte pairs instead of
             // 12-byte ones, and all 32 - kbits leading bits of f take part (fewer ties than with whole bytes of f). Only the top
             // `passes` bytes of ck are sorted on: the fewest that leave about two records or fewer per prefix value (short runs cost the
             // tie pass less than another radix pass). A forced `stream_sort_bytes` keeps the 64-bit keys (k bytes + that many bytes of f).
-            uint8_t *flag8 = (uint8_t *)flag;
-            u32 kbits = 1; while ((1ull << kbits) < (u64)kmax + 1ull) ++kbits;     // k - k_start <= kmax - 1 < 2^kbits - 1: all ones = the sentinel only
-            const bool compact_keys = !rp.stream_fbytes && kbits <= 16u;
+            uint8_t *flag8 = (uint8_t *)flag;                                      // (kbits: k - k_start <= kmax - 1 < 2^kbits - 1, all ones = the sentinel only)
             u32 *isrc = NULL, *idst = perm_a, *iother = perm_b;
             CU(cudaMemsetAsync(&bf.ctr->n_long, 0, 4, st));
             if (compact_keys) {
                 u32 fbits = 0; while (fbits < 32u - kbits && (double)nr > 2.0 * (double)kmax * (double)(1ull << fbits)) ++fbits;
                 const u32 passes = std::min(4u, std::max(1u, (kbits + fbits + 7u) / 8u));
-                const u32 cshift = 8u + kbits;
-                u32 *k32a = (u32 *)key_b, *k32b = (u32 *)key_b + rp.ring_cap, *ksrc32 = NULL, *kdst32 = k32a;
+                u32 *k32a = (u32 *)key_b, *k32b = (u32 *)key_b + rp.ring_cap, *ksrc32 = (u32 *)key_a, *kdst32 = k32a;   // the ring's keys are 32-bit already
                 for (u32 b = 4u - passes; b < 4u; ++b) {
-                    if (!ksrc32) {
-                        pair_hist_kernel<u64><<<nb, 256, 0, st>>>(key_a, nr, cshift, 8 * b, hist, nb);
-                        n_launch += 2 + scan_u32(hist, 256 * nb, scan_tmp, NULL, st);
-                        pair_scatter_kernel<u64, u32><<<nb, NS_PAIR_THREADS, NS_PAIR_SMEM(4u), st>>>(key_a, isrc, kdst32, idst, nr, cshift, 8 * b, hist, nb);
-                    } else {
-                        pair_hist_kernel<u32><<<nb, 256, 0, st>>>(ksrc32, nr, 0, 8 * b, hist, nb);
-                        n_launch += 2 + scan_u32(hist, 256 * nb, scan_tmp, NULL, st);
-                        pair_scatter_kernel<u32, u32><<<nb, NS_PAIR_THREADS, NS_PAIR_SMEM(4u), st>>>(ksrc32, isrc, kdst32, idst, nr, 0, 8 * b, hist, nb);
-                    }
+                    pair_hist_kernel<u32><<<nb, 256, 0, st>>>(ksrc32, nr, 0, 8 * b, hist, nb);
+                    n_launch += 2 + scan_u32(hist, 256 * nb, scan_tmp, NULL, st);
+                    pair_scatter_kernel<u32, u32><<<nb, NS_PAIR_THREADS, NS_PAIR_SMEM(4u), st>>>(ksrc32, isrc, kdst32, idst, nr, 0, 8 * b, hist, nb);
                     ksrc32 = kdst32; kdst32 = (ksrc32 == k32a) ? k32b : k32a;
                     isrc = idst; std::swap(idst, iother);
                 }

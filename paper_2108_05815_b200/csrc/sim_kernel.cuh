@@ -198,7 +198,13 @@ __device__ __forceinline__ void store_record(const SimBuffers &bf, u32 idx, u32 
     // and the habitat tables out of L2 (measured: L2 hit rate of the recording kernel 41 % with plain stores)
     __stcs(&bf.rec[2u * idx], make_uint4(loc, k, j, loc2));
     __stcs(&bf.rec[2u * idx + 1u], make_uint4((u32)f, (u32)(f >> 32), 0u, 0u));
-    __stcs((unsigned long long *)&bf.rec_key[idx], (unsigned long long)NS_STREAM_KEY(k - bf.k_base, f));
+    const u64 key = NS_STREAM_KEY(k - bf.k_base, f);
+    if (bf.key_shift) __stcs((u32 *)bf.rec_key + idx, (u32)(key >> bf.key_shift));
+    else __stcs((unsigned long long *)&bf.rec_key[idx], (unsigned long long)key);
+}
+// the sentinel key of a reserved but unused ring slot: all ones (sorts last, dropped)
+__device__ __forceinline__ void store_sentinel(const SimBuffers &bf, u32 idx) {
+    if (bf.key_shift) ((u32 *)bf.rec_key)[idx] = ~0u; else bf.rec_key[idx] = ~0ull;
 }
 __device__ __forceinline__ void record_event(const SimBuffers &bf, u32 loc, u32 k, u32 j, u64 f, u32 loc2) {
     const u32 mask = __activemask();
@@ -497,7 +503,7 @@ __global__ void __launch_bounds__(256) simulate_kernel(const ScenarioDev sc, con
             if (rm) {
                 const u32 cnt = __popc(rm);
                 if (rec_left < cnt) {
-                    if (lane < rec_left) bf.rec_key[rec_next + lane] = ~0ull;      // rec_left < cnt <= 32
+                    if (lane < rec_left) store_sentinel(bf, rec_next + lane);      // rec_left < cnt <= 32
                     const u32 take = ep.rec_chunk >= 64u ? ep.rec_chunk : cnt;     // small rings: exact reservations
                     u32 base = 0;
                     if (lane == 0) base = atomicAdd(&bf.ctr->n_rec, take);
@@ -509,7 +515,7 @@ __global__ void __launch_bounds__(256) simulate_kernel(const ScenarioDev sc, con
             }
         }
     }
-    if (REC) for (u32 q = lane; q < rec_left; q += 32u) if (rec_next + q < bf.rec_cap) bf.rec_key[rec_next + q] = ~0ull;   // the last chunk's unused end
+    if (REC) for (u32 q = lane; q < rec_left; q += 32u) if (rec_next + q < bf.rec_cap) store_sentinel(bf, rec_next + q);   // the last chunk's unused end
     // reduce the per-thread counters: warp shuffle, then one atomic per warp
     unsigned long long r_events = c_events, r_culled = c_culled, r_resamples = c_resamples;
     for (int o = 16; o; o >>= 1) {

@@ -83,6 +83,7 @@ struct SimBuffers {
     // rec_key[i] = (k - k_start) << 40 | f >> 8, which the per-epoch sort works on (coalesced (key, index) pairs, no gathers)
     uint4 *rec;
     u64 *rec_key;
+    u32 key_shift;             // 0: 64-bit keys; else the ring holds 32-bit keys (u32)(key >> key_shift) (the compact sort of an epoch of few intervals)
     u32 rec_cap;
     u32 k_base;                // radix passes sort k - k_base (0 for the species table; the epoch's k_start for the stream ring)
     SimCounters *ctr;

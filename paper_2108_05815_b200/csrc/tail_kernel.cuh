@@ -618,7 +618,7 @@ __global__ void __launch_bounds__(256, 2) tail_kernel(const ScenarioDev sc, cons
         const u32 nx = __shfl_sync(NS_FULL, rec_next, 0), lf = __shfl_sync(NS_FULL, rec_left, 0);
         for (u32 q = lane; q < lf; q += 32u) {
             const u32 ri = nx + q;
-            if (ri < bf.rec_cap) bf.rec_key[ri] = ~0ull;          // sentinel: sorts last, dropped
+            if (ri < bf.rec_cap) store_sentinel(bf, ri);          // sentinel: sorts last, dropped
         }
     }
     if (lane == 0) {
