@@ -321,8 +321,13 @@ __global__ void __launch_bounds__(256, 2) tail_kernel(const ScenarioDev sc, cons
                 if (DEDUP && pend) { if (resolve_pending()) break; }
                 u32 steps_all = steps;
                 bool lpend = false;
+                // s = the stream state of this lane's candidate interval, prime(loc, k + sp_dk). Inside the loop the NEXT round's states are
+                // primed ahead of the vote: every candidate's four lanes prime the four intervals the next round looks at from the
+                // candidate's own outcome (its target location, its interval + 0..3), while the ballots pick the winner; after the vote the
+                // states come from the winner's lanes by shuffle instead of six Feistel rounds at the head of the next round's chain.
+                u64 s = prime(ep.key, loc, k + sp_dk);
                 for (;;) {
-                    const u64 X = prime(ep.key, loc, k + sp_dk) + sp_cand_add;
+                    const u64 X = s + sp_cand_add;
                     u64 ua, ub;
                     hashF2((X ^ NS_L_DISP) + sp_a_add, X ^ sp_b_xor, ua, ub);
                     // duplicate check of the candidate, decided per lane ahead of the selection: whether its event probes the cache, and where.
@@ -375,6 +380,7 @@ __global__ void __launch_bounds__(256, 2) tail_kernel(const ScenarioDev sc, cons
                     const u32 loc2q = __shfl_sync(NS_FULL, loc2o, qsrc), cq = __shfl_sync(NS_FULL, c2o, qsrc);
                     u32 Cmq = Cm, shq = sh;
                     if (PERCELL) { Cmq = __shfl_sync(NS_FULL, cso.x, qsrc); shq = __shfl_sync(NS_FULL, cso.y, qsrc); }
+                    const u64 s_own = prime(ep.key, loc2q, k + sp_dk + sp_q);    // next round's state of interval (this candidate's) + sp_q, if it wins
                     // the winner: first point of interval k after fa_last, else (interval exhausted, L719, L727) the first non-empty later interval
                     const u32 m0 = evm & kmask;
                     const u32 m1 = (crm & kmask) ? (evm & ~kmask) : 0u;
@@ -406,6 +412,7 @@ __global__ void __launch_bounds__(256, 2) tail_kernel(const ScenarioDev sc, cons
                         ln2_over_mu = NS_LN2F * finv; margin = NS_MARGIN * (1.0f + finv);
                     }
                     k = k2; loc = loc2; cell = cell2;
+                    s = __shfl_sync(NS_FULL, s_own, (int)(wl + sp_dk));
                 }
                 steps = steps_all;
                 if (DEDUP && lpend) {          // hand the pending check over to the general code, which keeps the result in lane 0

@@ -63,3 +63,24 @@ def test_partition_and_merge(ns, O, I):
     assert merged == fk
     assert all(merged.index(labels_keys[i]) == full["labels"][i] for i in range(0, n, 37))
     sc.close()
+
+
+@pytest.mark.parametrize("idx", [3, 4])
+def test_tail_without_horizon_worst_case(ns, O, I, idx):
+    """Guard for the worst case of the one-launch tail: the whole run as ONE tail launch without a horizon
+    and a duplicate-culling cache far too small to hold the leaders' entries (16 slots), so that merged lineages hardly ever find
+    each other again. The result must still be the oracle's, and the redundant work is bounded by the run without any culling."""
+    cfg = I.small_configs()[idx]
+    kw = I.scenario_kwargs(cfg)
+    ref = O.Scenario(**kw).simulate(cfg["seed"], cfg["nu"], cfg["mask"], dedup=True)
+    sc = ns.Scenario(**kw)
+    worst = sc.simulate(cfg["seed"], cfg["nu"], cfg["mask"], tail_threshold=0xFFFFFFFF, dedup_log2_slots=4)
+    good = sc.simulate(cfg["seed"], cfg["nu"], cfg["mask"], tail_threshold=0xFFFFFFFF)
+    none = sc.simulate(cfg["seed"], cfg["nu"], cfg["mask"], tail_threshold=0xFFFFFFFF, dedup=False)
+    assert same(worst, ref) and same(good, ref)
+    assert worst["stats"]["n_epochs"] == 1 and worst["stats"]["n_tail_epochs"] == 1
+    uniq = ref["stats"]["n_events"]                      # the oracle's exact culling: distinct events
+    ew, eg, en = worst["stats"]["n_events_raw"], good["stats"]["n_events_raw"], none["stats"]["n_events_raw"]
+    print("redundancy over %d distinct events: 16-slot cache %.2f, default cache %.2f, no culling %.2f" % (uniq, ew / uniq, eg / uniq, en / uniq))
+    assert uniq <= eg <= ew <= en
+    sc.close()
