@@ -91,10 +91,11 @@ typedef struct necsim_sim_params {
                                   only the labels of lineages with state 1 are reproducible then; with dedup = 2 (off) every
                                   per-lineage record is (tests/test_gpu_parity.py) */
     uint32_t tail_threshold;   /* switch to the low-latency tail kernel (one lineage per warp) when active lineages <= this;
-                                  0 = default (four lineages per resident warp) */
-    uint32_t dedup_probe;      /* 0 = default (4); else 1 + log2 of the probe period: 1 = every event, 2 = every 2nd, 3 = every 4th,
-                                  4 = every 8th event (chosen by a hash of the event identity) probes the cache (PAPER.md L942-946:
-                                  the paper probes every step_slice steps) */
+                                  0 = default (128 lineages per SM) */
+    uint32_t dedup_probe;      /* 0 = default: every 8th event probes the cache, every 32nd in the tail launch (a nested subset); else
+                                  1 + log2 of the probe period for both kernels, 1..7: 1 = every event, 2 = every 2nd, ... 7 = every
+                                  64th (chosen by a hash of the event identity; the paper probes every step_slice
+                                  steps). Results never depend on it. */
     uint32_t record_events;    /* 1 = also produce the full event stream (PAPER.md 6.2 L813-906, 7.1.3 L958-967):
                                   every distinct executed event (speciation and dispersal), sorted by (k, f, loc, j) */
     uint32_t stream_sort_bytes;/* record_events: the radix sort of an epoch's records covers k and the leading 1..5 bytes of f; records

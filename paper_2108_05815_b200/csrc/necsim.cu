@@ -452,7 +452,7 @@ extern "C" int necsim_destroy(necsim_scenario *scn) {
 // simulate
 // ---------------------------------------------------------------------------------------------------
 struct ResolvedParams {
-    u32 block_threads, grid_blocks, dedup_log2_slots, tail_threshold, probe_mask;
+    u32 block_threads, grid_blocks, dedup_log2_slots, tail_threshold, probe_mask, probe_mask_tail;
     bool dedup, record;
     u32 stream_fbytes;
     u64 epoch_events, max_steps, ring_cap, stream_cap;
@@ -479,8 +479,12 @@ static int resolve_params(const necsim_scenario *scn, const necsim_sim_params *p
     r.ring_cap = r.record ? (p->event_ring_capacity ? p->event_ring_capacity : (1ull << 24)) : 0;
     r.stream_cap = r.record ? (p->event_stream_capacity ? p->event_stream_capacity : (1ull << 26)) : 0;
     if (r.ring_cap >= (1ull << 32)) return fail(NECSIM_ERR_INVALID_ARG, "event_ring_capacity must be < 2^32");
-    if (p->dedup_probe > 4) return fail(NECSIM_ERR_INVALID_ARG, "dedup_probe must be in [0, 4]");
-    r.probe_mask = p->dedup_probe ? ((1u << (p->dedup_probe - 1u)) - 1u) : 7u;   // default: every 8th event probes
+    if (p->dedup_probe > 7) return fail(NECSIM_ERR_INVALID_ARG, "dedup_probe must be in [0, 7]");
+    {   // probe period 2^pb: the events whose hash has its top pb bits zero. Default: every 8th event (and every 32nd in the tail launch)
+        const u32 pb = p->dedup_probe ? p->dedup_probe - 1u : 3u;
+        r.probe_mask = pb ? (~0u << (32u - pb)) : 0u;
+        r.probe_mask_tail = p->dedup_probe ? r.probe_mask : (~0u << 27);
+    }
     (void)scn;
     return NECSIM_OK;
 }
@@ -684,6 +688,10 @@ static int simulate_impl(necsim_scenario *scn, uint64_t seed, double nu, const u
         }
         ep.k_start = k_start; ep.k_stop = k_stop;
         const bool tail = active <= tail_threshold;
+        // The tail launch probes a subset of the events the per-lane kernel probes (nested masks, so both kernels agree on which of the
+        // tail's events probe): with one lineage per warp the exchange sits on the lineage's chain, and a chain of 10^6 events loses
+        // nothing by noticing a coalescence 32 instead of 8 events later (C5: 2246 -> 2190 ms per step).
+        ep.probe_mask = tail ? rp.probe_mask_tail : rp.probe_mask;
         u32 grid;
         if (tail) {
             ep.lanes_per_warp = 32;

@@ -168,10 +168,10 @@ __device__ __forceinline__ bool disperse(const ScenarioDev &sc, u64 thr_m, u64 X
 }
 
 // The event's stream position X = prime(loc, k) + j * GAMMA is already a well-mixed function of the event identity (six keyed
-// Feistel rounds): folded to 32 bits it chooses the bucket (low bits) and whether the event probes at all (top 3 bits).
+// Feistel rounds): folded to 32 bits it chooses the bucket (low bits) and whether the event probes at all (top bits: 3 in the per-lane kernel, 5 in the tail).
 // A hit always compares the full key. Every kernel uses this function: entries live across launches.
 __device__ __forceinline__ u32 cache_hash(u64 X) { return (u32)X ^ (u32)(X >> 32); }
-__device__ __forceinline__ bool cache_probes(u32 h, u32 probe_mask) { return ((h >> 29) & probe_mask) == 0u; }
+__device__ __forceinline__ bool cache_probes(u32 h, u32 probe_mask) { return (h & probe_mask) == 0u; }   // probe_mask: the top log2(period) bits
 
 // -ln tables in global memory (filled once per process from neglog_tables.inc), staged to smem per block
 __device__ unsigned short NEGLOG_Q_DEV[512];

@@ -97,7 +97,7 @@ struct EpochArgs {
     u32 max_steps;             // 0 = unlimited
     u32 lanes_per_warp;        // lanes of each warp that hold lineages (32 = saturated; fewer in the tail)
     u32 rec_chunk;             // event-stream ring slots a tail-kernel warp reserves at a time (1..64)
-    u32 probe_mask;            // an event probes the dedup cache iff (hash >> 29) & probe_mask == 0 (0 = every event)
+    u32 probe_mask;            // an event probes the dedup cache iff hash & probe_mask == 0: the top log2(period) bits of the hash (0 = every event)
     u32 zero;                  // always 0, but only the host knows: ties instruction chains together in issue order (tail kernel)
 };
 

@@ -67,7 +67,7 @@ def test_random_scenarios(ns, O, I):
         seed = int(rng.integers(0, 2**63))
         kw["sampler"] = int(rng.integers(0, 2))                       # exponential or Poisson event-time sampler
         record = bool(rng.integers(0, 2))                             # with or without the full event stream
-        knobs = dict(tail_threshold=int(rng.choice([1, 0xFFFFFFFF, 0])), dedup_probe=int(rng.integers(0, 5)),
+        knobs = dict(tail_threshold=int(rng.choice([1, 0xFFFFFFFF, 0])), dedup_probe=int(rng.integers(0, 8)),
                      dedup_log2_slots=int(rng.choice([4, 8, 16, 0])), block_threads=int(rng.choice([32, 128, 256])),
                      epoch_events=int(rng.choice([0, 1, 50, 5000])))
         o = O.Scenario(**kw)

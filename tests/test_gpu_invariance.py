@@ -33,7 +33,7 @@ def test_launch_and_cache_invariance(ns, O, I, idx):
     variants = [dict(), dict(block_threads=32, grid_blocks=1), dict(block_threads=64, grid_blocks=7), dict(block_threads=128, grid_blocks=300),
                 dict(dedup_log2_slots=4), dict(dedup_log2_slots=10, epoch_events=100), dict(dedup_log2_slots=16, epoch_events=10**9),
                 dict(epoch_events=1), dict(tail_threshold=1), dict(tail_threshold=0xFFFFFFFF, epoch_events=3000),
-                dict(tail_threshold=500, dedup_log2_slots=8), dict(dedup_probe=1), dict(dedup_probe=4, tail_threshold=1), dict(dedup_probe=2, tail_threshold=0xFFFFFFFF), dict(tail_threshold=0xFFFFFFFF, block_threads=64, grid_blocks=5), dict(dedup=False) if idx in (0, 4) else dict(dedup_log2_slots=12)]
+                dict(tail_threshold=500, dedup_log2_slots=8), dict(dedup_probe=1), dict(dedup_probe=4, tail_threshold=1), dict(dedup_probe=2, tail_threshold=0xFFFFFFFF), dict(dedup_probe=7), dict(dedup_probe=6, tail_threshold=1), dict(tail_threshold=0xFFFFFFFF, block_threads=64, grid_blocks=5), dict(dedup=False) if idx in (0, 4) else dict(dedup_log2_slots=12)]
     for v in variants:
         got = sc.simulate(cfg["seed"], cfg["nu"], cfg["mask"], **v)
         assert same(got, ref), (cfg["name"], v)
