@@ -326,8 +326,14 @@ __global__ void __launch_bounds__(256, 2) tail_kernel(const ScenarioDev sc, cons
                 // candidate's own outcome (its target location, its interval + 0..3), while the ballots pick the winner; after the vote the
                 // states come from the winner's lanes by shuffle instead of six Feistel rounds at the head of the next round's chain.
                 u64 s = prime(ep.key, loc, k + sp_dk);
+                // continuation rounds: when none of the five points of interval k looked at lies after the bound and the interval is not
+                // exhausted either (1.1 % of the events: a late bound in a new stream with many early points), the next round looks at the
+                // following five points, j0 + 1 .. j0 + 5, with the partial sum a0 carried over, instead of falling back to the exact path
+                u32 j0 = 0;
+                float a0 = 0.0f;
+                u64 cand_add = sp_cand_add;
                 for (;;) {
-                    const u64 X = s + sp_cand_add;
+                    const u64 X = s + cand_add;
                     u64 ua, ub;
                     hashF2((X ^ NS_L_DISP) + sp_a_add, X ^ sp_b_xor, ua, ub);
                     // duplicate check of the candidate, decided per lane ahead of the selection: whether its event probes the cache, and where.
@@ -344,6 +350,7 @@ __global__ void __launch_bounds__(256, 2) tail_kernel(const ScenarioDev sc, cons
                     // (the draw is tied to the target cell of slot A by an OR with zero: the table gathers, which have the longest latency,
                     // are then issued before this chain starts)
                     float a = sp_q == 0u ? approx_exp_time(ubh | (c2o & ep.zero), ln2_over_mu) : 0.0f;
+                    if (lane == 0) a += a0;
                     // (the partial sums are tied to the gathered table entry by an OR with zero: ptxas otherwise places the gather, whose
                     // consumers come late, behind the whole shuffle / compare / ballot chain, and its latency ends up on the lineage's chain
                     // instead of under it. With the tie the gather is issued first and the logarithms run while it is in flight.)
@@ -363,7 +370,7 @@ __global__ void __launch_bounds__(256, 2) tail_kernel(const ScenarioDev sc, cons
                     bool aft = a > fa_last + mc, bef = a < fa_last - mc;
                     // a lineage that stayed where it was (self-dispersal) sees the points of the same stream again: after the last event
                     // means a larger ordinal, exactly (the partial sums are the same numbers as in the round before)
-                    if (loc == e_loc && fa_last >= 0.0f) { aft = sp_c + 1u > e_j; bef = !aft; }
+                    if (loc == e_loc && fa_last >= 0.0f) { aft = j0 + sp_c + 1u > e_j; bef = !aft; }
                     const bool kvalid = (ep.k_stop - k) > sp_dk;              // never look at or past the horizon (k < k_stop here)
                     // draws with hi < 2^20 (coarse logarithm) or hi >= 2^32 - 2^8 (an increment that may round to zero) are not decided here
                     const bool amb = (ubh - (1u << 20) >= 0xFFEFFF00u) || !(ins || outs) || (sp_in_k && !(aft || bef));
@@ -392,11 +399,19 @@ __global__ void __launch_bounds__(256, 2) tail_kernel(const ScenarioDev sc, cons
                     const u32 steps_e = steps_all + 1u;                 // step count after this event
                     // clean: a winner, no trouble at the time lanes or in the winner's lanes, an attempt accepted, no speciation, no step cap
                     const bool clean = wm != 0u && ((trm & 0x11111111u) | (badm & q4) | spec_w) == 0u && (okm & q4) != 0u && steps_e < cap_at;
-                    if (!clean) break;                 // warp-uniform: every term comes out of a ballot or is lineage state
+                    if (!clean) {                      // warp-uniform: every term comes out of a ballot or is lineage state
+                        if (wm == 0u && (crm & kmask) == 0u && (trm & 0x11111111u) == 0u && j0 < 25u) {   // continuation round (see above)
+                            a0 = __shfl_sync(NS_FULL, a, (int)(4u * (NS_SPEC_NJ - 1u)));
+                            j0 += NS_SPEC_NJ;
+                            if (sp_in_k) cand_add += (u64)NS_SPEC_NJ * NS_GAMMA;
+                            continue;
+                        }
+                        break;
+                    }
                     // commit: event (loc, k2, j2) executed, the lineage moves to the winner's target
                     const u32 wc = wl >> 2;
                     const u32 k2 = k + (wc < NS_SPEC_NJ ? 0u : wc - NS_SPEC_NJ + 1u);
-                    const u32 j2 = wc < NS_SPEC_NJ ? wc + 1u : 1u;
+                    const u32 j2 = wc < NS_SPEC_NJ ? j0 + wc + 1u : 1u;
                     const u32 loc2 = __shfl_sync(NS_FULL, loc2q, (int)wl), cell2 = __shfl_sync(NS_FULL, cq, (int)wl);
                     const float a_w = __shfl_sync(NS_FULL, a, (int)wl);
                     if (KIND == 3) w_resamples += (u32)first_bit((okm >> wl) & 15u);
@@ -414,6 +429,7 @@ __global__ void __launch_bounds__(256, 2) tail_kernel(const ScenarioDev sc, cons
                     }
                     k = k2; loc = loc2; cell = cell2;
                     s = __shfl_sync(NS_FULL, s_own, (int)(wl + sp_dk));
+                    if (j0) { j0 = 0; a0 = 0.0f; cand_add = sp_cand_add; }
                 }
                 steps = steps_all;
                 if (DEDUP && lpend) {          // hand the pending check over to the general code, which keeps the result in lane 0
