@@ -398,7 +398,10 @@ __global__ void __launch_bounds__(256, 2) tail_kernel(const ScenarioDev sc, cons
                     const u32 spec_w = (KIND == 1 && cell == 0) ? 0u : ((bm >> wl) & 2u);
                     const u32 steps_e = steps_all + 1u;                 // step count after this event
                     // clean: a winner, no trouble at the time lanes or in the winner's lanes, an attempt accepted, no speciation, no step cap
-                    const bool clean = wm != 0u && ((trm & 0x11111111u) | (badm & q4) | spec_w) == 0u && (okm & q4) != 0u && steps_e < cap_at;
+                    // (an undetermined target matters only up to the winner's first accepted attempt -- later attempts are never looked at:
+                    // x ^ (x - 1) = the bits up to and including the lowest set bit of x)
+                    const u32 okw = okm & q4;
+                    const bool clean = wm != 0u && ((trm & 0x11111111u) | (badm & q4 & (okw ^ (okw - 1u))) | spec_w) == 0u && okw != 0u && steps_e < cap_at;
                     if (!clean) {                      // warp-uniform: every term comes out of a ballot or is lineage state
                         if (wm == 0u && (crm & kmask) == 0u && (trm & 0x11111111u) == 0u && j0 < 25u) {   // continuation round (see above)
                             a0 = __shfl_sync(NS_FULL, a, (int)(4u * (NS_SPEC_NJ - 1u)));
