@@ -332,6 +332,12 @@ __global__ void __launch_bounds__(256, 2) tail_kernel(const ScenarioDev sc, cons
                 u32 j0 = 0;
                 float a0 = 0.0f;
                 u64 cand_add = sp_cand_add;
+                // attempt round (after the loop): the event is known and everything about it is settled except that its first four dispersal
+                // attempts were all rejected (1.4 % of the events of C5's tail: lineages in sparsely inhabited neighbourhoods)
+                bool rs = false;
+                u32 rs_k2 = 0, rs_j2 = 0, rs_xlo = 0, rs_xhi = 0;
+                u64 rs_X = 0;
+                float rs_a = 0.0f;
                 for (;;) {
                     const u64 X = s + cand_add;
                     u64 ua, ub;
@@ -409,6 +415,13 @@ __global__ void __launch_bounds__(256, 2) tail_kernel(const ScenarioDev sc, cons
                             if (sp_in_k) cand_add += (u64)NS_SPEC_NJ * NS_GAMMA;
                             continue;
                         }
+                        if (KIND == 3 && wm != 0u && ((trm & 0x11111111u) | (badm & q4) | spec_w | okw) == 0u && steps_e < cap_at) {
+                            const u32 wc = wl >> 2;
+                            rs = true;
+                            rs_k2 = k + (wc < NS_SPEC_NJ ? 0u : wc - NS_SPEC_NJ + 1u); rs_j2 = wc < NS_SPEC_NJ ? j0 + wc + 1u : 1u;
+                            rs_X = __shfl_sync(NS_FULL, X, (int)wl); rs_a = __shfl_sync(NS_FULL, a, (int)wl);
+                            rs_xlo = __shfl_sync(NS_FULL, (u32)ub, (int)(wl + 2u)); rs_xhi = __shfl_sync(NS_FULL, ubh, (int)(wl + 2u));
+                        }
                         break;
                     }
                     // commit: event (loc, k2, j2) executed, the lineage moves to the winner's target
@@ -440,6 +453,35 @@ __global__ void __launch_bounds__(256, 2) tail_kernel(const ScenarioDev sc, cons
                     pold_lo = __shfl_sync(NS_FULL, pold_lo, (int)p_lane); pold_hi = __shfl_sync(NS_FULL, pold_hi, (int)p_lane);
                 }
                 p_lane = 0u;
+                if (KIND == 3 && rs) {
+                    // the 32 lanes evaluate attempts 4 .. 35 of the event (loc, rs_k2, rs_j2): one hash, the lookups and the gather, instead of
+                    // the exact path. (The pending duplicate check, if any, was clear in the round that found the event: resolved first.)
+                    const u64 ua2 = hashF((rs_X ^ NS_L_DISP) + (u64)(4u + lane) * NS_GAMMA);
+                    u32 loc2b, c2b, tieb; uint2 csb = make_uint2(Cm, sh); bool accb, badb;
+                    fast_slot_a<KIND, PERCELL, COMPACT>(sc, gl, 0u, lane, 0u, cell, rs_k2, ua2, rs_xlo, rs_xhi, loc2b, c2b, csb, accb, badb, tieb);
+                    const u32 okb = __ballot_sync(NS_FULL, accb), bdb = __ballot_sync(NS_FULL, badb);
+                    const u32 fa = (u32)first_bit(okb | 0x80000000u);
+                    if (okb != 0u && (bdb & ((2u << fa) - 1u)) == 0u) {
+                        if (resolve_pending()) break;
+                        bool probes = false;
+                        if (DEDUP) {
+                            const u32 h = cache_hash(rs_X);
+                            probes = cache_probes(h, ep.probe_mask);
+                            atomic_exch_128_if(probes && lane == 0, &bf.cache[h & bf.cache_mask], make_uint4(loc, rs_k2, rs_j2, id), pold_lo, pold_hi);
+                            if (probes) { p_loc = loc; p_k = rs_k2; p_j = rs_j2; p_T_known = false; pend = true; }
+                        }
+                        if (!probes) steps++;
+                        w_resamples += 4u + fa;
+                        e_loc = loc; e_j = rs_j2; e_Cm = Cm; e_sh = sh; f_exact = false; fa_last = rs_a; fm_last = margin;
+                        if (PERCELL) {
+                            Cm = __shfl_sync(NS_FULL, csb.x, (int)fa); sh = __shfl_sync(NS_FULL, csb.y, (int)fa);
+                            const float finv = rate_to_float(Cm, sh);
+                            ln2_over_mu = NS_LN2F * finv; margin = NS_MARGIN * (1.0f + finv);
+                        }
+                        k = rs_k2; loc = __shfl_sync(NS_FULL, loc2b, (int)fa); cell = __shfl_sync(NS_FULL, c2b, (int)fa);
+                        continue;
+                    }
+                }
                 // the round that was not clean is done below in exact arithmetic, from the exact lower bound
                 if (!f_exact) { f_last = (i64)exact_offset(ep.key, smt, e_loc, k, e_j, e_Cm, e_sh); f_exact = true; }
                 c_exact++;
