@@ -332,9 +332,10 @@ __global__ void __launch_bounds__(256, 2) tail_kernel(const ScenarioDev sc, cons
                 u32 j0 = 0;
                 float a0 = 0.0f;
                 u64 cand_add = sp_cand_add;
-                // attempt round (after the loop): the event is known and everything about it is settled except that its first four dispersal
-                // attempts were all rejected (1.4 % of the events of C5's tail: lineages in sparsely inhabited neighbourhoods)
-                bool rs = false;
+                // attempt round (after the loop): the event is known and everything about it is settled except its dispersal: the first four
+                // attempts were all rejected (1.4 % of the events of C5's tail: lineages in sparsely inhabited neighbourhoods), or a target at
+                // or before the first accepted attempt fell into a crowded bucket of the rounded-normal guide (0.2 %)
+                bool rs = false, rs_rej = false;   // rs_rej: four determined attempts, all rejected -> attempts 4..35 with the fast lookup
                 u32 rs_k2 = 0, rs_j2 = 0, rs_xlo = 0, rs_xhi = 0;
                 u64 rs_X = 0;
                 float rs_a = 0.0f;
@@ -415,9 +416,11 @@ __global__ void __launch_bounds__(256, 2) tail_kernel(const ScenarioDev sc, cons
                             if (sp_in_k) cand_add += (u64)NS_SPEC_NJ * NS_GAMMA;
                             continue;
                         }
-                        if (KIND == 3 && wm != 0u && ((trm & 0x11111111u) | (badm & q4) | spec_w | okw) == 0u && steps_e < cap_at) {
+                        // (here with a winner, no ambiguity, no duplicate, no speciation: what is wrong is the winner's dispersal -- four
+                        // attempts rejected, or an undetermined target at or before the first accepted one)
+                        if (KIND == 3 && wm != 0u && ((trm & 0x11111111u) | spec_w) == 0u && steps_e < cap_at) {
                             const u32 wc = wl >> 2;
-                            rs = true;
+                            rs = true; rs_rej = okw == 0u && (badm & q4) == 0u;
                             rs_k2 = k + (wc < NS_SPEC_NJ ? 0u : wc - NS_SPEC_NJ + 1u); rs_j2 = wc < NS_SPEC_NJ ? j0 + wc + 1u : 1u;
                             rs_X = __shfl_sync(NS_FULL, X, (int)wl); rs_a = __shfl_sync(NS_FULL, a, (int)wl);
                             rs_xlo = __shfl_sync(NS_FULL, (u32)ub, (int)(wl + 2u)); rs_xhi = __shfl_sync(NS_FULL, ubh, (int)(wl + 2u));
@@ -454,14 +457,30 @@ __global__ void __launch_bounds__(256, 2) tail_kernel(const ScenarioDev sc, cons
                 }
                 p_lane = 0u;
                 if (KIND == 3 && rs) {
-                    // the 32 lanes evaluate attempts 4 .. 35 of the event (loc, rs_k2, rs_j2): one hash, the lookups and the gather, instead of
-                    // the exact path. (The pending duplicate check, if any, was clear in the round that found the event: resolved first.)
-                    const u64 ua2 = hashF((rs_X ^ NS_L_DISP) + (u64)(4u + lane) * NS_GAMMA);
-                    u32 loc2b, c2b, tieb; uint2 csb = make_uint2(Cm, sh); bool accb, badb;
-                    fast_slot_a<KIND, PERCELL, COMPACT>(sc, gl, 0u, lane, 0u, cell, rs_k2, ua2, rs_xlo, rs_xhi, loc2b, c2b, csb, accb, badb, tieb);
-                    const u32 okb = __ballot_sync(NS_FULL, accb), bdb = __ballot_sync(NS_FULL, badb);
-                    const u32 fa = (u32)first_bit(okb | 0x80000000u);
-                    if (okb != 0u && (bdb & ((2u << fa) - 1u)) == 0u) {
+                    // the 32 lanes evaluate attempts 0 .. 31 of the event (loc, rs_k2, rs_j2) with the exact rounded-normal lookup: one hash,
+                    // the lookups and the gather, instead of the exact path. (The pending duplicate check, if any, was clear in the round
+                    // that found the event: it is resolved first.)
+                    u32 c2b, loc2b, okb, fa, nres;
+                    uint2 csb = make_uint2(Cm, sh);
+                    if (rs_rej) {
+                        const u64 ua2 = hashF((rs_X ^ NS_L_DISP) + (u64)(4u + lane) * NS_GAMMA);
+                        u32 tieb; bool accb, badb;
+                        fast_slot_a<KIND, PERCELL, COMPACT>(sc, gl, 0u, lane, 0u, cell, rs_k2, ua2, rs_xlo, rs_xhi, loc2b, c2b, csb, accb, badb, tieb);
+                        okb = __ballot_sync(NS_FULL, accb);
+                        const u32 bdb = __ballot_sync(NS_FULL, badb);
+                        fa = (u32)first_bit(okb | 0x80000000u);
+                        if (bdb & ((2u << fa) - 1u)) okb = 0u;          // an undetermined target at or before the first accepted: exact path
+                        nres = 4u + fa;
+                    } else {
+                        const u64 ua2 = hashF((rs_X ^ NS_L_DISP) + (u64)lane * NS_GAMMA);
+                        u32 db, pfb; bool badb;
+                        gauss_target<PERCELL, SAMP, COMPACT, false>(sc, gl, cell & 0xFFFFu, cell >> 16, ua2, rs_k2, c2b, db, pfb, csb, badb);
+                        loc2b = pfb + ((db == 1u) ? 0u : mulhi64_u32_parts(rs_xlo, rs_xhi, db));
+                        okb = __ballot_sync(NS_FULL, db > 0u);
+                        fa = (u32)first_bit(okb | 0x80000000u);
+                        nres = fa;
+                    }
+                    if (okb != 0u) {
                         if (resolve_pending()) break;
                         bool probes = false;
                         if (DEDUP) {
@@ -471,7 +490,7 @@ __global__ void __launch_bounds__(256, 2) tail_kernel(const ScenarioDev sc, cons
                             if (probes) { p_loc = loc; p_k = rs_k2; p_j = rs_j2; p_T_known = false; pend = true; }
                         }
                         if (!probes) steps++;
-                        w_resamples += 4u + fa;
+                        w_resamples += nres;
                         e_loc = loc; e_j = rs_j2; e_Cm = Cm; e_sh = sh; f_exact = false; fa_last = rs_a; fm_last = margin;
                         if (PERCELL) {
                             Cm = __shfl_sync(NS_FULL, csb.x, (int)fa); sh = __shfl_sync(NS_FULL, csb.y, (int)fa);
