@@ -268,6 +268,7 @@ __device__ __noinline__ u64 exact_offset_of_loc_nl(SeedKey key, u32 q_addr, u32 
 #define NS_PHASE_WE 1u
 #define NS_PHASE_WS 1u
 #endif
+#define NS_COOP_LANES 8u       // cooperative resampling when a warp of an exhausted queue holds at most this many lineages
 #define NS_ST_IDLE 0u
 #define NS_ST_SEARCH 1u     // needs draws of the event-time search (re-primes first when `need_prime`)
 #define NS_ST_EVENT 2u      // event (loc, k, j) found at offset T: `att` dispersal attempts rejected so far
@@ -492,6 +493,49 @@ __global__ void __launch_bounds__(256) simulate_kernel(const ScenarioDev sc, con
                 } else {
                     c_resamples++;
                     if (++att >= NS_MAX_RESAMPLE) { atomicMax(&bf.ctr->error, 3u); st = NS_ST_IDLE; }
+                }
+            }
+        }
+        if (KIND == 3 && !REC && exhausted && n_search + n_event <= NS_COOP_LANES) {
+            // Cooperative resampling at the ragged end of an epoch: the queue is empty and this warp holds only a few lineages. One that
+            // has just had a dispersal attempt rejected (a sparsely inhabited neighbourhood: tens of attempts per event, one pass each)
+            // gets its next 32 attempts evaluated by the whole warp. Same draws, same first accepted attempt (R16): identical results.
+            u32 em = __ballot_sync(NS_FULL, st == NS_ST_EVENT && att >= 1u);
+            while (em) {
+                const int L = __ffs(em) - 1;
+                em &= em - 1u;
+                const u64 bX = __shfl_sync(NS_FULL, X, L);
+                const u32 bcell = __shfl_sync(NS_FULL, cell, L), batt = __shfl_sync(NS_FULL, att, L), bk = __shfl_sync(NS_FULL, k, L);
+                const u64 x = draw_disp(bX, batt + lane);
+                const u32 xx = wrap_add(bcell & 0xFFFFu, gauss_disp(gl, (u32)(x >> 32)), sc.width);
+                const u32 yy = wrap_add(bcell >> 16, gauss_disp(gl, (u32)x), sc.height);
+                u32 d, pfx;
+                if (COMPACT) {
+                    const uint2 hb = __ldg(&sc.hab64[hab64_index(sc, xx, yy)]);
+                    const u32 bit = 1u << (xx & 31u);
+                    d = (hb.x & bit) ? sc.compact_deme : 0u;
+                    pfx = hb.y + sc.compact_deme * (u32)__popc(hb.x & (bit - 1u));
+                } else {
+                    d = cell_deme_at(sc, yy * sc.width + xx, bk);
+                    pfx = d ? cell_prefix(sc, yy * sc.width + xx) : 0u;
+                }
+                const u32 okm = __ballot_sync(NS_FULL, d > 0u);
+                const int fa = okm ? __ffs(okm) - 1 : 0;
+                const u32 d_f = __shfl_sync(NS_FULL, d, fa), pfx_f = __shfl_sync(NS_FULL, pfx, fa), c2_f = __shfl_sync(NS_FULL, (yy << 16) | xx, fa);
+                if ((int)lane == L) {
+                    if (okm) {
+                        c_resamples += (u32)fa;
+                        loc = pfx_f + ((d_f == 1u) ? 0u : mulhi64_u32(draw_index(X), d_f)); cell = c2_f; need_prime = true; st = NS_ST_SEARCH;
+                        if (ep.max_steps && steps >= ep.max_steps) {
+                            if (FILT) T = exact_offset_nl(ep.key, smt.q, smt.a, e_loc, k, j, Cm, sh);   // (Cm, sh) are still the origin's
+                            bf.state[id] = 3;
+                            bf.term_loc[id] = loc; bf.term_k[id] = k; bf.term_j[id] = j; bf.term_f[id] = T; bf.steps[id] = steps;
+                            st = NS_ST_IDLE;
+                        }
+                    } else {
+                        c_resamples += 32u; att += 32u;
+                        if (att >= NS_MAX_RESAMPLE) { atomicMax(&bf.ctr->error, 3u); st = NS_ST_IDLE; }
+                    }
                 }
             }
         }

@@ -24,7 +24,13 @@
 // While the gathers are in flight the warp computes the logarithms and the partial sums; two ballots pick the event, a third
 // the first accepted attempt among the winner's four lanes. The critical path of an event is prime -> hash -> max(gather,
 // logarithm + scan) -> select instead of prime -> hash -> logarithm -> scan -> select -> hash -> gather -> select.
-// A candidate outside the set, or four rejected attempts, falls back to the general code below (identical results).
+// While the ballots pick the winner, every candidate's lanes already prime the stream states of the NEXT round from the candidate's own
+// outcome; after the commit they come from the winner's lanes by shuffle. Rounds that are not clean but common are handled without the
+// exact path: the first five points all before the bound -> a continuation round over the next five (partial sum carried over); the
+// winner's dispersal unsettled (four attempts rejected, or an undetermined target at or before the first accepted one) -> an attempt
+// round after the loop that puts 32 attempts of the known event on the lanes. Everything else (ambiguous comparisons, a duplicate, a
+// speciation, the step cap, three empty intervals in a row: 0.6 % of the events of C5's tail) falls back to the general code below,
+// which recomputes the exact lower bound from the last event's identity (identical results).
 #pragma once
 #include "sim_kernel.cuh"
 
