@@ -276,7 +276,7 @@ __device__ __noinline__ u64 exact_offset_of_loc_nl(SeedKey key, u32 q_addr, u32 
 // SAMP: 0 = exponential event-time sampler, 1 = Poisson / order statistics (2.7)
 // REC: also append every executed event to the stream ring (NEXT-3)
 template <int KIND, bool DEDUP, bool PERCELL, int SAMP, bool REC, bool COMPACT>
-__global__ void __launch_bounds__(256) simulate_kernel(const ScenarioDev sc, const SimBuffers bf, const EpochArgs ep) {
+__global__ void __launch_bounds__(256, 5) simulate_kernel(const ScenarioDev sc, const SimBuffers bf, const EpochArgs ep) {
     __shared__ unsigned short sQ[SAMP == 0 ? 512 : 256];      // SAMP 1: the Poisson guide
     __shared__ u64 sA[SAMP == 0 ? 512 : 256];                 // SAMP 1: the Poisson cdf thresholds
     __shared__ u32 sG[KIND == 3 ? 1024 : 1];
